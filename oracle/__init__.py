@@ -1,0 +1,2 @@
+"""fp64 CPU oracle for MSA -- test infrastructure only (see msa_oracle.c header)."""
+from .msa_oracle import build, forward, forward_problem, num_threads  # noqa: F401
