@@ -1,0 +1,194 @@
+/*
+ * msa.h -- C ABI of the B200-native Multi-Segment Attention (MSA) library (libmsa.so).
+ *
+ * MSA (arxiv/paper_2606_02964, section 4.1) computes exact causal
+ * attention for runs of query tokens against a logically contiguous KV context that is
+ * physically split into several segments.  Definition of the result, per query row i of a
+ * run (absolute position p_i = q_abs_start + i) and q head h (KV head kvh = map[h]):
+ *
+ *     keys    = every token j of every segment of the run's segment list, at absolute
+ *               position a_j = seg.abs_start + (index of the token in its segment)
+ *     visible = { j : a_j <= p_i }                       (causal by absolute position)
+ *     s_j     = softmax_scale * <q[i][h][:], K_j[kvh][:]>
+ *     LSE     = ln sum_{visible} exp(s_j)                (natural log)
+ *     O[d]    = sum_{visible} exp(s_j - LSE) * V_j[kvh][d]
+ *     no visible key  =>  O = 0, LSE = -inf
+ *
+ * This is Eq. (1) (A = QK^T/sqrt(d_k), O = softmax(A)V) applied the way
+ * Eq. (2) states it for several runs: each run attends to everything
+ * that precedes it, cached or recomputed (Eq. (4)'s l1,q1,l2,q2 layout);
+ * "only the attention module requires the token dependency information" and
+ * one launch serves "any number of non-contiguous cache segments" of many requests
+ * (PAPER.md:124).  Precision: bf16 q/k/v, fp32 accumulation, bf16 O, fp32 LSE.
+ *
+ * All pointers named "device" are CUDA device pointers on the handle's device; all others
+ * are host pointers.  The library never takes ownership of caller memory.  No torch types
+ * appear here; PyTorch (or anything else) only supplies device memory and a cudaStream_t.
+ * Every call returns an int status (MSA_OK == 0, errors negative); nothing throws or aborts.
+ */
+#ifndef MSA_H_
+#define MSA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MSA_BLOCK_SIZE 16          /* tokens per paged KV block */
+#define MSA_MAX_GROUP 16           /* max q heads per KV head */
+
+enum {
+    MSA_OK = 0,
+    MSA_ERR_INVALID_ARG = -1,      /* NULL pointer, negative size, non-positive / non-finite scale */
+    MSA_ERR_UNSUPPORTED = -2,      /* head_dim not in {64,128}, block_size != 16, Hq % Hkv != 0, G > 16,
+                                      head map that does not give every KV head exactly G q heads */
+    MSA_ERR_OVERLAP = -3,          /* segments of one request overlap in absolute position, or two
+                                      requests write the same q rows */
+    MSA_ERR_UNSORTED = -4,         /* segments of one request not in ascending abs_start */
+    MSA_ERR_OUT_OF_RANGE = -5,     /* descriptor refers outside the extents given to msa_forward */
+    MSA_ERR_MISALIGNED = -6,       /* device pointer not 16-byte aligned */
+    MSA_ERR_WORKSPACE = -7,        /* workspace NULL / too small */
+    MSA_ERR_CUDA = -8,             /* a CUDA runtime / driver call failed (see msa_last_cuda_error) */
+    MSA_ERR_NO_DEVICE = -9         /* no CUDA device, or the device is not sm_100 */
+};
+
+/* Segment kinds (BASELINE.json north_star):
+ *   PAGED  -- cached tokens in 16-token blocks of the pool, reached through block_table
+ *   CONTIG -- a run just recomputed into the contiguous arena
+ *   SELF   -- the current chunk's own K/V, also rows of the contiguous arena           */
+enum { MSA_SEG_PAGED = 0, MSA_SEG_CONTIG = 1, MSA_SEG_SELF = 2 };
+
+typedef struct {
+    int32_t num_q_heads;           /* Hq                                                     */
+    int32_t num_kv_heads;          /* Hkv, divides Hq; G = Hq/Hkv <= 16                      */
+    int32_t head_dim;              /* D in {64, 128}                                         */
+    int32_t block_size;            /* must be 16                                             */
+    const int32_t *q_to_kv_head;   /* host int32[Hq] GQA head map, or NULL => h / G (Llama)  */
+    int32_t device;                /* CUDA device ordinal                                    */
+} msa_config;
+
+typedef struct {
+    int32_t kind;                  /* MSA_SEG_*                                              */
+    int32_t abs_start;             /* absolute position of the segment's first token, >= 0   */
+    int32_t len;                   /* tokens, >= 1; the last paged block may be partly filled */
+    int32_t block_off;             /* PAGED: index into block_table of the segment's first
+                                      block; token idx lives in block block_table[block_off +
+                                      idx/16], slot idx%16 (a PAGED segment starts at slot 0) */
+    int64_t row_off;               /* CONTIG/SELF: arena row of the segment's first token     */
+} msa_segment;
+
+typedef struct {
+    int32_t q_row_start;           /* first row of q / o / lse of this query run             */
+    int32_t q_len;                 /* rows (tokens) of the run, >= 0                         */
+    int32_t q_abs_start;           /* absolute position of the run's first token             */
+    int32_t seg_begin, seg_count;  /* slice of the segment array this run attends to;
+                                      several runs may share one slice (hybrid chunks,
+                                      PAPER.md:92 step 5, :247).  Ascending abs_start, no
+                                      overlap; gaps are legal (attention over the union).    */
+} msa_request;
+
+typedef struct {
+    int32_t num_ctas;              /* persistent CTAs the forward kernel is launched with    */
+    int32_t num_items;             /* (run, kv-head, q-tile) work items                      */
+    int32_t num_units;             /* (item, kv-tile-range) units after split-KV             */
+    int32_t num_split_items;       /* items whose KV range was split (need the merge kernel) */
+    int32_t num_partials;          /* partial (O, LSE) results written to the workspace      */
+    int32_t rows_per_tile;         /* packed (token, q-head) rows per 128-row MMA tile used  */
+    int64_t kv_tiles;              /* total 128-key tiles visited                            */
+    int64_t visible_pairs;         /* sum over rows of visible keys, per q head              */
+    int64_t max_block_table_index; /* extents the plan needs at msa_forward                  */
+    int64_t max_contig_row;
+    int64_t max_q_row;
+} msa_plan_info;
+
+typedef struct msa_handle_s *msa_handle;
+typedef struct msa_plan_s *msa_plan;
+
+/*
+ * Create a handle for one model shape on one device.  Owns only small host state and a
+ * few KB of device memory.  Fails with MSA_ERR_NO_DEVICE when there is no sm_100 GPU:
+ * there is no CPU fallback.  cfg->device < 0 makes a planning-only handle (descriptor
+ * validation and scheduling on the host, for tools and tests); msa_forward on it returns
+ * MSA_ERR_NO_DEVICE.
+ */
+int msa_create(const msa_config *cfg, msa_handle *out);
+void msa_destroy(msa_handle h);
+
+/* Build the launch plan for a batch of query runs (host arrays, copied; may be freed after
+ * the call).  This is the paper's attention metadata -- "split indices" and the per-token-
+ * block "equivalent seq_len" array -- plus the persistent tile schedule
+ * and split-KV decisions.  All descriptor validation happens here.  The plan depends only
+ * on lengths and residency, not on tensor values or block ids, so one plan serves every
+ * layer of a model step.  Owns a small device buffer; uploads it synchronously. */
+int msa_plan_create(msa_handle h, const msa_request *requests, int32_t n_req,
+                    const msa_segment *segments, int32_t n_seg, msa_plan *out);
+void msa_plan_destroy(msa_plan p);
+int msa_plan_get_info(msa_plan p, msa_plan_info *info);
+
+/* Introspection (tests, tools): copy one of the plan's host-side arrays out.
+ *   which = 0  virtual blocks      int32[4]  {src, abs_start, nvalid, paged}
+ *           1  work units          int32[12] {q_row0, n_tok, q_abs0, kvh, vb_begin, vb_count,
+ *                                             tile_begin, tile_end, partial_off, 0, 0, 0}
+ *           2  cta_unit_begin      int32     [num_ctas + 1]
+ *           3  merge items         {int32 q_row0, n_tok, kvh, n_partials; int64 first_off, stride}
+ * With buf == NULL only *bytes is set; otherwise *bytes is the capacity on entry. */
+int msa_plan_export(msa_plan p, int which, void *buf, size_t *bytes);
+
+/* Bytes of device scratch msa_forward needs for this plan (split-KV partials); may be 0. */
+int msa_workspace_bytes(msa_plan p, size_t *bytes);
+
+/* One MSA forward pass, asynchronous on `cuda_stream` (a cudaStream_t; NULL = default
+ * stream).  Never allocates, never synchronises, never reads device memory on the host.
+ *
+ *   q            device bf16 [total_q][Hq][D]
+ *   pool_k/v     device bf16 [num_blocks][16][Hkv][D]      (paged KV cache)
+ *   block_table  device int32 [block_table_len], physical block ids in logical order
+ *   contig_k/v   device bf16 [contig_rows][Hkv][D]         (recomputed runs + own chunk)
+ *   o            device bf16 [total_q][Hq][D]   (written for every row of every run)
+ *   lse          device fp32 [total_q][Hq]      (natural log; -inf for rows with no key)
+ *   workspace    device, >= msa_workspace_bytes(), 16-byte aligned; may be NULL if 0 bytes
+ *
+ * Rows of q/o/lse not covered by any run are left untouched.  pool/contig pointers may be
+ * NULL when the plan references no segment of that kind.  Block ids are trusted (they live
+ * on the device); slots past a segment's length and unused blocks may hold anything,
+ * including NaN: they never reach O. */
+int msa_forward(msa_handle h, msa_plan p,
+                const void *q, int64_t total_q,
+                const void *pool_k, const void *pool_v, int64_t num_blocks,
+                const int32_t *block_table, int64_t block_table_len,
+                const void *contig_k, const void *contig_v, int64_t contig_rows,
+                float softmax_scale,
+                void *o, float *lse,
+                void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* End-to-end convenience call with HOST buffers for everything a serving step produces:
+ * q, the block table, the contiguous arena (recomputed runs + own chunk) come from host
+ * memory and O / LSE go back to host memory; the paged pool is the resident KV cache and
+ * stays a device pointer.  Copies are issued on `cuda_stream` around the same kernels as
+ * msa_forward, using staging buffers owned by the handle (grown on demand, so the first
+ * call may allocate); the call returns after the results have landed (it synchronises the
+ * stream).  Host buffers should be pinned for full PCIe speed but need not be.  All total_q
+ * rows of o_host / lse_host are overwritten; rows not covered by any run hold unspecified
+ * values. */
+int msa_forward_host(msa_handle h, msa_plan p,
+                     const void *q_host, int64_t total_q,
+                     const void *pool_k, const void *pool_v, int64_t num_blocks,
+                     const int32_t *block_table_host, int64_t block_table_len,
+                     const void *contig_k_host, const void *contig_v_host, int64_t contig_rows,
+                     float softmax_scale,
+                     void *o_host, float *lse_host, void *cuda_stream);
+
+/* Number of kernels the last msa_forward / msa_forward_host on this handle launched. */
+int msa_last_launch_count(msa_handle h);
+
+const char *msa_strerror(int status);
+/* Text of the last CUDA error seen by this thread inside the library ("" if none). */
+const char *msa_last_cuda_error(void);
+const char *msa_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MSA_H_ */

@@ -1,0 +1,251 @@
+"""Thin ctypes binding of libmsa.so -- same names as include/msa.h, argument marshalling only.
+
+Every step of the hot path runs inside the library's CUDA kernels.  PyTorch appears only as
+the owner of device memory and streams (``tensor.data_ptr()``, ``torch.cuda.current_stream``).
+There is no fallback: if libmsa.so is missing or no sm_100 GPU is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Dict, Optional, Tuple
+
+import numpy as np
+
+from ._build import LIB_PATH
+
+MSA_OK = 0
+MSA_ERR_INVALID_ARG, MSA_ERR_UNSUPPORTED, MSA_ERR_OVERLAP, MSA_ERR_UNSORTED = -1, -2, -3, -4
+MSA_ERR_OUT_OF_RANGE, MSA_ERR_MISALIGNED, MSA_ERR_WORKSPACE, MSA_ERR_CUDA, MSA_ERR_NO_DEVICE = -5, -6, -7, -8, -9
+MSA_SEG_PAGED, MSA_SEG_CONTIG, MSA_SEG_SELF = 0, 1, 2
+
+
+class MsaConfig(ctypes.Structure):
+    _fields_ = [("num_q_heads", ctypes.c_int32), ("num_kv_heads", ctypes.c_int32), ("head_dim", ctypes.c_int32),
+                ("block_size", ctypes.c_int32), ("q_to_kv_head", ctypes.POINTER(ctypes.c_int32)),
+                ("device", ctypes.c_int32)]
+
+
+class MsaSegment(ctypes.Structure):
+    _fields_ = [("kind", ctypes.c_int32), ("abs_start", ctypes.c_int32), ("len", ctypes.c_int32),
+                ("block_off", ctypes.c_int32), ("row_off", ctypes.c_int64)]
+
+
+class MsaRequest(ctypes.Structure):
+    _fields_ = [("q_row_start", ctypes.c_int32), ("q_len", ctypes.c_int32), ("q_abs_start", ctypes.c_int32),
+                ("seg_begin", ctypes.c_int32), ("seg_count", ctypes.c_int32)]
+
+
+class MsaPlanInfo(ctypes.Structure):
+    _fields_ = [("num_ctas", ctypes.c_int32), ("num_items", ctypes.c_int32), ("num_units", ctypes.c_int32),
+                ("num_split_items", ctypes.c_int32), ("num_partials", ctypes.c_int32),
+                ("rows_per_tile", ctypes.c_int32), ("kv_tiles", ctypes.c_int64), ("visible_pairs", ctypes.c_int64),
+                ("max_block_table_index", ctypes.c_int64), ("max_contig_row", ctypes.c_int64),
+                ("max_q_row", ctypes.c_int64)]
+
+
+class MsaError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        lib = _lib()
+        msg = lib.msa_strerror(status).decode()
+        cuda = lib.msa_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg} ({status})" + (f" [{cuda}]" if cuda and status == MSA_ERR_CUDA else ""))
+        self.status = status
+
+
+_LIB: Optional[ctypes.CDLL] = None
+
+EXPORTS = ["msa_create", "msa_destroy", "msa_plan_create", "msa_plan_destroy", "msa_plan_get_info",
+           "msa_plan_export", "msa_workspace_bytes", "msa_forward", "msa_forward_host",
+           "msa_last_launch_count", "msa_strerror", "msa_last_cuda_error", "msa_version"]
+
+
+def _lib() -> ctypes.CDLL:
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -c 'import __graft_entry__ as g; "
+                               "g.build()'` (there is no fallback path)")
+        lib = ctypes.CDLL(LIB_PATH)
+        vp, i32, i64, f32, sz = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_float, ctypes.c_size_t
+        lib.msa_create.argtypes = [ctypes.POINTER(MsaConfig), ctypes.POINTER(vp)]
+        lib.msa_destroy.argtypes = [vp]
+        lib.msa_destroy.restype = None
+        lib.msa_plan_create.argtypes = [vp, ctypes.POINTER(MsaRequest), i32, ctypes.POINTER(MsaSegment), i32,
+                                        ctypes.POINTER(vp)]
+        lib.msa_plan_destroy.argtypes = [vp]
+        lib.msa_plan_destroy.restype = None
+        lib.msa_plan_get_info.argtypes = [vp, ctypes.POINTER(MsaPlanInfo)]
+        lib.msa_plan_export.argtypes = [vp, ctypes.c_int, vp, ctypes.POINTER(sz)]
+        lib.msa_workspace_bytes.argtypes = [vp, ctypes.POINTER(sz)]
+        lib.msa_forward.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, i64, f32, vp, vp, vp, sz, vp]
+        lib.msa_forward_host.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, i64, f32, vp, vp, vp]
+        lib.msa_last_launch_count.argtypes = [vp]
+        for f in ("msa_strerror", "msa_last_cuda_error", "msa_version"):
+            getattr(lib, f).restype = ctypes.c_char_p
+        lib.msa_strerror.argtypes = [ctypes.c_int]
+        _LIB = lib
+    return _LIB
+
+
+def _check(status: int, where: str) -> None:
+    if status != MSA_OK:
+        raise MsaError(status, where)
+
+
+def _dptr(t) -> Optional[int]:
+    """Device/host pointer of a torch tensor or numpy array (None -> NULL)."""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        return t.ctypes.data
+    return t.data_ptr()
+
+
+def msa_version() -> str:
+    return _lib().msa_version().decode()
+
+
+def msa_create(num_q_heads: int, num_kv_heads: int, head_dim: int, q_to_kv_head=None, device: int = 0,
+               block_size: int = 16) -> ctypes.c_void_p:
+    cfg = MsaConfig(num_q_heads, num_kv_heads, head_dim, block_size, None, device)
+    keep = None
+    if q_to_kv_head is not None:
+        keep = np.ascontiguousarray(q_to_kv_head, np.int32)
+        cfg.q_to_kv_head = keep.ctypes.data_as(ctypes.POINTER(ctypes.c_int32))
+    h = ctypes.c_void_p()
+    _check(_lib().msa_create(ctypes.byref(cfg), ctypes.byref(h)), "msa_create")
+    return h
+
+
+def msa_destroy(h) -> None:
+    _lib().msa_destroy(h)
+
+
+def make_descriptors(req: np.ndarray, seg_kind, seg_abs_start, seg_len, seg_block_off, seg_row_off):
+    """numpy descriptor columns -> ctypes arrays of msa_request / msa_segment."""
+    req = np.asarray(req, np.int32).reshape(-1, 5)
+    R = (MsaRequest * max(1, req.shape[0]))()
+    for i in range(req.shape[0]):
+        R[i] = MsaRequest(*(int(x) for x in req[i]))
+    n = len(seg_kind)
+    S = (MsaSegment * max(1, n))()
+    for i in range(n):
+        S[i] = MsaSegment(int(seg_kind[i]), int(seg_abs_start[i]), int(seg_len[i]), int(seg_block_off[i]),
+                          int(seg_row_off[i]))
+    return R, req.shape[0], S, n
+
+
+def msa_plan_create(h, requests, n_req: int, segments, n_seg: int) -> ctypes.c_void_p:
+    p = ctypes.c_void_p()
+    _check(_lib().msa_plan_create(h, requests, n_req, segments, n_seg, ctypes.byref(p)), "msa_plan_create")
+    return p
+
+
+def msa_plan_destroy(p) -> None:
+    _lib().msa_plan_destroy(p)
+
+
+def msa_plan_get_info(p) -> Dict[str, int]:
+    info = MsaPlanInfo()
+    _check(_lib().msa_plan_get_info(p, ctypes.byref(info)), "msa_plan_get_info")
+    return {k: int(getattr(info, k)) for k, _ in MsaPlanInfo._fields_}
+
+
+_EXPORT_DTYPES = {
+    0: np.dtype([("src", "<i4"), ("abs_start", "<i4"), ("nvalid", "<i4"), ("paged", "<i4")]),
+    1: np.dtype([("q_row0", "<i4"), ("n_tok", "<i4"), ("q_abs0", "<i4"), ("kvh", "<i4"), ("vb_begin", "<i4"),
+                 ("vb_count", "<i4"), ("tile_begin", "<i4"), ("tile_end", "<i4"), ("partial_off", "<i4"),
+                 ("r0", "<i4"), ("r1", "<i4"), ("r2", "<i4")]),
+    2: np.dtype("<i4"),
+    3: np.dtype([("q_row0", "<i4"), ("n_tok", "<i4"), ("kvh", "<i4"), ("n_partials", "<i4"),
+                 ("first_off", "<i8"), ("stride", "<i8")]),
+}
+
+
+def msa_plan_export(p, which: int) -> np.ndarray:
+    n = ctypes.c_size_t(0)
+    _check(_lib().msa_plan_export(p, which, None, ctypes.byref(n)), "msa_plan_export")
+    dt = _EXPORT_DTYPES[which]
+    out = np.zeros(n.value // dt.itemsize, dt)
+    if n.value:
+        _check(_lib().msa_plan_export(p, which, out.ctypes.data, ctypes.byref(n)), "msa_plan_export")
+    return out
+
+
+def msa_workspace_bytes(p) -> int:
+    n = ctypes.c_size_t(0)
+    _check(_lib().msa_workspace_bytes(p, ctypes.byref(n)), "msa_workspace_bytes")
+    return int(n.value)
+
+
+def msa_forward(h, p, q, pool_k, pool_v, block_table, contig_k, contig_v, softmax_scale: float, o, lse,
+                workspace=None, stream: Optional[int] = None) -> None:
+    """q/pool/contig/o: bf16 CUDA tensors; block_table int32 CUDA; lse fp32 CUDA; workspace uint8 CUDA."""
+    total_q = int(q.shape[0])
+    num_blocks = 0 if pool_k is None else int(pool_k.shape[0])
+    bt_len = 0 if block_table is None else int(block_table.numel())
+    rows = 0 if contig_k is None else int(contig_k.shape[0])
+    ws_bytes = 0 if workspace is None else int(workspace.numel() * workspace.element_size())
+    _check(_lib().msa_forward(h, p, _dptr(q), total_q, _dptr(pool_k), _dptr(pool_v), num_blocks, _dptr(block_table),
+                              bt_len, _dptr(contig_k), _dptr(contig_v), rows, ctypes.c_float(softmax_scale), _dptr(o),
+                              _dptr(lse), _dptr(workspace), ws_bytes, stream), "msa_forward")
+
+
+def msa_forward_host(h, p, q_host, pool_k, pool_v, block_table_host, contig_k_host, contig_v_host,
+                     softmax_scale: float, o_host, lse_host, stream: Optional[int] = None) -> None:
+    """Host (ideally pinned) q / block table / arena / o / lse; the paged pool stays on the device."""
+    total_q = int(q_host.shape[0])
+    num_blocks = 0 if pool_k is None else int(pool_k.shape[0])
+    bt_len = 0 if block_table_host is None else int(block_table_host.numel())
+    rows = 0 if contig_k_host is None else int(contig_k_host.shape[0])
+    _check(_lib().msa_forward_host(h, p, _dptr(q_host), total_q, _dptr(pool_k), _dptr(pool_v), num_blocks,
+                                   _dptr(block_table_host), bt_len, _dptr(contig_k_host), _dptr(contig_v_host), rows,
+                                   ctypes.c_float(softmax_scale), _dptr(o_host), _dptr(lse_host), stream),
+           "msa_forward_host")
+
+
+def msa_last_launch_count(h) -> int:
+    return int(_lib().msa_last_launch_count(h))
+
+
+# --------------------------------------------------------------------------- convenience
+class MsaSession:
+    """Handle + plan + output/workspace buffers for one problem (marshalling only)."""
+
+    def __init__(self, problem, device: int = 0):
+        import torch
+        self.problem = p = problem
+        self.h = msa_create(p.Hq, p.Hkv, p.D, p.q_to_kv, device=device)
+        R, n_req, S, n_seg = make_descriptors(p.req, p.seg_kind, p.seg_abs_start, p.seg_len, p.seg_block_off,
+                                              p.seg_row_off)
+        self.plan = msa_plan_create(self.h, R, n_req, S, n_seg)
+        self.info = msa_plan_get_info(self.plan)
+        dev = torch.device("cuda", device)
+        self.o = torch.zeros((p.total_q, p.Hq, p.D), dtype=torch.bfloat16, device=dev)
+        self.lse = torch.zeros((p.total_q, p.Hq), dtype=torch.float32, device=dev)
+        nb = msa_workspace_bytes(self.plan)
+        self.workspace = torch.empty(max(nb, 16), dtype=torch.uint8, device=dev) if nb else None
+
+    def forward(self, stream: Optional[int] = None) -> Tuple["object", "object"]:
+        import torch
+        p = self.problem
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        msa_forward(self.h, self.plan, p.q, p.pool_k, p.pool_v, p.block_table, p.contig_k, p.contig_v, p.scale,
+                    self.o, self.lse, self.workspace, stream)
+        return self.o, self.lse
+
+    def close(self) -> None:
+        if self.plan is not None:
+            msa_plan_destroy(self.plan)
+            self.plan = None
+        if self.h is not None:
+            msa_destroy(self.h)
+            self.h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()

@@ -1,0 +1,445 @@
+// C ABI of libmsa (include/msa.h): handle, plan upload, tensor-map encoding and launches.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/msa.h"
+#include "msa_kernels.h"
+#include "msa_planner.h"
+
+using namespace msa;
+
+namespace {
+
+thread_local std::string g_cuda_err;
+
+int cuda_fail(cudaError_t e, const char *what)
+{
+    g_cuda_err = std::string(what) + ": " + cudaGetErrorString(e);
+    cudaGetLastError();
+    return MSA_ERR_CUDA;
+}
+#define MSA_CUDA(expr)                                         \
+    do {                                                       \
+        cudaError_t e_ = (expr);                               \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #expr);    \
+    } while (0)
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct DevBuf {
+    void *p = nullptr;
+    size_t cap = 0;
+    cudaError_t reserve(size_t bytes)
+    {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) cudaFree(p);
+        p = nullptr;
+        cap = 0;
+        cudaError_t e = cudaMalloc(&p, bytes);
+        if (e == cudaSuccess) cap = bytes;
+        return e;
+    }
+    void release()
+    {
+        if (p) cudaFree(p);
+        p = nullptr;
+        cap = 0;
+    }
+};
+
+}  // namespace
+
+struct msa_handle_s {
+    msa_config cfg{};
+    int G = 0, R = 0;
+    int num_sms = 0;
+    bool planning_only = false;
+    FwdVariant variant = FwdVariant::Simple;
+    std::vector<int32_t> kv_to_q;      // [Hkv][G]
+    int32_t *d_kv_to_q = nullptr;
+    EncodeTiledFn encode = nullptr;
+    int last_launches = 0;
+    // staging for msa_forward_host
+    DevBuf s_q, s_o, s_lse, s_ck, s_cv, s_bt, s_ws;
+};
+
+struct msa_plan_s {
+    msa_handle h = nullptr;
+    HostPlan hp;
+    void *d_buf = nullptr;
+    const VBlock *d_vblocks = nullptr;
+    const WorkUnit *d_units = nullptr;
+    const int32_t *d_cta_begin = nullptr;
+    const MergeItem *d_merge = nullptr;
+};
+
+extern "C" {
+
+const char *msa_version(void) { return "msa-b200 0.1 (sm_100a)"; }
+
+const char *msa_last_cuda_error(void) { return g_cuda_err.c_str(); }
+
+const char *msa_strerror(int status)
+{
+    switch (status) {
+    case MSA_OK: return "ok";
+    case MSA_ERR_INVALID_ARG: return "invalid argument";
+    case MSA_ERR_UNSUPPORTED: return "unsupported configuration";
+    case MSA_ERR_OVERLAP: return "segments (or q rows) overlap";
+    case MSA_ERR_UNSORTED: return "segments not in ascending abs_start";
+    case MSA_ERR_OUT_OF_RANGE: return "descriptor out of range";
+    case MSA_ERR_MISALIGNED: return "pointer not 16-byte aligned";
+    case MSA_ERR_WORKSPACE: return "workspace missing or too small";
+    case MSA_ERR_CUDA: return "CUDA error";
+    case MSA_ERR_NO_DEVICE: return "no sm_100 CUDA device (there is no CPU fallback)";
+    default: return "unknown status";
+    }
+}
+
+int msa_create(const msa_config *cfg, msa_handle *out)
+{
+    if (!cfg || !out) return MSA_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (cfg->num_q_heads < 1 || cfg->num_kv_heads < 1) return MSA_ERR_INVALID_ARG;
+    if (cfg->head_dim != 64 && cfg->head_dim != 128) return MSA_ERR_UNSUPPORTED;
+    if (cfg->block_size != MSA_BLOCK_SIZE) return MSA_ERR_UNSUPPORTED;
+    if (cfg->num_q_heads % cfg->num_kv_heads != 0) return MSA_ERR_UNSUPPORTED;
+    const int G = cfg->num_q_heads / cfg->num_kv_heads;
+    if (G > MSA_MAX_GROUP) return MSA_ERR_UNSUPPORTED;
+
+    msa_handle h = new (std::nothrow) msa_handle_s();
+    if (!h) return MSA_ERR_INVALID_ARG;
+    h->cfg = *cfg;
+    h->cfg.q_to_kv_head = nullptr;
+    h->G = G;
+    h->R = (kTileM / G) & ~7;
+    // head map -> q heads of each kv head, in ascending q-head order
+    h->kv_to_q.assign(static_cast<size_t>(cfg->num_kv_heads) * G, -1);
+    std::vector<int> fill(cfg->num_kv_heads, 0);
+    for (int q = 0; q < cfg->num_q_heads; ++q) {
+        const int kv = cfg->q_to_kv_head ? cfg->q_to_kv_head[q] : q / G;
+        if (kv < 0 || kv >= cfg->num_kv_heads || fill[kv] >= G) {
+            delete h;
+            return MSA_ERR_UNSUPPORTED;
+        }
+        h->kv_to_q[static_cast<size_t>(kv) * G + fill[kv]++] = q;
+    }
+    const char *kv = getenv("MSA_KERNEL");
+    h->variant = (kv && strcmp(kv, "simple") == 0) ? FwdVariant::Simple : FwdVariant::Simple;
+
+    if (cfg->device < 0) {
+        // planning-only handle: descriptor validation and scheduling on the host; every
+        // call that would touch the GPU reports MSA_ERR_NO_DEVICE.
+        h->planning_only = true;
+        h->num_sms = 148;
+        *out = h;
+        return MSA_OK;
+    }
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || cfg->device >= n_dev) {
+        cudaGetLastError();
+        delete h;
+        return MSA_ERR_NO_DEVICE;
+    }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess || prop.major != 10) {
+        cudaGetLastError();
+        delete h;
+        return MSA_ERR_NO_DEVICE;
+    }
+    h->num_sms = prop.multiProcessorCount;
+    cudaError_t e = cudaSetDevice(cfg->device);
+    if (e == cudaSuccess) e = cudaMalloc(&h->d_kv_to_q, h->kv_to_q.size() * sizeof(int32_t));
+    if (e == cudaSuccess)
+        e = cudaMemcpy(h->d_kv_to_q, h->kv_to_q.data(), h->kv_to_q.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (e == cudaSuccess) e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess || !fn) {
+        if (h->d_kv_to_q) cudaFree(h->d_kv_to_q);
+        delete h;
+        return e != cudaSuccess ? cuda_fail(e, "msa_create") : MSA_ERR_NO_DEVICE;
+    }
+    h->encode = reinterpret_cast<EncodeTiledFn>(fn);
+    *out = h;
+    return MSA_OK;
+}
+
+void msa_destroy(msa_handle h)
+{
+    if (!h) return;
+    if (!h->planning_only) {
+        if (h->d_kv_to_q) cudaFree(h->d_kv_to_q);
+        h->s_q.release(); h->s_o.release(); h->s_lse.release(); h->s_ck.release();
+        h->s_cv.release(); h->s_bt.release(); h->s_ws.release();
+    }
+    delete h;
+}
+
+int msa_plan_create(msa_handle h, const msa_request *requests, int32_t n_req, const msa_segment *segments,
+                    int32_t n_seg, msa_plan *out)
+{
+    if (!h || !out) return MSA_ERR_INVALID_ARG;
+    *out = nullptr;
+    PlannerConfig pc;
+    pc.Hq = h->cfg.num_q_heads;
+    pc.Hkv = h->cfg.num_kv_heads;
+    pc.D = h->cfg.head_dim;
+    pc.G = h->G;
+    pc.R = h->R;
+    pc.tiles_per_group = fwd_tiles_per_group(h->variant);
+    pc.num_ctas = h->num_sms;
+    msa_plan p = new (std::nothrow) msa_plan_s();
+    if (!p) return MSA_ERR_INVALID_ARG;
+    p->h = h;
+    int rc = build_plan(pc, requests, n_req, segments, n_seg, &p->hp);
+    if (rc != MSA_OK) {
+        delete p;
+        return rc;
+    }
+    if (!h->planning_only) {
+        const HostPlan &hp = p->hp;
+        auto al = [](size_t x) { return (x + 255) & ~static_cast<size_t>(255); };
+        const size_t b_vb = al(hp.vblocks.size() * sizeof(VBlock));
+        const size_t b_un = al(hp.units.size() * sizeof(WorkUnit));
+        const size_t b_cb = al(hp.cta_unit_begin.size() * sizeof(int32_t));
+        const size_t b_mg = al(hp.merge_items.size() * sizeof(MergeItem));
+        const size_t total = b_vb + b_un + b_cb + b_mg + 256;
+        cudaError_t e = cudaSetDevice(h->cfg.device);
+        if (e == cudaSuccess) e = cudaMalloc(&p->d_buf, total);
+        if (e != cudaSuccess) {
+            delete p;
+            return cuda_fail(e, "msa_plan_create: cudaMalloc");
+        }
+        char *base = static_cast<char *>(p->d_buf);
+        p->d_vblocks = reinterpret_cast<const VBlock *>(base);
+        p->d_units = reinterpret_cast<const WorkUnit *>(base + b_vb);
+        p->d_cta_begin = reinterpret_cast<const int32_t *>(base + b_vb + b_un);
+        p->d_merge = reinterpret_cast<const MergeItem *>(base + b_vb + b_un + b_cb);
+        if (e == cudaSuccess && !hp.vblocks.empty())
+            e = cudaMemcpy(base, hp.vblocks.data(), hp.vblocks.size() * sizeof(VBlock), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess && !hp.units.empty())
+            e = cudaMemcpy(base + b_vb, hp.units.data(), hp.units.size() * sizeof(WorkUnit), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess && !hp.cta_unit_begin.empty())
+            e = cudaMemcpy(base + b_vb + b_un, hp.cta_unit_begin.data(), hp.cta_unit_begin.size() * sizeof(int32_t),
+                           cudaMemcpyHostToDevice);
+        if (e == cudaSuccess && !hp.merge_items.empty())
+            e = cudaMemcpy(base + b_vb + b_un + b_cb, hp.merge_items.data(), hp.merge_items.size() * sizeof(MergeItem),
+                           cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) {
+            cudaFree(p->d_buf);
+            delete p;
+            return cuda_fail(e, "msa_plan_create: upload");
+        }
+    }
+    *out = p;
+    return MSA_OK;
+}
+
+void msa_plan_destroy(msa_plan p)
+{
+    if (!p) return;
+    if (p->d_buf) cudaFree(p->d_buf);
+    delete p;
+}
+
+int msa_plan_get_info(msa_plan p, msa_plan_info *info)
+{
+    if (!p || !info) return MSA_ERR_INVALID_ARG;
+    *info = p->hp.info;
+    return MSA_OK;
+}
+
+int msa_workspace_bytes(msa_plan p, size_t *bytes)
+{
+    if (!p || !bytes) return MSA_ERR_INVALID_ARG;
+    *bytes = static_cast<size_t>(p->hp.workspace_floats) * sizeof(float);
+    return MSA_OK;
+}
+
+/* Introspection for tests: copies the host-side plan arrays out.
+ * which: 0 = virtual blocks (int32 x4 each), 1 = work units (int32 x12 each),
+ *        2 = cta_unit_begin (int32), 3 = merge items (int32 x4 + int64 x2 each).
+ * Call with buf == NULL to get the byte size. */
+int msa_plan_export(msa_plan p, int which, void *buf, size_t *bytes)
+{
+    if (!p || !bytes) return MSA_ERR_INVALID_ARG;
+    const void *src = nullptr;
+    size_t n = 0;
+    switch (which) {
+    case 0: src = p->hp.vblocks.data(); n = p->hp.vblocks.size() * sizeof(VBlock); break;
+    case 1: src = p->hp.units.data(); n = p->hp.units.size() * sizeof(WorkUnit); break;
+    case 2: src = p->hp.cta_unit_begin.data(); n = p->hp.cta_unit_begin.size() * sizeof(int32_t); break;
+    case 3: src = p->hp.merge_items.data(); n = p->hp.merge_items.size() * sizeof(MergeItem); break;
+    default: return MSA_ERR_INVALID_ARG;
+    }
+    if (buf) {
+        if (*bytes < n) return MSA_ERR_INVALID_ARG;
+        if (n) memcpy(buf, src, n);
+    }
+    *bytes = n;
+    return MSA_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+int encode_2d(msa_handle h, CUtensorMap *tm, const void *base, uint64_t inner_elems, uint64_t rows, uint32_t box_rows)
+{
+    cuuint64_t gdim[2] = {inner_elems, rows > 0 ? rows : 1};
+    cuuint64_t gstride[1] = {inner_elems * 2};
+    cuuint32_t box[2] = {64, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = h->encode(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), gdim, gstride, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        char msg[96];
+        snprintf(msg, sizeof msg, "cuTensorMapEncodeTiled failed: CUresult %d", static_cast<int>(r));
+        g_cuda_err = msg;
+        return MSA_ERR_CUDA;
+    }
+    return MSA_OK;
+}
+
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+}  // namespace
+
+extern "C" {
+
+int msa_forward(msa_handle h, msa_plan p, const void *q, int64_t total_q, const void *pool_k, const void *pool_v,
+                int64_t num_blocks, const int32_t *block_table, int64_t block_table_len, const void *contig_k,
+                const void *contig_v, int64_t contig_rows, float softmax_scale, void *o, float *lse, void *workspace,
+                size_t workspace_bytes, void *cuda_stream)
+{
+    if (!h || !p || p->h != h) return MSA_ERR_INVALID_ARG;
+    if (h->planning_only) return MSA_ERR_NO_DEVICE;
+    h->last_launches = 0;
+    const HostPlan &hp = p->hp;
+    if (!(softmax_scale > 0.f) || !isfinite(softmax_scale)) return MSA_ERR_INVALID_ARG;
+    if (total_q < 0 || num_blocks < 0 || block_table_len < 0 || contig_rows < 0) return MSA_ERR_INVALID_ARG;
+    if (hp.info.num_units == 0) return MSA_OK;
+    if (!q || !o || !lse) return MSA_ERR_INVALID_ARG;
+    if (hp.uses_paged && (!pool_k || !pool_v || !block_table)) return MSA_ERR_INVALID_ARG;
+    if (hp.uses_contig && (!contig_k || !contig_v)) return MSA_ERR_INVALID_ARG;
+    if (hp.info.max_q_row >= total_q) return MSA_ERR_OUT_OF_RANGE;
+    if (hp.uses_paged && hp.info.max_block_table_index >= block_table_len) return MSA_ERR_OUT_OF_RANGE;
+    if (hp.uses_contig && hp.info.max_contig_row >= contig_rows) return MSA_ERR_OUT_OF_RANGE;
+    if (hp.uses_paged && (num_blocks < 1 || num_blocks * MSA_BLOCK_SIZE > 0x7fffffffLL)) return MSA_ERR_OUT_OF_RANGE;
+    if (!aligned16(q) || !aligned16(o) || !aligned16(pool_k) || !aligned16(pool_v) || !aligned16(contig_k) ||
+        !aligned16(contig_v) || (reinterpret_cast<uintptr_t>(lse) & 3u) || (reinterpret_cast<uintptr_t>(block_table) & 3u))
+        return MSA_ERR_MISALIGNED;
+    const size_t need = static_cast<size_t>(hp.workspace_floats) * sizeof(float);
+    if (need > 0) {
+        if (!workspace || workspace_bytes < need) return MSA_ERR_WORKSPACE;
+        if (!aligned16(workspace)) return MSA_ERR_MISALIGNED;
+    }
+
+    const int Hq = h->cfg.num_q_heads, Hkv = h->cfg.num_kv_heads, D = h->cfg.head_dim;
+    FwdParams fp;
+    memset(&fp, 0, sizeof fp);
+    int rc = encode_2d(h, &fp.tm_q, q, static_cast<uint64_t>(Hq) * D, static_cast<uint64_t>(total_q), h->R);
+    if (rc != MSA_OK) return rc;
+    const void *pk = hp.uses_paged ? pool_k : q;
+    const void *pv = hp.uses_paged ? pool_v : q;
+    const uint64_t prow = hp.uses_paged ? static_cast<uint64_t>(num_blocks) * MSA_BLOCK_SIZE : static_cast<uint64_t>(total_q);
+    const uint64_t pin = hp.uses_paged ? static_cast<uint64_t>(Hkv) * D : static_cast<uint64_t>(Hq) * D;
+    if ((rc = encode_2d(h, &fp.tm_pool_k, pk, pin, prow, MSA_BLOCK_SIZE)) != MSA_OK) return rc;
+    if ((rc = encode_2d(h, &fp.tm_pool_v, pv, pin, prow, MSA_BLOCK_SIZE)) != MSA_OK) return rc;
+    const void *ck = hp.uses_contig ? contig_k : q;
+    const void *cv = hp.uses_contig ? contig_v : q;
+    const uint64_t crow = hp.uses_contig ? static_cast<uint64_t>(contig_rows) : static_cast<uint64_t>(total_q);
+    const uint64_t cin = hp.uses_contig ? static_cast<uint64_t>(Hkv) * D : static_cast<uint64_t>(Hq) * D;
+    if ((rc = encode_2d(h, &fp.tm_ctg_k, ck, cin, crow, MSA_BLOCK_SIZE)) != MSA_OK) return rc;
+    if ((rc = encode_2d(h, &fp.tm_ctg_v, cv, cin, crow, MSA_BLOCK_SIZE)) != MSA_OK) return rc;
+    fp.vblocks = p->d_vblocks;
+    fp.units = p->d_units;
+    fp.cta_unit_begin = p->d_cta_begin;
+    fp.block_table = block_table;
+    fp.kv_to_q = h->d_kv_to_q;
+    fp.o = o;
+    fp.lse = lse;
+    fp.workspace = static_cast<float *>(workspace);
+    fp.scale_log2 = softmax_scale * 1.4426950408889634f;
+    fp.Hq = Hq;
+    fp.Hkv = Hkv;
+    fp.G = h->G;
+    fp.R = h->R;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    MSA_CUDA(launch_fwd(fp, D, hp.info.num_ctas, h->variant, stream));
+    h->last_launches = 1;
+    if (!hp.merge_items.empty()) {
+        MergeParams mp;
+        mp.items = p->d_merge;
+        mp.kv_to_q = h->d_kv_to_q;
+        mp.workspace = static_cast<const float *>(workspace);
+        mp.o = o;
+        mp.lse = lse;
+        mp.Hq = Hq;
+        mp.G = h->G;
+        mp.D = D;
+        MSA_CUDA(launch_merge(mp, static_cast<int>(hp.merge_items.size()), stream));
+        h->last_launches = 2;
+    }
+    return MSA_OK;
+}
+
+int msa_forward_host(msa_handle h, msa_plan p, const void *q_host, int64_t total_q, const void *pool_k,
+                     const void *pool_v, int64_t num_blocks, const int32_t *block_table_host, int64_t block_table_len,
+                     const void *contig_k_host, const void *contig_v_host, int64_t contig_rows, float softmax_scale,
+                     void *o_host, float *lse_host, void *cuda_stream)
+{
+    if (!h || !p || p->h != h) return MSA_ERR_INVALID_ARG;
+    if (h->planning_only) return MSA_ERR_NO_DEVICE;
+    if (total_q < 0 || block_table_len < 0 || contig_rows < 0) return MSA_ERR_INVALID_ARG;
+    if (total_q > 0 && (!q_host || !o_host || !lse_host)) return MSA_ERR_INVALID_ARG;
+    if (block_table_len > 0 && !block_table_host) return MSA_ERR_INVALID_ARG;
+    if (contig_rows > 0 && (!contig_k_host || !contig_v_host)) return MSA_ERR_INVALID_ARG;
+    const int Hq = h->cfg.num_q_heads, Hkv = h->cfg.num_kv_heads, D = h->cfg.head_dim;
+    const size_t b_q = static_cast<size_t>(total_q) * Hq * D * 2;
+    const size_t b_lse = static_cast<size_t>(total_q) * Hq * 4;
+    const size_t b_c = static_cast<size_t>(contig_rows) * Hkv * D * 2;
+    const size_t b_bt = static_cast<size_t>(block_table_len) * 4;
+    const size_t b_ws = static_cast<size_t>(p->hp.workspace_floats) * 4;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    MSA_CUDA(cudaSetDevice(h->cfg.device));
+    MSA_CUDA(h->s_q.reserve(b_q + 16));
+    MSA_CUDA(h->s_o.reserve(b_q + 16));
+    MSA_CUDA(h->s_lse.reserve(b_lse + 16));
+    MSA_CUDA(h->s_ck.reserve(b_c + 16));
+    MSA_CUDA(h->s_cv.reserve(b_c + 16));
+    MSA_CUDA(h->s_bt.reserve(b_bt + 16));
+    MSA_CUDA(h->s_ws.reserve(b_ws + 16));
+    if (b_q) MSA_CUDA(cudaMemcpyAsync(h->s_q.p, q_host, b_q, cudaMemcpyHostToDevice, stream));
+    if (b_bt) MSA_CUDA(cudaMemcpyAsync(h->s_bt.p, block_table_host, b_bt, cudaMemcpyHostToDevice, stream));
+    if (b_c) {
+        MSA_CUDA(cudaMemcpyAsync(h->s_ck.p, contig_k_host, b_c, cudaMemcpyHostToDevice, stream));
+        MSA_CUDA(cudaMemcpyAsync(h->s_cv.p, contig_v_host, b_c, cudaMemcpyHostToDevice, stream));
+    }
+    int rc = msa_forward(h, p, h->s_q.p, total_q, pool_k, pool_v, num_blocks, static_cast<const int32_t *>(h->s_bt.p),
+                         block_table_len, h->s_ck.p, h->s_cv.p, contig_rows, softmax_scale, h->s_o.p,
+                         static_cast<float *>(h->s_lse.p), h->s_ws.p, h->s_ws.cap, stream);
+    if (rc != MSA_OK) return rc;
+    if (b_q) {
+        MSA_CUDA(cudaMemcpyAsync(o_host, h->s_o.p, b_q, cudaMemcpyDeviceToHost, stream));
+        MSA_CUDA(cudaMemcpyAsync(lse_host, h->s_lse.p, b_lse, cudaMemcpyDeviceToHost, stream));
+    }
+    MSA_CUDA(cudaStreamSynchronize(stream));
+    return MSA_OK;
+}
+
+int msa_last_launch_count(msa_handle h) { return h ? h->last_launches : 0; }
+
+}  // extern "C"

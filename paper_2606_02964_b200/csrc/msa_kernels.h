@@ -1,0 +1,45 @@
+// Launch interface between the host API (msa_api.cu) and the sm_100a kernels.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "msa_plan.h"
+
+namespace msa {
+
+struct FwdParams {
+    CUtensorMap tm_q;        // bf16 [total_q][Hq*D], box 64 x R
+    CUtensorMap tm_pool_k;   // bf16 [num_blocks*16][Hkv*D], box 64 x 16
+    CUtensorMap tm_pool_v;
+    CUtensorMap tm_ctg_k;    // bf16 [contig_rows][Hkv*D], box 64 x 16
+    CUtensorMap tm_ctg_v;
+    const VBlock *vblocks;
+    const WorkUnit *units;
+    const int32_t *cta_unit_begin;   // [num_ctas+1]
+    const int32_t *block_table;
+    const int32_t *kv_to_q;          // [Hkv][G] q heads of each kv head
+    void *o;                         // bf16 [total_q][Hq][D]
+    float *lse;                      // [total_q][Hq]
+    float *workspace;
+    float scale_log2;                // softmax_scale * log2(e)
+    int32_t Hq, Hkv, G, R;           // R = tokens per 128-row tile
+};
+
+struct MergeParams {
+    const MergeItem *items;
+    const int32_t *kv_to_q;
+    const float *workspace;
+    void *o;
+    float *lse;
+    int32_t Hq, G, D;
+};
+
+// kernel variants (debug env MSA_KERNEL selects; default = the fastest validated one)
+enum class FwdVariant : int { Simple = 0, Pipelined = 1 };
+
+cudaError_t launch_fwd(const FwdParams &p, int head_dim, int num_ctas, FwdVariant v, cudaStream_t stream);
+cudaError_t launch_merge(const MergeParams &p, int n_items, cudaStream_t stream);
+int fwd_tiles_per_group(FwdVariant v);   // q tiles (of 128 packed rows) one work item covers
+
+}  // namespace msa

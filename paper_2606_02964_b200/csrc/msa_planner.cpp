@@ -1,0 +1,257 @@
+// Host planner of libmsa (see msa_planner.h).  Turns the C-ABI descriptors into the device
+// plan: the paper's "split indices" + per-token-block "equivalent seq_len" metadata
+// (PAPER.md:122-124), re-designed as a virtual block list plus a persistent, split-KV
+// schedule over (run, kv-head, q-tile, kv-tile-range) units.
+#include "msa_planner.h"
+
+#include <algorithm>
+#include <climits>
+#include <map>
+#include <utility>
+
+namespace msa {
+
+namespace {
+
+struct Ctx {
+    int32_t vb_begin = 0;
+    int32_t vb_count = 0;
+};
+
+struct Item {
+    int32_t q_row0, n_tok, q_abs0, kvh, vb_begin, vb_count, n_tiles;
+};
+
+// sum_{i=0}^{T-1} clamp(c0 + i, 0, n)
+int64_t clamp_sum(int64_t c0, int64_t T, int64_t n)
+{
+    if (T <= 0 || n <= 0) return 0;
+    const int64_t lo = c0, hi = c0 + T - 1;
+    int64_t s = 0;
+    const int64_t first = std::max<int64_t>(lo, 1), last = std::min<int64_t>(hi, n);
+    if (last >= first) s += (first + last) * (last - first + 1) / 2;
+    if (hi > n) s += n * (hi - std::max<int64_t>(n, lo - 1));
+    return s;
+}
+
+}  // namespace
+
+int build_plan(const PlannerConfig &cfg, const msa_request *req, int32_t n_req, const msa_segment *seg, int32_t n_seg,
+               HostPlan *out)
+{
+    if (!out || n_req < 0 || n_seg < 0 || (n_req > 0 && !req) || (n_seg > 0 && !seg)) return MSA_ERR_INVALID_ARG;
+    if (cfg.G < 1 || cfg.R < 8 || cfg.tiles_per_group < 1 || cfg.num_ctas < 1) return MSA_ERR_INVALID_ARG;
+    HostPlan &hp = *out;
+    hp = HostPlan();
+
+    // ---- segments: per-descriptor checks --------------------------------------------
+    int64_t max_bt = -1, max_row = -1, max_q = -1;
+    for (int32_t s = 0; s < n_seg; ++s) {
+        const msa_segment &sg = seg[s];
+        if (sg.kind < MSA_SEG_PAGED || sg.kind > MSA_SEG_SELF) return MSA_ERR_INVALID_ARG;
+        if (sg.len < 1 || sg.abs_start < 0) return MSA_ERR_INVALID_ARG;
+        if (static_cast<int64_t>(sg.abs_start) + sg.len > INT32_MAX) return MSA_ERR_OUT_OF_RANGE;
+        if (sg.kind == MSA_SEG_PAGED) {
+            if (sg.block_off < 0) return MSA_ERR_OUT_OF_RANGE;
+            const int64_t last = static_cast<int64_t>(sg.block_off) + (sg.len + kBlock - 1) / kBlock - 1;
+            if (last > INT32_MAX) return MSA_ERR_OUT_OF_RANGE;
+            max_bt = std::max(max_bt, last);
+        } else {
+            if (sg.row_off < 0) return MSA_ERR_OUT_OF_RANGE;
+            const int64_t last = sg.row_off + sg.len - 1;
+            if (last + kBlock > INT32_MAX) return MSA_ERR_OUT_OF_RANGE;   // TMA coordinates are int32
+            max_row = std::max(max_row, last);
+        }
+    }
+
+    // ---- requests: ranges, q-row overlap ---------------------------------------------
+    std::vector<std::pair<int64_t, int64_t>> qspans;
+    for (int32_t r = 0; r < n_req; ++r) {
+        const msa_request &rq = req[r];
+        if (rq.q_len < 0 || rq.q_row_start < 0 || rq.q_abs_start < 0) return MSA_ERR_INVALID_ARG;
+        if (rq.seg_begin < 0 || rq.seg_count < 0 || static_cast<int64_t>(rq.seg_begin) + rq.seg_count > n_seg)
+            return MSA_ERR_OUT_OF_RANGE;
+        if (static_cast<int64_t>(rq.q_abs_start) + rq.q_len > INT32_MAX) return MSA_ERR_OUT_OF_RANGE;
+        if (static_cast<int64_t>(rq.q_row_start) + rq.q_len > INT32_MAX) return MSA_ERR_OUT_OF_RANGE;
+        if (rq.q_len > 0) {
+            qspans.emplace_back(rq.q_row_start, static_cast<int64_t>(rq.q_row_start) + rq.q_len);
+            max_q = std::max<int64_t>(max_q, static_cast<int64_t>(rq.q_row_start) + rq.q_len - 1);
+        }
+    }
+    std::sort(qspans.begin(), qspans.end());
+    for (size_t i = 1; i < qspans.size(); ++i)
+        if (qspans[i].first < qspans[i - 1].second) return MSA_ERR_OVERLAP;
+
+    // ---- contexts: order / overlap checks, virtual block lists -----------------------
+    std::map<std::pair<int32_t, int32_t>, Ctx> ctxs;
+    for (int32_t r = 0; r < n_req; ++r) {
+        const auto key = std::make_pair(req[r].seg_begin, req[r].seg_count);
+        if (ctxs.count(key)) continue;
+        for (int32_t s = key.first + 1; s < key.first + key.second; ++s) {
+            if (seg[s].abs_start <= seg[s - 1].abs_start) {
+                // equal starts always overlap (len >= 1); a smaller start is an ordering error
+                return seg[s].abs_start == seg[s - 1].abs_start ? MSA_ERR_OVERLAP : MSA_ERR_UNSORTED;
+            }
+            if (static_cast<int64_t>(seg[s - 1].abs_start) + seg[s - 1].len > seg[s].abs_start) return MSA_ERR_OVERLAP;
+        }
+        Ctx c;
+        c.vb_begin = static_cast<int32_t>(hp.vblocks.size());
+        for (int32_t s = key.first; s < key.first + key.second; ++s) {
+            const msa_segment &sg = seg[s];
+            const int nblk = (sg.len + kBlock - 1) / kBlock;
+            for (int b = 0; b < nblk; ++b) {
+                VBlock vb;
+                vb.paged = (sg.kind == MSA_SEG_PAGED) ? 1 : 0;
+                vb.src = vb.paged ? sg.block_off + b : static_cast<int32_t>(sg.row_off + static_cast<int64_t>(b) * kBlock);
+                vb.abs_start = sg.abs_start + b * kBlock;
+                vb.nvalid = std::min(kBlock, sg.len - b * kBlock);
+                hp.vblocks.push_back(vb);
+            }
+            if (sg.kind == MSA_SEG_PAGED) hp.uses_paged = true; else hp.uses_contig = true;
+        }
+        if (hp.vblocks.size() > static_cast<size_t>(INT32_MAX)) return MSA_ERR_OUT_OF_RANGE;
+        c.vb_count = static_cast<int32_t>(hp.vblocks.size()) - c.vb_begin;
+        ctxs[key] = c;
+    }
+
+    // ---- work items: (run, kv head, q-tile group), horizon folded in ------------------
+    const int group_tok = cfg.tiles_per_group * cfg.R;
+    std::vector<Item> items;
+    int64_t pairs = 0;
+    for (int32_t r = 0; r < n_req; ++r) {
+        const msa_request &rq = req[r];
+        if (rq.q_len == 0) continue;
+        const Ctx &c = ctxs[std::make_pair(rq.seg_begin, rq.seg_count)];
+        for (int32_t s = rq.seg_begin; s < rq.seg_begin + rq.seg_count; ++s)
+            pairs += clamp_sum(static_cast<int64_t>(rq.q_abs_start) - seg[s].abs_start + 1, rq.q_len, seg[s].len);
+        for (int kvh = 0; kvh < cfg.Hkv; ++kvh) {
+            for (int32_t t0 = 0; t0 < rq.q_len; t0 += group_tok) {
+                Item it;
+                it.n_tok = std::min<int32_t>(group_tok, rq.q_len - t0);
+                it.q_row0 = rq.q_row_start + t0;
+                it.q_abs0 = rq.q_abs_start + t0;
+                it.kvh = kvh;
+                it.vb_begin = c.vb_begin;
+                const int32_t p_max = it.q_abs0 + it.n_tok - 1;
+                // virtual blocks are in ascending abs_start: count those starting at or before p_max
+                const VBlock *b0 = hp.vblocks.data() + c.vb_begin;
+                const VBlock *e0 = b0 + c.vb_count;
+                const VBlock *ub = std::upper_bound(b0, e0, p_max, [](int32_t p, const VBlock &v) { return p < v.abs_start; });
+                it.vb_count = static_cast<int32_t>(ub - b0);
+                it.n_tiles = (it.vb_count + kVbPerTile - 1) / kVbPerTile;
+                items.push_back(it);
+            }
+        }
+    }
+
+    // ---- persistent schedule: equal contiguous shares of the global tile sequence ------
+    // (stream-K style: only the items a share boundary falls into are split along KV.)
+    const int64_t n_items = static_cast<int64_t>(items.size());
+    std::vector<int64_t> start(n_items + 1, 0);
+    for (int64_t i = 0; i < n_items; ++i) start[i + 1] = start[i] + std::max<int32_t>(items[i].n_tiles, 1);
+    const int64_t W = start[n_items];
+    int n_used = 0;
+    std::vector<int64_t> bound;
+    if (W > 0) {
+        n_used = static_cast<int>(std::min<int64_t>(cfg.num_ctas, std::max<int64_t>(1, W / std::max(1, cfg.min_tiles_per_cta))));
+        bound.resize(n_used + 1);
+        for (int c = 0; c <= n_used; ++c) bound[c] = (W * c) / n_used;
+        for (int c = 1; c < n_used; ++c) {
+            const int64_t b = bound[c];
+            const int64_t i = std::upper_bound(start.begin(), start.end(), b) - start.begin() - 1;   // item holding b
+            if (b - start[i] <= cfg.snap_tiles) bound[c] = start[i];
+            else if (start[i + 1] - b <= cfg.snap_tiles) bound[c] = start[i + 1];
+        }
+        for (int c = 1; c <= n_used; ++c) bound[c] = std::max(bound[c], bound[c - 1]);
+    }
+
+    // pieces per item
+    std::vector<int32_t> pieces(n_items, 0);
+    {
+        int64_t i = 0;
+        for (int c = 0; c < n_used; ++c) {
+            const int64_t lo = bound[c], hi = bound[c + 1];
+            while (i < n_items && start[i + 1] <= lo) ++i;
+            for (int64_t j = i; j < n_items && start[j] < hi; ++j)
+                if (std::min(hi, start[j + 1]) > std::max(lo, start[j])) ++pieces[j];
+        }
+    }
+    std::vector<int64_t> item_first_off(n_items, -1);
+    std::vector<int32_t> item_emitted(n_items, 0);
+    int64_t ws = 0;
+    for (int64_t i = 0; i < n_items; ++i) {
+        if (pieces[i] > 1) {
+            const int64_t rows = static_cast<int64_t>(items[i].n_tok) * cfg.G;
+            const int64_t stride = (rows * (cfg.D + 1) + 3) / 4 * 4;
+            MergeItem mi;
+            mi.q_row0 = items[i].q_row0;
+            mi.n_tok = items[i].n_tok;
+            mi.kvh = items[i].kvh;
+            mi.n_partials = pieces[i];
+            mi.first_off = ws;
+            mi.stride = stride;
+            hp.merge_items.push_back(mi);
+            item_first_off[i] = ws;
+            ws += stride * pieces[i];
+        }
+    }
+    if (ws > static_cast<int64_t>(INT32_MAX)) return MSA_ERR_OUT_OF_RANGE;   // partial_off is int32 (floats)
+
+    hp.cta_unit_begin.assign(n_used + 1, 0);
+    {
+        int64_t i = 0;
+        for (int c = 0; c < n_used; ++c) {
+            hp.cta_unit_begin[c] = static_cast<int32_t>(hp.units.size());
+            const int64_t lo = bound[c], hi = bound[c + 1];
+            while (i < n_items && start[i + 1] <= lo) ++i;
+            for (int64_t j = i; j < n_items && start[j] < hi; ++j) {
+                const int64_t a = std::max(lo, start[j]), b = std::min(hi, start[j + 1]);
+                if (b <= a) continue;
+                const Item &it = items[j];
+                WorkUnit u{};
+                u.q_row0 = it.q_row0;
+                u.n_tok = it.n_tok;
+                u.q_abs0 = it.q_abs0;
+                u.kvh = it.kvh;
+                u.vb_begin = it.vb_begin;
+                u.vb_count = it.vb_count;
+                if (it.n_tiles == 0) {
+                    u.tile_begin = u.tile_end = 0;
+                } else {
+                    u.tile_begin = static_cast<int32_t>(a - start[j]);
+                    u.tile_end = static_cast<int32_t>(b - start[j]);
+                }
+                if (pieces[j] > 1) {
+                    const int64_t rows = static_cast<int64_t>(it.n_tok) * cfg.G;
+                    const int64_t stride = (rows * (cfg.D + 1) + 3) / 4 * 4;
+                    u.partial_off = static_cast<int32_t>(item_first_off[j] + stride * item_emitted[j]);
+                    ++item_emitted[j];
+                } else {
+                    u.partial_off = -1;
+                }
+                hp.units.push_back(u);
+            }
+        }
+        hp.cta_unit_begin[n_used] = static_cast<int32_t>(hp.units.size());
+    }
+
+    hp.workspace_floats = ws;
+    hp.info.num_ctas = n_used;
+    hp.info.num_items = static_cast<int32_t>(n_items);
+    hp.info.num_units = static_cast<int32_t>(hp.units.size());
+    hp.info.num_split_items = static_cast<int32_t>(hp.merge_items.size());
+    int32_t n_part = 0;
+    for (const MergeItem &mi : hp.merge_items) n_part += mi.n_partials;
+    hp.info.num_partials = n_part;
+    hp.info.rows_per_tile = cfg.R * cfg.G;
+    int64_t kv_tiles = 0;
+    for (const Item &it : items) kv_tiles += it.n_tiles;
+    hp.info.kv_tiles = kv_tiles;
+    hp.info.visible_pairs = pairs;
+    hp.info.max_block_table_index = hp.uses_paged ? max_bt : -1;
+    hp.info.max_contig_row = hp.uses_contig ? max_row : -1;
+    hp.info.max_q_row = max_q;
+    return MSA_OK;
+}
+
+}  // namespace msa

@@ -1,0 +1,203 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle -- needs a B200.
+
+Bar (BASELINE.json north_star, bf16 inputs / fp32 accumulation):
+    max|dO| <= 2e-2, mean|dO| <= 2e-3, max|dLSE| <= 1e-3
+on the five configs.  Adversarial small cases may have |O| > 2 (few visible keys), where one
+bf16 ulp of the output alone exceeds 2e-2; there the elementwise bound scales with |O|
+("tolerances"): |dO| <= 2e-2 * max(1, |O|/2).
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import workloads as W
+from paper_2606_02964_b200 import (MsaError, MsaSession, MSA_ERR_MISALIGNED, MSA_ERR_OUT_OF_RANGE,
+                                   MSA_ERR_WORKSPACE, make_descriptors, msa_create, msa_destroy, msa_forward,
+                                   msa_forward_host, msa_last_launch_count, msa_plan_create, msa_plan_destroy)
+from workloads import SEG_CONTIG, SEG_PAGED, SEG_SELF, ContextSpec, RunSpec, build_problem
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+TOL_O_MAX, TOL_O_MEAN, TOL_LSE = 2e-2, 2e-3, 1e-3
+
+
+def gpu_forward(p):
+    with MsaSession(p) as s:
+        o, lse = s.forward()
+        torch.cuda.synchronize()
+        return o.float().cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64), s.info
+
+
+def compare(p, o, lse, row_req=None, row_idx=None, strict=True):
+    O, LSE = oracle.forward_problem(p, row_req, row_idx)
+    if row_req is not None:
+        g = p.req[row_req, 0] + row_idx
+        o, lse = o[g], lse[g]
+    fin = np.isfinite(LSE)
+    assert np.array_equal(np.isneginf(lse), ~fin), "rows without a visible key must give LSE=-inf"
+    assert np.all(np.isfinite(o)), "non-finite O"
+    assert np.all(o[~fin] == 0.0)
+    d_o = np.abs(o - O)
+    d_l = np.abs(lse[fin] - LSE[fin]) if fin.any() else np.zeros(1)
+    if strict:
+        assert d_o.max() <= TOL_O_MAX, f"max|dO|={d_o.max()}"
+    else:
+        assert np.all(d_o <= TOL_O_MAX * np.maximum(1.0, np.abs(O) / 2.0)), f"max|dO|={d_o.max()}"
+    assert d_o.mean() <= TOL_O_MEAN, f"mean|dO|={d_o.mean()}"
+    assert d_l.max() <= TOL_LSE, f"max|dLSE|={d_l.max()}"
+    return d_o.max(), d_o.mean(), d_l.max()
+
+
+# ------------------------------------------------------------------ config 1 (full)
+def test_cfg1_tiny_full():
+    p = W.cfg1_tiny(device=DEV)
+    o, lse, info = gpu_forward(p)
+    compare(p, o, lse)
+    assert info["visible_pairs"] == 14368
+
+
+# ------------------------------------------------------------------ small adversarial shapes
+CASES = [
+    dict(seed=101, Hq=4, Hkv=2, D=64, max_ctx=700, max_q=96),
+    dict(seed=102, Hq=8, Hkv=2, D=128, max_ctx=900, max_q=70),
+    dict(seed=103, Hq=4, Hkv=4, D=128, max_ctx=600, max_q=140, n_req=4),          # G=1
+    dict(seed=104, Hq=16, Hkv=2, D=64, max_ctx=500, max_q=40),                    # G=8
+    dict(seed=105, Hq=16, Hkv=1, D=128, max_ctx=400, max_q=30),                   # G=16
+    dict(seed=106, Hq=6, Hkv=2, D=128, max_ctx=500, max_q=90),                    # G=3 (R=40)
+    dict(seed=107, Hq=4, Hkv=2, D=64, max_ctx=600, max_q=80, gaps=True),
+    dict(seed=108, Hq=8, Hkv=2, D=128, max_ctx=600, max_q=100, hybrid=True, gaps=True),
+    dict(seed=109, Hq=4, Hkv=2, D=128, max_ctx=300, max_q=8, n_req=12, max_segs=8),   # short queries
+    dict(seed=110, Hq=4, Hkv=2, D=64, max_ctx=40, max_q=3, n_req=10, max_segs=4),     # tiny everything
+    dict(seed=111, Hq=4, Hkv=2, D=128, max_ctx=500, max_q=64, q_to_kv=[1, 0, 0, 1]),   # custom GQA map
+    dict(seed=112, Hq=8, Hkv=2, D=128, max_ctx=800, max_q=200, ragged=False),
+    dict(seed=113, Hq=4, Hkv=2, D=128, max_ctx=700, max_q=64, arena_gap=5),
+]
+
+
+@pytest.mark.parametrize("kw", CASES, ids=lambda k: f"seed{k['seed']}")
+def test_random_small_problems(kw):
+    p = W.random_problem(device=DEV, **kw)
+    o, lse, _ = gpu_forward(p)
+    compare(p, o, lse, strict=False)
+
+
+@pytest.mark.parametrize("seed", [201, 202])
+def test_nan_poisoned_slack_never_reaches_output(seed):
+    """Block tails, unused blocks and arena gaps hold NaN (SURVEY.md hard part 4)."""
+    p = W.random_problem(seed, Hq=8, Hkv=2, D=128, max_ctx=600, max_q=70, fill="nan", arena_gap=3, device=DEV)
+    assert torch.isnan(p.pool_k.float()).any()
+    o, lse, _ = gpu_forward(p)
+    compare(p, o, lse, strict=False)
+
+
+def test_empty_rows_one_token_segments_and_q_len_one():
+    Hq, Hkv, D = 4, 2, 128
+    # run 0: positions 0..4 but the only keys sit at 3..(1-token segments) -> rows 0..2 see nothing
+    c0 = ContextSpec([(SEG_PAGED, 3, 1), (SEG_CONTIG, 4, 1), (SEG_PAGED, 9, 1)])
+    # run 1: a single query token far behind a ragged context
+    c1 = ContextSpec([(SEG_PAGED, 0, 131), (SEG_CONTIG, 131, 1), (SEG_SELF, 132, 1)])
+    # run 2: every key lies after the run (fully masked)
+    c2 = ContextSpec([(SEG_CONTIG, 50, 20)])
+    p = build_problem("edge", Hq, Hkv, D, [c0, c1, c2], [RunSpec(0, 0, 5), RunSpec(1, 132, 1), RunSpec(2, 10, 7)],
+                      seed=7, device=DEV, keep_dense=True, fill="nan")
+    o, lse, _ = gpu_forward(p)
+    compare(p, o, lse, strict=False)
+    assert np.all(np.isneginf(lse[:3])) and np.all(np.isneginf(lse[6:13]))
+
+
+def test_split_kv_merge_path_and_determinism():
+    """Few long streams: the persistent schedule must split them along KV and merge."""
+    Hq, Hkv, D = 8, 2, 128
+    ctx = ContextSpec([(SEG_PAGED, 0, 3000), (SEG_CONTIG, 3000, 1777), (SEG_PAGED, 4777, 1500), (SEG_SELF, 6277, 40)])
+    p = build_problem("split", Hq, Hkv, D, [ctx], [RunSpec(0, 6277, 40)], seed=8, device=DEV, keep_dense=True)
+    with MsaSession(p) as s:
+        assert s.info["num_split_items"] > 0 and s.info["num_partials"] > s.info["num_split_items"]
+        o1, l1 = s.forward()
+        o1, l1 = o1.clone(), l1.clone()
+        assert msa_last_launch_count(s.h) == 2
+        o2, l2 = s.forward()
+        torch.cuda.synchronize()
+        assert torch.equal(o1, o2) and torch.equal(l1, l2), "run-to-run determinism"
+        compare(p, o1.float().cpu().numpy().astype(np.float64), l1.cpu().numpy().astype(np.float64))
+
+
+def test_empty_batch_and_zero_length_run():
+    p = W.random_problem(5, n_req=2, Hq=4, Hkv=2, D=64, device=DEV)
+    h = msa_create(p.Hq, p.Hkv, p.D)
+    try:
+        R, n, S, m = make_descriptors(np.zeros((0, 5), np.int32), [], [], [], [], [])
+        plan = msa_plan_create(h, R, 0, S, 0)
+        o = torch.zeros_like(p.q)
+        lse = torch.zeros(p.total_q, p.Hq, device=DEV)
+        msa_forward(h, plan, p.q, p.pool_k, p.pool_v, p.block_table, p.contig_k, p.contig_v, p.scale, o, lse)
+        assert msa_last_launch_count(h) == 0
+        msa_plan_destroy(plan)
+    finally:
+        msa_destroy(h)
+    p.req[1, 1] = 0                                   # second run has no rows
+    o, lse, _ = gpu_forward(p)
+    rr = np.zeros(int(p.req[0, 1]), np.int32)
+    compare(p, o, lse, rr, np.arange(int(p.req[0, 1]), dtype=np.int32), strict=False)
+
+
+def test_forward_host_matches_forward_and_error_codes():
+    p = W.random_problem(31, n_req=3, Hq=8, Hkv=2, D=128, max_ctx=3000, max_q=64, device=DEV, min_ctx=2000)
+    with MsaSession(p) as s:
+        o, lse = s.forward()
+        torch.cuda.synchronize()
+        qh = p.q.cpu().pin_memory()
+        ck, cv = p.contig_k.cpu().pin_memory(), p.contig_v.cpu().pin_memory()
+        bt = p.block_table.cpu().pin_memory()
+        oh = torch.empty_like(qh).pin_memory()
+        lh = torch.empty(p.total_q, p.Hq, dtype=torch.float32).pin_memory()
+        msa_forward_host(s.h, s.plan, qh, p.pool_k, p.pool_v, bt, ck, cv, p.scale, oh, lh,
+                         torch.cuda.current_stream().cuda_stream)
+        assert torch.equal(oh, o.cpu()) and torch.equal(lh, lse.cpu())
+        # error paths: nothing is launched, status says why
+        with pytest.raises(MsaError) as e:
+            msa_forward(s.h, s.plan, p.q[1:], p.pool_k, p.pool_v, p.block_table, p.contig_k, p.contig_v, p.scale,
+                        s.o, s.lse, s.workspace)
+        assert e.value.status == MSA_ERR_OUT_OF_RANGE
+        with pytest.raises(MsaError) as e:
+            msa_forward(s.h, s.plan, p.q, p.pool_k, p.pool_v, p.block_table, p.contig_k[:5], p.contig_v, p.scale,
+                        s.o, s.lse, s.workspace)
+        assert e.value.status == MSA_ERR_OUT_OF_RANGE
+        if s.workspace is not None:
+            with pytest.raises(MsaError) as e:
+                msa_forward(s.h, s.plan, p.q, p.pool_k, p.pool_v, p.block_table, p.contig_k, p.contig_v, p.scale,
+                            s.o, s.lse, s.workspace[:16])
+            assert e.value.status == MSA_ERR_WORKSPACE
+        mis = torch.empty(p.q.numel() + 8, dtype=torch.bfloat16, device=DEV)[1:1 + p.q.numel()].view_as(p.q)
+        with pytest.raises(MsaError) as e:
+            msa_forward(s.h, s.plan, mis, p.pool_k, p.pool_v, p.block_table, p.contig_k, p.contig_v, p.scale,
+                        s.o, s.lse, s.workspace)
+        assert e.value.status == MSA_ERR_MISALIGNED
+
+
+# ------------------------------------------------------------------ configs 2-5 at full size (sampled rows)
+def _full_config(name, n_req_sample, n_random, seed):
+    p = W.CONFIGS[name](device=DEV)
+    o, lse, info = gpu_forward(p)
+    rng = np.random.default_rng(seed)
+    reqs = sorted(int(x) for x in rng.choice(p.n_req, size=min(n_req_sample, p.n_req), replace=False))
+    rr, ii = W.pick_rows(p, n_random, seed, reqs)
+    stats = compare(p, o, lse, rr, ii, strict=True)
+    assert info["visible_pairs"] == W.visible_pairs(p)
+    print(name, "rows", len(rr), "max|dO| mean|dO| max|dLSE|", stats, info)
+
+
+def test_cfg2_llama8b_full_size_sampled_rows():
+    _full_config("cfg2_llama8b", 8, 6, 2)
+
+
+def test_cfg3_70b_long_full_size_sampled_rows():
+    _full_config("cfg3_70b_long", 1, 24, 3)
+
+
+def test_cfg4_mixed_full_size_sampled_rows():
+    _full_config("cfg4_mixed", 6, 4, 4)
+
+
+def test_cfg5_short_query_full_size_sampled_rows():
+    _full_config("cfg5_short_query", 24, 0, 5)
