@@ -1,0 +1,328 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the MSA hot path on B200 (one JSON line on stdout).
+
+A "step" is one pass of the whole hot path (plan reused; forward kernel + LSE-merge kernel)
+over one synthetic batch.  Default workload = BASELINE.json configs[1] (Llama-3-8B-shaped
+layer), metric = MSA attention TFLOP/s (algorithmic FLOPs = 4*D*Hq*visible pairs).
+`--workload cfg5_short_query` reports the memory-bound metric (HBM GB/s) instead; at N=1
+the default run appends it as `secondary`.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl reference]
+
+N>1: launched by torchrun, one rank per GPU, every rank runs its own replica of the batch
+(work units are independent: no data-path collective, "weak" scaling); time = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+
+def _env_int(name: str, default: int) -> int:
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+def measured_peaks():
+    """(tflops, gbs, label): driver-measured peaks, else the profiling guide's fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["bf16_tflops"]), float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json, burst bf16 / copy GB/s)"
+    except Exception:
+        return 1590.0, 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def committed_traffic(workload: str):
+    """dram bytes per launch of the dominant kernel from the committed ncu capture, or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "roofline_traffic.json")) as f:
+            return json.load(f).get(workload)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """Polls SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.hd = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.hd, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.hd, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.hd))
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def start(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join(timeout=1.0)
+        med = int(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def oracle_sample(p, n_rows: int, seed: int, reqs=None):
+    """Time the fp64 oracle, as it stands, on a bounded row sample.  Returns (seconds, flops, pairs)."""
+    import oracle
+    rng = np.random.default_rng(seed)
+    if reqs is None:
+        reqs = [int(rng.integers(0, p.n_req))]
+    rr, ii = [], []
+    per = max(1, n_rows // len(reqs))
+    for r in reqs:
+        T = int(p.req[r, 1])
+        idx = np.sort(rng.choice(T, size=min(per, T), replace=False))
+        rr += [r] * len(idx)
+        ii += [int(x) for x in idx]
+    rr, ii = np.asarray(rr, np.int32), np.asarray(ii, np.int32)
+    arrays = p.host_arrays(reqs=reqs)
+    pairs = 0
+    for r, i in zip(rr, ii):
+        pos = int(p.req[r, 2]) + int(i)
+        sb, sc = int(p.req[r, 3]), int(p.req[r, 4])
+        for s in range(sb, sb + sc):
+            pairs += int(np.clip(pos - int(p.seg_abs_start[s]) + 1, 0, int(p.seg_len[s])))
+    t0 = time.perf_counter()
+    oracle.forward(arrays, p.Hq, p.Hkv, p.D, p.scale, rr, ii)
+    dt = time.perf_counter() - t0
+    return dt, 4.0 * p.D * p.Hq * pairs, pairs, len(rr)
+
+
+def metric_of(workload: str):
+    if workload == "cfg5_short_query":
+        return "msa_short_query_hbm_gbs", "GB/s", "hbm"
+    return "msa_attention_tflops", "TFLOP/s", "tensor"
+
+
+def run_mine(args, rank: int, world: int, local_rank: int):
+    import torch
+    import workloads as W
+    from paper_2606_02964_b200 import (MsaSession, msa_forward_host, msa_get_timing, msa_last_launch_count,
+                                       msa_set_timing)
+    import __graft_entry__ as ge
+    if rank == 0:
+        ge.build()
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        dist.barrier()
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    tfl_peak, gbs_peak, peak_label = measured_peaks()
+
+    def bench_workload(name: str, steps: int, warmup: int, do_e2e: bool):
+        metric, unit, bound = metric_of(name)
+        p = W.CONFIGS[name](device=dev)
+        alg = p.algorithmic()
+        units_per_step = alg["flops"] / 1e12 if bound == "tensor" else alg["bytes"] / 1e9
+        s = MsaSession(p, device=local_rank)
+        stream = torch.cuda.current_stream().cuda_stream
+        for _ in range(max(3, warmup)):
+            s.forward(stream)
+        torch.cuda.synchronize()
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        sampler = ClockSampler(local_rank)
+        msa_set_timing(s.h, steps)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        sampler.start()
+        e0.record()
+        launches = 0
+        for _ in range(steps):
+            s.forward(stream)
+            launches += msa_last_launch_count(s.h)
+        e1.record()
+        torch.cuda.synchronize()
+        clocks = sampler.stop()
+        ms = e0.elapsed_time(e1) / steps
+        n_rec, fwd_ms, merge_ms = msa_get_timing(s.h)
+        msa_set_timing(s.h, 0)
+        if world > 1:
+            import torch.distributed as dist
+            t = torch.tensor([ms], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        value = world * units_per_step / (ms * 1e-3)
+        kern_units = units_per_step          # the forward kernel does all algorithmic work of a step
+        achieved = kern_units / (fwd_ms * 1e-3) if fwd_ms > 0 else None
+        peak = tfl_peak if bound == "tensor" else gbs_peak
+        traffic = committed_traffic(name)
+        out = dict(metric=metric, value=value, unit=unit, ms_per_step=ms, gpu_launches=launches,
+                   roofline=dict(bound=bound, achieved=achieved, peak=peak, unit=unit,
+                                 frac=(achieved / peak) if achieved else None, traffic=traffic,
+                                 kernel="msa_fwd", kernel_ms=fwd_ms, merge_ms=merge_ms, steps_timed=n_rec,
+                                 peak_source=peak_label,
+                                 frac_of_nominal=(achieved / (2250.0 if bound == "tensor" else 8000.0)) if achieved else None),
+                   clocks=clocks, plan=s.info, algorithmic=alg)
+        if do_e2e:
+            qh = p.q.cpu().pin_memory()
+            ck, cv = p.contig_k.cpu().pin_memory(), p.contig_v.cpu().pin_memory()
+            bt = p.block_table.cpu().pin_memory()
+            oh = torch.empty_like(qh).pin_memory()
+            lh = torch.empty(p.total_q, p.Hq, dtype=torch.float32).pin_memory()
+            k_e2e = max(3, min(steps, 20))
+            for _ in range(2):
+                msa_forward_host(s.h, s.plan, qh, p.pool_k, p.pool_v, bt, ck, cv, p.scale, oh, lh, stream)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(k_e2e):
+                msa_forward_host(s.h, s.plan, qh, p.pool_k, p.pool_v, bt, ck, cv, p.scale, oh, lh, stream)
+            e1.record()
+            torch.cuda.synchronize()
+            ems = e0.elapsed_time(e1) / k_e2e
+            if world > 1:
+                import torch.distributed as dist
+                t = torch.tensor([ems], device=dev, dtype=torch.float64)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                ems = float(t.item())
+            h2d = qh.numel() * 2 + ck.numel() * 2 + cv.numel() * 2 + bt.numel() * 4
+            d2h = oh.numel() * 2 + lh.numel() * 4
+            out["e2e"] = dict(value=world * units_per_step / (ems * 1e-3), unit=unit, ms_per_step=ems, steps=k_e2e,
+                              h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
+                              note="msa_forward_host: q, block table, contiguous arena from pinned host memory; "
+                                   "O and LSE back to host; the paged pool is the resident KV cache")
+        s.close()
+        return out, p
+
+    res, p = bench_workload(args.workload, args.steps, args.warmup, do_e2e=True)
+    line = dict(metric=res["metric"], value=res["value"], unit=res["unit"], n_gpus=world, steps=args.steps,
+                warmup=max(3, args.warmup), ms_per_step=res["ms_per_step"], higher_is_better=True, scaling="weak",
+                vs_baseline=None, dtype="bf16", data="synthetic",
+                config=dict(workload=args.workload, Hq=p.Hq, Hkv=p.Hkv, head_dim=p.D, requests=p.n_req,
+                            total_q=p.total_q, kv_tokens=p.kv_tokens(), block_size=16,
+                            l2_policy="inputs larger than L2 (%.0f MB per step), no flush" % (res["algorithmic"]["bytes"] / 1e6),
+                            parallelism=f"replicas x{world}" if world > 1 else "single GPU"),
+                clocks=res["clocks"], e2e=res.get("e2e"), gpu_launches=res["gpu_launches"],
+                roofline=res["roofline"], plan=res["plan"])
+    if rank == 0 and world == 1:
+        # the oracle, as it stands, on a bounded sample of the same workload (reported baseline)
+        import oracle
+        reqs = list(range(min(2, p.n_req)))
+        dt, fl, pairs, n = oracle_sample(p, 8, 1, reqs)                     # calibrate
+        rows = int(np.clip(15.0 / max(dt / n, 1e-6), 16, 4096))
+        dt, fl, pairs, n = oracle_sample(p, rows, 2, reqs)
+        unit = res["unit"]
+        if unit == "TFLOP/s":
+            cv = fl / dt / 1e12
+        else:
+            cv = pairs * p.Hkv * p.D * 2 * 2 / dt / 1e9     # K and V bytes of the visible keys, per kv head
+        line["cpu_baseline"] = dict(value=cv, unit=unit, cores=oracle.num_threads(), kind="oracle",
+                                    sample=f"{n} query rows of requests {reqs} (all {p.Hq} heads), {dt:.2f} s",
+                                    seconds=dt)
+        if args.workload == "cfg2_llama8b" and not args.no_secondary:
+            del p
+            torch.cuda.empty_cache()
+            sec, p5 = bench_workload("cfg5_short_query", max(10, min(args.steps, 50)), args.warmup, do_e2e=False)
+            line["secondary"] = dict(workload="cfg5_short_query", metric=sec["metric"], value=sec["value"],
+                                     unit=sec["unit"], ms_per_step=sec["ms_per_step"], roofline=sec["roofline"],
+                                     clocks=sec["clocks"], plan=sec["plan"])
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line))
+
+
+def run_reference(args, rank: int, world: int):
+    """The reference arm of this tier = the fp64 CPU oracle on the box's host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    import oracle
+    import workloads as W
+    import __graft_entry__ as ge
+    ge.build()
+    metric, unit, bound = metric_of(args.workload)
+    p = W.CONFIGS[args.workload](device="cpu") if args.workload in ("cfg1_tiny",) else None
+    if p is None:
+        # values on the CPU; only the requests sampled are ever read
+        small = dict(cfg2_llama8b=dict(n_req=2), cfg4_mixed=dict(n_req=4), cfg5_short_query=dict(n_req=8))
+        p = W.CONFIGS[args.workload](device="cpu", **small.get(args.workload, {}))
+    reqs = list(range(min(2, p.n_req)))
+    dt, fl, pairs, n = oracle_sample(p, 8, 1, reqs)
+    total = max(1, args.steps + args.warmup)
+    rows = int(np.clip((90.0 / total) / max(dt / n, 1e-6), 4, 2048))
+    for _ in range(args.warmup):
+        oracle_sample(p, rows, 3, reqs)
+    t_sum, f_sum, p_sum, n_sum = 0.0, 0.0, 0, 0
+    for k in range(args.steps):
+        dt, fl, pairs, n = oracle_sample(p, rows, 10 + k, reqs)
+        t_sum, f_sum, p_sum, n_sum = t_sum + dt, f_sum + fl, p_sum + pairs, n_sum + n
+    if bound == "tensor":
+        value = f_sum / t_sum / 1e12
+    else:
+        value = p_sum * p.Hkv * p.D * 2 * 2 / t_sum / 1e9      # K and V bytes of the visible keys, per kv head
+    sample = f"{n_sum // max(1, args.steps)} query rows per step of requests {reqs} (all {p.Hq} heads)"
+    line = dict(impl="reference", metric=metric, value=value, unit=unit, n_gpus=world, steps=args.steps,
+                warmup=args.warmup, ms_per_step=1e3 * t_sum / max(1, args.steps), higher_is_better=True,
+                scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+                config=dict(workload=args.workload, Hq=p.Hq, Hkv=p.Hkv, head_dim=p.D, sample=sample),
+                cpu_baseline=dict(value=value, unit=unit, cores=oracle.num_threads(), kind="oracle", sample=sample),
+                e2e=dict(value=value, unit=unit, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="mine", choices=["mine", "reference"])
+    ap.add_argument("--workload", default="cfg2_llama8b",
+                    choices=["cfg2_llama8b", "cfg3_70b_long", "cfg4_mixed", "cfg5_short_query"])
+    ap.add_argument("--no-secondary", action="store_true")
+    args = ap.parse_args()
+    rank, world, local_rank = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_mine(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

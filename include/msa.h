@@ -183,6 +183,14 @@ int msa_forward_host(msa_handle h, msa_plan p,
 /* Number of kernels the last msa_forward / msa_forward_host on this handle launched. */
 int msa_last_launch_count(msa_handle h);
 
+/* Per-kernel device timing for benchmarks.  msa_set_timing(h, n) makes the next n calls of
+ * msa_forward record CUDA events on their stream around the forward kernel and the merge
+ * kernel (n = 0 switches it off); msa_get_timing waits for the last recorded step, returns
+ * how many steps were recorded and the average duration of each kernel in milliseconds,
+ * and restarts the recording window. */
+int msa_set_timing(msa_handle h, int max_steps);
+int msa_get_timing(msa_handle h, int32_t *steps, double *fwd_ms_avg, double *merge_ms_avg);
+
 const char *msa_strerror(int status);
 /* Text of the last CUDA error seen by this thread inside the library ("" if none). */
 const char *msa_last_cuda_error(void);

@@ -57,7 +57,7 @@ _LIB: Optional[ctypes.CDLL] = None
 
 EXPORTS = ["msa_create", "msa_destroy", "msa_plan_create", "msa_plan_destroy", "msa_plan_get_info",
            "msa_plan_export", "msa_workspace_bytes", "msa_forward", "msa_forward_host",
-           "msa_last_launch_count", "msa_strerror", "msa_last_cuda_error", "msa_version"]
+           "msa_last_launch_count", "msa_set_timing", "msa_get_timing", "msa_strerror", "msa_last_cuda_error", "msa_version"]
 
 
 def _lib() -> ctypes.CDLL:
@@ -81,6 +81,9 @@ def _lib() -> ctypes.CDLL:
         lib.msa_forward.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, i64, f32, vp, vp, vp, sz, vp]
         lib.msa_forward_host.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, i64, f32, vp, vp, vp]
         lib.msa_last_launch_count.argtypes = [vp]
+        lib.msa_set_timing.argtypes = [vp, ctypes.c_int]
+        lib.msa_get_timing.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(ctypes.c_double),
+                                       ctypes.POINTER(ctypes.c_double)]
         for f in ("msa_strerror", "msa_last_cuda_error", "msa_version"):
             getattr(lib, f).restype = ctypes.c_char_p
         lib.msa_strerror.argtypes = [ctypes.c_int]
@@ -207,6 +210,17 @@ def msa_forward_host(h, p, q_host, pool_k, pool_v, block_table_host, contig_k_ho
 
 def msa_last_launch_count(h) -> int:
     return int(_lib().msa_last_launch_count(h))
+
+
+def msa_set_timing(h, max_steps: int) -> None:
+    _check(_lib().msa_set_timing(h, max_steps), "msa_set_timing")
+
+
+def msa_get_timing(h) -> Tuple[int, float, float]:
+    """(steps recorded, average forward-kernel ms, average merge-kernel ms)."""
+    n, a, b = ctypes.c_int32(0), ctypes.c_double(0), ctypes.c_double(0)
+    _check(_lib().msa_get_timing(h, ctypes.byref(n), ctypes.byref(a), ctypes.byref(b)), "msa_get_timing")
+    return int(n.value), float(a.value), float(b.value)
 
 
 # --------------------------------------------------------------------------- convenience

@@ -69,6 +69,10 @@ struct msa_handle_s {
     int32_t *d_kv_to_q = nullptr;
     EncodeTiledFn encode = nullptr;
     int last_launches = 0;
+    // optional per-launch timing (msa_set_timing): 3 events per recorded step
+    bool timing = false;
+    std::vector<cudaEvent_t> ev;
+    int ev_steps = 0;
     // staging for msa_forward_host
     DevBuf s_q, s_o, s_lse, s_ck, s_cv, s_bt, s_ws;
 };
@@ -180,6 +184,7 @@ void msa_destroy(msa_handle h)
     if (!h) return;
     if (!h->planning_only) {
         if (h->d_kv_to_q) cudaFree(h->d_kv_to_q);
+        for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
         h->s_q.release(); h->s_o.release(); h->s_lse.release(); h->s_ck.release();
         h->s_cv.release(); h->s_bt.release(); h->s_ws.release();
     }
@@ -378,7 +383,11 @@ int msa_forward(msa_handle h, msa_plan p, const void *q, int64_t total_q, const 
     fp.G = h->G;
     fp.R = h->R;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const bool rec = h->timing && static_cast<size_t>(h->ev_steps) * 3 + 3 <= h->ev.size();
+    cudaEvent_t *ev = rec ? &h->ev[static_cast<size_t>(h->ev_steps) * 3] : nullptr;
+    if (rec) MSA_CUDA(cudaEventRecord(ev[0], stream));
     MSA_CUDA(launch_fwd(fp, D, hp.info.num_ctas, h->variant, stream));
+    if (rec) MSA_CUDA(cudaEventRecord(ev[1], stream));
     h->last_launches = 1;
     if (!hp.merge_items.empty()) {
         MergeParams mp;
@@ -392,6 +401,10 @@ int msa_forward(msa_handle h, msa_plan p, const void *q, int64_t total_q, const 
         mp.D = D;
         MSA_CUDA(launch_merge(mp, static_cast<int>(hp.merge_items.size()), stream));
         h->last_launches = 2;
+    }
+    if (rec) {
+        MSA_CUDA(cudaEventRecord(ev[2], stream));
+        ++h->ev_steps;
     }
     return MSA_OK;
 }
@@ -441,5 +454,42 @@ int msa_forward_host(msa_handle h, msa_plan p, const void *q_host, int64_t total
 }
 
 int msa_last_launch_count(msa_handle h) { return h ? h->last_launches : 0; }
+
+int msa_set_timing(msa_handle h, int max_steps)
+{
+    if (!h || max_steps < 0) return MSA_ERR_INVALID_ARG;
+    if (h->planning_only) return MSA_ERR_NO_DEVICE;
+    for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
+    h->ev.clear();
+    h->ev_steps = 0;
+    h->timing = max_steps > 0;
+    for (int i = 0; i < max_steps * 3; ++i) {
+        cudaEvent_t e;
+        MSA_CUDA(cudaEventCreate(&e));
+        h->ev.push_back(e);
+    }
+    return MSA_OK;
+}
+
+int msa_get_timing(msa_handle h, int32_t *steps, double *fwd_ms_avg, double *merge_ms_avg)
+{
+    if (!h || !steps || !fwd_ms_avg || !merge_ms_avg) return MSA_ERR_INVALID_ARG;
+    *steps = h->ev_steps;
+    *fwd_ms_avg = *merge_ms_avg = 0.0;
+    if (h->ev_steps == 0) return MSA_OK;
+    MSA_CUDA(cudaEventSynchronize(h->ev[static_cast<size_t>(h->ev_steps) * 3 - 1]));
+    double a = 0.0, b = 0.0;
+    for (int i = 0; i < h->ev_steps; ++i) {
+        float f = 0.f, m = 0.f;
+        MSA_CUDA(cudaEventElapsedTime(&f, h->ev[i * 3], h->ev[i * 3 + 1]));
+        MSA_CUDA(cudaEventElapsedTime(&m, h->ev[i * 3 + 1], h->ev[i * 3 + 2]));
+        a += f;
+        b += m;
+    }
+    *fwd_ms_avg = a / h->ev_steps;
+    *merge_ms_avg = b / h->ev_steps;
+    h->ev_steps = 0;
+    return MSA_OK;
+}
 
 }  // extern "C"
