@@ -130,9 +130,11 @@ int msa_plan_get_info(msa_plan p, msa_plan_info *info);
 /* Introspection (tests, tools): copy one of the plan's host-side arrays out.
  *   which = 0  virtual blocks      int32[4]  {src, abs_start, nvalid, paged}
  *           1  work units          int32[12] {q_row0, n_tok, q_abs0, kvh, vb_begin, vb_count,
- *                                             tile_begin, tile_end, partial_off, 0, 0, 0}
+ *                                             tile_begin, tile_end, partial_off, mode,
+ *                                             tile_info_begin, 0}
  *           2  cta_unit_begin      int32     [num_ctas + 1]
  *           3  merge items         {int32 q_row0, n_tok, kvh, n_partials; int64 first_off, stride}
+ *           4  tile mask summaries int32[2]  {max_abs, ragged} per context KV tile
  * With buf == NULL only *bytes is set; otherwise *bytes is the capacity on entry. */
 int msa_plan_export(msa_plan p, int which, void *buf, size_t *bytes);
 

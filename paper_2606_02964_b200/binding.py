@@ -159,10 +159,11 @@ _EXPORT_DTYPES = {
     0: np.dtype([("src", "<i4"), ("abs_start", "<i4"), ("nvalid", "<i4"), ("paged", "<i4")]),
     1: np.dtype([("q_row0", "<i4"), ("n_tok", "<i4"), ("q_abs0", "<i4"), ("kvh", "<i4"), ("vb_begin", "<i4"),
                  ("vb_count", "<i4"), ("tile_begin", "<i4"), ("tile_end", "<i4"), ("partial_off", "<i4"),
-                 ("r0", "<i4"), ("r1", "<i4"), ("r2", "<i4")]),
+                 ("mode", "<i4"), ("tile_info_begin", "<i4"), ("r2", "<i4")]),
     2: np.dtype("<i4"),
     3: np.dtype([("q_row0", "<i4"), ("n_tok", "<i4"), ("kvh", "<i4"), ("n_partials", "<i4"),
                  ("first_off", "<i8"), ("stride", "<i8")]),
+    4: np.dtype([("max_abs", "<i4"), ("ragged", "<i4")]),
 }
 
 

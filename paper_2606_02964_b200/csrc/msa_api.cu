@@ -6,6 +6,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <algorithm>
 #include <new>
 #include <string>
 #include <vector>
@@ -85,6 +86,7 @@ struct msa_plan_s {
     const WorkUnit *d_units = nullptr;
     const int32_t *d_cta_begin = nullptr;
     const MergeItem *d_merge = nullptr;
+    const TileInfo *d_tile_info = nullptr;
 };
 
 extern "C" {
@@ -139,7 +141,7 @@ int msa_create(const msa_config *cfg, msa_handle *out)
         h->kv_to_q[static_cast<size_t>(kv) * G + fill[kv]++] = q;
     }
     const char *kv = getenv("MSA_KERNEL");
-    h->variant = (kv && strcmp(kv, "simple") == 0) ? FwdVariant::Simple : FwdVariant::Simple;
+    h->variant = (kv && strcmp(kv, "simple") == 0) ? FwdVariant::Simple : FwdVariant::Pipelined;
 
     if (cfg->device < 0) {
         // planning-only handle: descriptor validation and scheduling on the host; every
@@ -219,7 +221,8 @@ int msa_plan_create(msa_handle h, const msa_request *requests, int32_t n_req, co
         const size_t b_un = al(hp.units.size() * sizeof(WorkUnit));
         const size_t b_cb = al(hp.cta_unit_begin.size() * sizeof(int32_t));
         const size_t b_mg = al(hp.merge_items.size() * sizeof(MergeItem));
-        const size_t total = b_vb + b_un + b_cb + b_mg + 256;
+        const size_t b_ti = al(hp.tile_info.size() * sizeof(TileInfo));
+        const size_t total = b_vb + b_un + b_cb + b_mg + b_ti + 256;
         cudaError_t e = cudaSetDevice(h->cfg.device);
         if (e == cudaSuccess) e = cudaMalloc(&p->d_buf, total);
         if (e != cudaSuccess) {
@@ -231,6 +234,7 @@ int msa_plan_create(msa_handle h, const msa_request *requests, int32_t n_req, co
         p->d_units = reinterpret_cast<const WorkUnit *>(base + b_vb);
         p->d_cta_begin = reinterpret_cast<const int32_t *>(base + b_vb + b_un);
         p->d_merge = reinterpret_cast<const MergeItem *>(base + b_vb + b_un + b_cb);
+        p->d_tile_info = reinterpret_cast<const TileInfo *>(base + b_vb + b_un + b_cb + b_mg);
         if (e == cudaSuccess && !hp.vblocks.empty())
             e = cudaMemcpy(base, hp.vblocks.data(), hp.vblocks.size() * sizeof(VBlock), cudaMemcpyHostToDevice);
         if (e == cudaSuccess && !hp.units.empty())
@@ -240,6 +244,9 @@ int msa_plan_create(msa_handle h, const msa_request *requests, int32_t n_req, co
                            cudaMemcpyHostToDevice);
         if (e == cudaSuccess && !hp.merge_items.empty())
             e = cudaMemcpy(base + b_vb + b_un + b_cb, hp.merge_items.data(), hp.merge_items.size() * sizeof(MergeItem),
+                           cudaMemcpyHostToDevice);
+        if (e == cudaSuccess && !hp.tile_info.empty())
+            e = cudaMemcpy(base + b_vb + b_un + b_cb + b_mg, hp.tile_info.data(), hp.tile_info.size() * sizeof(TileInfo),
                            cudaMemcpyHostToDevice);
         if (e != cudaSuccess) {
             cudaFree(p->d_buf);
@@ -274,7 +281,8 @@ int msa_workspace_bytes(msa_plan p, size_t *bytes)
 
 /* Introspection for tests: copies the host-side plan arrays out.
  * which: 0 = virtual blocks (int32 x4 each), 1 = work units (int32 x12 each),
- *        2 = cta_unit_begin (int32), 3 = merge items (int32 x4 + int64 x2 each).
+ *        2 = cta_unit_begin (int32), 3 = merge items (int32 x4 + int64 x2 each),
+ *        4 = per-tile mask summaries (int32 x2 each).
  * Call with buf == NULL to get the byte size. */
 int msa_plan_export(msa_plan p, int which, void *buf, size_t *bytes)
 {
@@ -286,6 +294,7 @@ int msa_plan_export(msa_plan p, int which, void *buf, size_t *bytes)
     case 1: src = p->hp.units.data(); n = p->hp.units.size() * sizeof(WorkUnit); break;
     case 2: src = p->hp.cta_unit_begin.data(); n = p->hp.cta_unit_begin.size() * sizeof(int32_t); break;
     case 3: src = p->hp.merge_items.data(); n = p->hp.merge_items.size() * sizeof(MergeItem); break;
+    case 4: src = p->hp.tile_info.data(); n = p->hp.tile_info.size() * sizeof(TileInfo); break;
     default: return MSA_ERR_INVALID_ARG;
     }
     if (buf) {
@@ -361,17 +370,22 @@ int msa_forward(msa_handle h, msa_plan p, const void *q, int64_t total_q, const 
     const void *pv = hp.uses_paged ? pool_v : q;
     const uint64_t prow = hp.uses_paged ? static_cast<uint64_t>(num_blocks) * MSA_BLOCK_SIZE : static_cast<uint64_t>(total_q);
     const uint64_t pin = hp.uses_paged ? static_cast<uint64_t>(Hkv) * D : static_cast<uint64_t>(Hq) * D;
-    if ((rc = encode_2d(h, &fp.tm_pool_k, pk, pin, prow, MSA_BLOCK_SIZE)) != MSA_OK) return rc;
-    if ((rc = encode_2d(h, &fp.tm_pool_v, pv, pin, prow, MSA_BLOCK_SIZE)) != MSA_OK) return rc;
+    for (int i = 0; i < 5; ++i) {
+        if ((rc = encode_2d(h, &fp.tm_pool_k[i], pk, pin, prow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
+        if ((rc = encode_2d(h, &fp.tm_pool_v[i], pv, pin, prow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
+    }
     const void *ck = hp.uses_contig ? contig_k : q;
     const void *cv = hp.uses_contig ? contig_v : q;
     const uint64_t crow = hp.uses_contig ? static_cast<uint64_t>(contig_rows) : static_cast<uint64_t>(total_q);
     const uint64_t cin = hp.uses_contig ? static_cast<uint64_t>(Hkv) * D : static_cast<uint64_t>(Hq) * D;
-    if ((rc = encode_2d(h, &fp.tm_ctg_k, ck, cin, crow, MSA_BLOCK_SIZE)) != MSA_OK) return rc;
-    if ((rc = encode_2d(h, &fp.tm_ctg_v, cv, cin, crow, MSA_BLOCK_SIZE)) != MSA_OK) return rc;
+    for (int i = 0; i < 5; ++i) {
+        if ((rc = encode_2d(h, &fp.tm_ctg_k[i], ck, cin, crow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
+        if ((rc = encode_2d(h, &fp.tm_ctg_v[i], cv, cin, crow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
+    }
     fp.vblocks = p->d_vblocks;
     fp.units = p->d_units;
     fp.cta_unit_begin = p->d_cta_begin;
+    fp.tile_info = p->d_tile_info;
     fp.block_table = block_table;
     fp.kv_to_q = h->d_kv_to_q;
     fp.o = o;
@@ -399,7 +413,9 @@ int msa_forward(msa_handle h, msa_plan p, const void *q, int64_t total_q, const 
         mp.Hq = Hq;
         mp.G = h->G;
         mp.D = D;
-        MSA_CUDA(launch_merge(mp, static_cast<int>(hp.merge_items.size()), stream));
+        int max_rows = 0;
+        for (const MergeItem &mi : hp.merge_items) max_rows = std::max(max_rows, mi.n_tok * h->G);
+        MSA_CUDA(launch_merge(mp, static_cast<int>(hp.merge_items.size()), max_rows, stream));
         h->last_launches = 2;
     }
     if (rec) {

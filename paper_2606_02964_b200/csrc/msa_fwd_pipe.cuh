@@ -1,0 +1,528 @@
+// msa_fwd_pipe: the warp-specialised, pipelined MSA forward kernel for sm_100a.
+//
+// One persistent CTA per SM (512 threads), roles by warp:
+//   warps 0-3   softmax warpgroup of chain 0   (one thread per packed (head, token) row)
+//   warps 4-7   softmax warpgroup of chain 1
+//   warps 8-11  epilogue warpgroup (O / l -> bf16, LSE, split-KV partials; in-CTA merge)
+//   warp  12    loader: virtual blocks -> TMA boxes (paged and contiguous alike)
+//   warp  13    MMA issuer: tcgen05.mma for S = Q K^T and O += P V, accumulators in TMEM
+//   warps 14-15 idle (they only complete the 4-warp group setmaxnreg needs)
+//
+// Two independent "chains" keep the tensor core busy while the other chain's softmax runs:
+//   kModePair   chain c owns q tile c of the unit; both chains consume every KV tile
+//   kModeSplit  one q tile; chain c owns KV tiles c, c+2, ... with its own (m, l, O);
+//               the epilogue merges the two partial softmaxes (short / decode-like queries)
+// TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P (bf16) aliases
+// the first 64 columns of its S.  Shared memory: Q 2 tiles, one ring of 5 K/V tile slots.
+//
+// Invalid KV slots (block tails, blocks past a context's end) never reach O: their scores
+// are replaced by -inf, and their K/V rows are never written by TMA -- partly filled blocks
+// load through 8/4/2/1-row boxes -- so those smem rows keep earlier, valid (finite) tile
+// data (the ring is zeroed once at kernel start) and P = 0 times a finite value stays 0.
+#pragma once
+#include <math.h>
+
+#include "msa_kernels.h"
+#include "msa_ptx.cuh"
+
+namespace msa {
+
+template <int D>
+struct PipeCfg {
+    static constexpr int kHalves = D / 64;
+    static constexpr int kHalfBytes = kTileM * 128;                  // 128 rows x 128 B
+    static constexpr int kTileBytes = kHalves * kHalfBytes;
+    static constexpr int kStages = 5;
+    static constexpr int kQBytes = 2 * kTileBytes;
+    static constexpr int kRingBytes = kStages * kTileBytes;
+    static constexpr int kStatsBytes = 2 * kTileM * 2 * 4;           // [chain][row]{l, m}
+    static constexpr int kBarBytes = 256;
+    static constexpr int kSmemBytes = kQBytes + kRingBytes + kStatsBytes + kBarBytes;
+    static constexpr uint32_t kColS = 0, kColO = 256, kChainCols = 128;
+    static constexpr float kRescaleThreshold = 8.0f;                 // log2 units (lazy rescale)
+};
+
+enum PipeBar : int {
+    kBarQFull = 0, kBarQEmpty = 1,
+    kBarKvFull = 2,      // [5]
+    kBarKvEmpty = 7,     // [5]
+    kBarSFull = 12,      // [2]
+    kBarPFull = 14,      // [2]
+    kBarOFull = 16,      // [2]
+    kBarOFree = 18,      // [2]
+    kBarStFull = 20,     // [2]
+    kBarStFree = 22,     // [2]
+    kBarCount = 24
+};
+
+struct RingPos {
+    uint32_t slot, phase;
+    __device__ __forceinline__ void advance(int stages)
+    {
+        if (++slot == static_cast<uint32_t>(stages)) {
+            slot = 0;
+            phase ^= 1;
+        }
+    }
+};
+
+struct ResolvedVb {
+    int32_t row;      // first row in the pool / arena row space
+    int32_t nvalid;   // 0: nothing to load
+    int32_t paged;
+};
+
+template <int D>
+__global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_constant__ FwdParams P)
+{
+    using C = PipeCfg<D>;
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const uint32_t sbase = smem_u32(smem);
+    const uint32_t sQ = sbase, sRing = sbase + C::kQBytes;
+    float2 *stats = reinterpret_cast<float2 *>(smem + C::kQBytes + C::kRingBytes);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + C::kQBytes + C::kRingBytes + C::kStatsBytes);
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(bars + kBarCount);
+    const uint32_t bar0 = smem_u32(bars);
+    auto bar = [bar0](int i) { return bar0 + static_cast<uint32_t>(i) * 8u; };
+
+    const int warp = __shfl_sync(0xffffffffu, static_cast<int>(threadIdx.x >> 5), 0);
+    const int lane = threadIdx.x & 31;
+    if ((sbase & 1023u) != 0) __trap();
+
+    // one-time setup: zero the K/V ring (see header), barriers, TMEM
+    for (uint32_t i = threadIdx.x * 16u; i < static_cast<uint32_t>(C::kRingBytes); i += 512u * 16u)
+        *reinterpret_cast<uint4 *>(smem + C::kQBytes + i) = make_uint4(0, 0, 0, 0);
+    fence_proxy_async_smem();
+    if (threadIdx.x == 0) {
+        mbar_init(bar(kBarQFull), 1);
+        mbar_init(bar(kBarQEmpty), 1);
+        for (int i = 0; i < C::kStages; ++i) {
+            mbar_init(bar(kBarKvFull + i), 1);
+            mbar_init(bar(kBarKvEmpty + i), 1);
+        }
+        for (int c = 0; c < 2; ++c) {
+            mbar_init(bar(kBarSFull + c), 1);
+            mbar_init(bar(kBarPFull + c), 4);
+            mbar_init(bar(kBarOFull + c), 1);
+            mbar_init(bar(kBarOFree + c), 4);
+            mbar_init(bar(kBarStFull + c), 4);
+            mbar_init(bar(kBarStFree + c), 4);
+        }
+        fence_mbar_init();
+    }
+    if (warp == 13) {
+        tmem_alloc(smem_u32(tmem_slot), 512);
+        tmem_relinquish();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+    const int u_begin = P.cta_unit_begin[blockIdx.x], u_end = P.cta_unit_begin[blockIdx.x + 1];
+    const int G = P.G, R = P.R;
+    const float sl = P.scale_log2;
+
+    if (warp < 8) {
+        // =========================================================== softmax warpgroups
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 192;");
+        const int c = warp >> 2;                       // chain
+        const int row = threadIdx.x & 127;
+        const int g = row / R, t = row - g * R;
+        const uint32_t trow = tmem + (static_cast<uint32_t>((warp & 3) * 32) << 16);
+        const uint32_t tS = trow + C::kColS + c * C::kChainCols;
+        const uint32_t tO = trow + C::kColO + c * C::kChainCols;
+        uint32_t ph_s = 0, ph_stfree = 1;
+        for (int u = u_begin; u < u_end; ++u) {
+            const WorkUnit wu = P.units[u];
+            const int n = wu.tile_end - wu.tile_begin;
+            if (n <= 0) continue;
+            const bool pair = wu.mode == kModePair;
+            const int steps = pair ? n : (n - c + 1) >> 1;
+            if (steps <= 0) continue;
+            const int p_row = wu.q_abs0 + (pair ? c * R : 0) + t;
+            const int p_min = wu.q_abs0 + (pair ? c * R : 0);
+            float m = -INFINITY, l = 0.f;
+            for (int s = 0; s < steps; ++s) {
+                const int tile = wu.tile_begin + (pair ? s : 2 * s + c);
+                const TileInfo ti = P.tile_info[wu.tile_info_begin + tile];
+                const bool need_mask = ti.ragged != 0 || ti.max_abs > p_min;
+                mbar_wait(bar(kBarSFull + c), ph_s);
+                ph_s ^= 1;
+                tc_fence_after();
+                uint32_t sr[128];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) tmem_ld32(tS + q * 32, *reinterpret_cast<uint32_t(*)[32]>(&sr[q * 32]));
+                tmem_wait_ld();
+                if (need_mask) {
+                    const VBlock *vbp = P.vblocks + wu.vb_begin + tile * kVbPerTile;
+#pragma unroll
+                    for (int b = 0; b < kVbPerTile; ++b) {
+                        const int4 e = __ldg(reinterpret_cast<const int4 *>(vbp + b));   // {src, abs_start, nvalid, paged}
+                        int lim = min(e.z, p_row - e.y + 1);
+                        if (tile * kVbPerTile + b >= wu.vb_count) lim = 0;               // past the causal horizon: not loaded
+#pragma unroll
+                        for (int j = 0; j < kBlock; ++j)
+                            if (j >= lim) sr[b * kBlock + j] = 0xff800000u;             // -inf
+                    }
+                }
+                float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+#pragma unroll
+                for (int j = 0; j < 128; j += 4) {
+                    mx0 = fmaxf(mx0, __uint_as_float(sr[j]));
+                    mx1 = fmaxf(mx1, __uint_as_float(sr[j + 1]));
+                    mx2 = fmaxf(mx2, __uint_as_float(sr[j + 2]));
+                    mx3 = fmaxf(mx3, __uint_as_float(sr[j + 3]));
+                }
+                const float m_new = fmaxf(m, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)));
+                // lazy rescale: keep a stale max while the new one is within 2^8 of it
+                const bool grow = (m_new - m) * sl > C::kRescaleThreshold;
+                float alpha = 1.f;
+                if (grow) {
+                    alpha = ex2_approx((m - m_new) * sl);      // m = -inf -> 0
+                    l *= alpha;
+                    m = m_new;
+                }
+                if (s > 0 && __any_sync(0xffffffffu, grow)) {
+#pragma unroll
+                    for (int q = 0; q < D / 16; ++q) {
+                        uint32_t orr[16];
+                        tmem_ld16(tO + q * 16, orr);
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) orr[j] = __float_as_uint(__uint_as_float(orr[j]) * alpha);
+                        tmem_st16(tO + q * 16, orr);
+                    }
+                }
+                const float neg_ms = (m == -INFINITY) ? 0.f : -m * sl;
+                float sum0 = 0.f, sum1 = 0.f;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    uint32_t pk[16];
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) {
+                        const float p0 = ex2_approx(fmaf(__uint_as_float(sr[q * 32 + 2 * j]), sl, neg_ms));
+                        const float p1 = ex2_approx(fmaf(__uint_as_float(sr[q * 32 + 2 * j + 1]), sl, neg_ms));
+                        sum0 += p0;
+                        sum1 += p1;
+                        pk[j] = pack_bf16x2(p0, p1);
+                    }
+                    tmem_st16(tS + q * 16, pk);
+                }
+                l += sum0 + sum1;
+                tmem_wait_st();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(kBarPFull + c));
+            }
+            // hand (l, m) of my row to the epilogue
+            mbar_wait(bar(kBarStFree + c), ph_stfree);
+            ph_stfree ^= 1;
+            stats[c * kTileM + row] = make_float2(l, m);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(kBarStFull + c));
+        }
+    } else if (warp < 12) {
+        // =========================================================== epilogue warpgroup
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
+        const int row = threadIdx.x & 127;
+        const int g = row / R, t = row - g * R;
+        const uint32_t trow = tmem + (static_cast<uint32_t>((warp & 3) * 32) << 16);
+        uint32_t ph_st[2] = {0, 0}, ph_o[2] = {0, 0};
+        for (int u = u_begin; u < u_end; ++u) {
+            const WorkUnit wu = P.units[u];
+            const int n = wu.tile_end - wu.tile_begin;
+            const bool pair = wu.mode == kModePair;
+            const int rows_total = wu.n_tok * G;
+            const int n_out = pair ? 2 : 1;                       // q tiles written by this unit
+            for (int qt = 0; qt < n_out; ++qt) {
+                const int tok = qt * R + t;
+                const bool row_valid = (g < G) && (tok < wu.n_tok);
+                const int head = row_valid ? P.kv_to_q[wu.kvh * G + g] : 0;
+                float w0 = 0.f, w1 = 0.f, inv_l = 0.f, lse_val = -INFINITY;
+                bool act0 = false, act1 = false;
+                if (n > 0) {
+                    // which chains hold (partial) results for this q tile
+                    act0 = pair ? (qt == 0) : true;
+                    act1 = pair ? (qt == 1) : (n >= 2);
+                    float l0 = 0.f, m0 = -INFINITY, l1 = 0.f, m1 = -INFINITY;
+                    if (act0) {
+                        mbar_wait(bar(kBarStFull + 0), ph_st[0]);
+                        ph_st[0] ^= 1;
+                        const float2 st = stats[0 * kTileM + row];
+                        l0 = st.x;
+                        m0 = st.y;
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(bar(kBarStFree + 0));
+                    }
+                    if (act1) {
+                        mbar_wait(bar(kBarStFull + 1), ph_st[1]);
+                        ph_st[1] ^= 1;
+                        const float2 st = stats[1 * kTileM + row];
+                        l1 = st.x;
+                        m1 = st.y;
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(bar(kBarStFree + 1));
+                    }
+                    const float mm = fmaxf(m0, m1);
+                    w0 = (l0 > 0.f) ? ex2_approx((m0 - mm) * sl) : 0.f;
+                    w1 = (l1 > 0.f) ? ex2_approx((m1 - mm) * sl) : 0.f;
+                    const float lt = w0 * l0 + w1 * l1;
+                    if (lt > 0.f) {
+                        inv_l = 1.f / lt;
+                        lse_val = (mm * sl + log2f(lt)) * 0.6931471805599453f;
+                    }
+                    w0 *= inv_l;
+                    w1 *= inv_l;
+                    if (act0) {
+                        mbar_wait(bar(kBarOFull + 0), ph_o[0]);
+                        ph_o[0] ^= 1;
+                    }
+                    if (act1) {
+                        mbar_wait(bar(kBarOFull + 1), ph_o[1]);
+                        ph_o[1] ^= 1;
+                    }
+                    tc_fence_after();
+                }
+                __nv_bfloat16 *orow = reinterpret_cast<__nv_bfloat16 *>(P.o) +
+                                      (static_cast<size_t>(wu.q_row0 + tok) * P.Hq + head) * D;
+                float *prow = P.workspace + (wu.partial_off < 0 ? 0 : wu.partial_off) +
+                              static_cast<size_t>(g * wu.n_tok + tok) * D;
+#pragma unroll
+                for (int q = 0; q < D / 16; ++q) {
+                    float acc[16];
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) acc[j] = 0.f;
+                    if (act0) {
+                        uint32_t orr[16];
+                        tmem_ld16(trow + C::kColO + q * 16, orr);
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) acc[j] = (w0 > 0.f) ? __uint_as_float(orr[j]) * w0 : 0.f;
+                    }
+                    if (act1) {
+                        uint32_t orr[16];
+                        tmem_ld16(trow + C::kColO + C::kChainCols + q * 16, orr);
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) acc[j] += (w1 > 0.f) ? __uint_as_float(orr[j]) * w1 : 0.f;
+                    }
+                    if (row_valid) {
+                        if (wu.partial_off < 0) {
+                            uint4 v0, v1;
+                            v0.x = pack_bf16x2(acc[0], acc[1]);
+                            v0.y = pack_bf16x2(acc[2], acc[3]);
+                            v0.z = pack_bf16x2(acc[4], acc[5]);
+                            v0.w = pack_bf16x2(acc[6], acc[7]);
+                            v1.x = pack_bf16x2(acc[8], acc[9]);
+                            v1.y = pack_bf16x2(acc[10], acc[11]);
+                            v1.z = pack_bf16x2(acc[12], acc[13]);
+                            v1.w = pack_bf16x2(acc[14], acc[15]);
+                            *reinterpret_cast<uint4 *>(orow + q * 16) = v0;
+                            *reinterpret_cast<uint4 *>(orow + q * 16 + 8) = v1;
+                        } else {
+#pragma unroll
+                            for (int j = 0; j < 4; ++j)
+                                *reinterpret_cast<float4 *>(prow + q * 16 + j * 4) =
+                                    make_float4(acc[4 * j], acc[4 * j + 1], acc[4 * j + 2], acc[4 * j + 3]);
+                        }
+                    }
+                }
+                if (row_valid) {
+                    if (wu.partial_off < 0)
+                        P.lse[static_cast<size_t>(wu.q_row0 + tok) * P.Hq + head] = lse_val;
+                    else
+                        P.workspace[wu.partial_off + static_cast<size_t>(rows_total) * D + g * wu.n_tok + tok] = lse_val;
+                }
+                if (n > 0) {
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) {
+                        if (act0) mbar_arrive(bar(kBarOFree + 0));
+                        if (act1) mbar_arrive(bar(kBarOFree + 1));
+                    }
+                }
+            }
+        }
+    } else {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
+        if (warp == 12) {
+            // ======================================================= loader warp
+            RingPos rp{0, 1};
+            uint32_t ph_qempty = 1;
+            for (int u = u_begin; u < u_end; ++u) {
+                const WorkUnit wu = P.units[u];
+                const int n = wu.tile_end - wu.tile_begin;
+                if (n <= 0) continue;
+                const bool pair = wu.mode == kModePair;
+                const int nq = pair ? 2 : 1;
+                mbar_wait(bar(kBarQEmpty), ph_qempty);
+                ph_qempty ^= 1;
+                if (lane == 0) mbar_arrive_expect_tx(bar(kBarQFull), static_cast<uint32_t>(nq * G * R * D * 2));
+                if (lane < G) {
+                    const int hq = P.kv_to_q[wu.kvh * G + lane];
+                    for (int c = 0; c < nq; ++c)
+#pragma unroll
+                        for (int h = 0; h < C::kHalves; ++h)
+                            tma_load_2d(sQ + c * C::kTileBytes + h * C::kHalfBytes + lane * R * 128, &P.tm_q, bar(kBarQFull),
+                                        hq * D + h * 64, wu.q_row0 + c * R);
+                }
+                auto fetch = [&](int tile) -> int4 {
+                    int4 e = make_int4(0, 0, 0, 0);
+                    if (lane < kVbPerTile && tile < wu.tile_end && tile * kVbPerTile + lane < wu.vb_count)
+                        e = __ldg(reinterpret_cast<const int4 *>(P.vblocks + wu.vb_begin + tile * kVbPerTile + lane));
+                    return e;
+                };
+                auto resolve = [&](const int4 &e) -> ResolvedVb {
+                    ResolvedVb r;
+                    r.nvalid = e.z;
+                    r.paged = e.w;
+                    r.row = (e.z > 0 && e.w) ? __ldg(P.block_table + e.x) * kBlock : e.x;
+                    return r;
+                };
+                // One K or V tile into the next ring slot.  A full block is one 16-row box per
+                // 64-element half; a partly filled block loads only its valid rows through the
+                // 8/4/2/1-row boxes, so nothing outside a segment ever enters shared memory.
+                auto emit = [&](const ResolvedVb &r, const CUtensorMap *tm_pool, const CUtensorMap *tm_ctg) {
+                    mbar_wait(bar(kBarKvEmpty + rp.slot), rp.phase);
+                    const uint32_t rows = __reduce_add_sync(0xffffffffu, static_cast<uint32_t>(r.nvalid));
+                    if (lane == 0) mbar_arrive_expect_tx(bar(kBarKvFull + rp.slot), rows * D * 2);
+                    if (r.nvalid > 0) {
+                        const CUtensorMap *tm = r.paged ? tm_pool : tm_ctg;
+                        const uint32_t dst0 = sRing + rp.slot * C::kTileBytes + lane * (kBlock * 128);
+                        int off = 0;
+#pragma unroll
+                        for (int i = 0; i < 5; ++i) {
+                            const int rows_i = kBlock >> i;
+                            if (r.nvalid & rows_i) {
+#pragma unroll
+                                for (int h = 0; h < C::kHalves; ++h)
+                                    tma_load_2d(dst0 + h * C::kHalfBytes + off * 128, tm + i, bar(kBarKvFull + rp.slot),
+                                                wu.kvh * D + h * 64, r.row + off);
+                                off += rows_i;
+                            }
+                        }
+                    }
+                    rp.advance(C::kStages);
+                };
+                auto emit_k = [&](const ResolvedVb &r) { emit(r, P.tm_pool_k, P.tm_ctg_k); };
+                auto emit_v = [&](const ResolvedVb &r) { emit(r, P.tm_pool_v, P.tm_ctg_v); };
+                ResolvedVb cur = resolve(fetch(wu.tile_begin));
+                ResolvedVb nxt = resolve(fetch(wu.tile_begin + 1));
+                emit_k(cur);
+                for (int j = 0; j < n; ++j) {
+                    const int4 raw2 = fetch(wu.tile_begin + j + 2);
+                    if (pair) {
+                        emit_v(cur);
+                        if (j + 1 < n) emit_k(nxt);
+                    } else {
+                        if (j + 1 < n) emit_k(nxt);
+                        emit_v(cur);
+                    }
+                    cur = nxt;
+                    nxt = resolve(raw2);
+                }
+            }
+        } else if (warp == 13 && lane == 0) {
+            // ======================================================= MMA issuer (one thread)
+            constexpr uint32_t idesc_s = make_idesc(128, 128, false);
+            constexpr uint32_t idesc_o = make_idesc(128, D, true);
+            RingPos rp{0, 0};
+            uint32_t ph_q = 0, ph_p[2] = {0, 0}, ph_ofree[2] = {1, 1};
+            auto take = [&]() -> uint32_t {
+                const uint32_t slot = rp.slot;
+                mbar_wait(bar(kBarKvFull + slot), rp.phase);
+                rp.advance(C::kStages);
+                return slot;
+            };
+            auto qk = [&](int c, int qtile, uint32_t kslot) {
+                const uint32_t qa = sQ + qtile * C::kTileBytes, ka = sRing + kslot * C::kTileBytes;
+#pragma unroll
+                for (int k = 0; k < D / 16; ++k) {
+                    const uint32_t off = (k >> 2) * C::kHalfBytes + (k & 3) * 32;
+                    umma_ss(tmem + C::kColS + c * C::kChainCols, make_smem_desc(qa + off, 16, 1024),
+                            make_smem_desc(ka + off, 16, 1024), idesc_s, k > 0);
+                }
+                umma_commit(bar(kBarSFull + c));
+            };
+            auto pv = [&](int c, uint32_t vslot, bool first) {
+                mbar_wait(bar(kBarPFull + c), ph_p[c]);
+                ph_p[c] ^= 1;
+                if (first) {
+                    mbar_wait(bar(kBarOFree + c), ph_ofree[c]);
+                    ph_ofree[c] ^= 1;
+                }
+                tc_fence_after();
+                const uint32_t va = sRing + vslot * C::kTileBytes;
+#pragma unroll
+                for (int k = 0; k < kTileN / 16; ++k)
+                    umma_ts(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
+                            make_smem_desc(va + k * (kBlock * 128), C::kHalfBytes, 1024), idesc_o, (!first || k > 0) ? 1u : 0u);
+            };
+            for (int u = u_begin; u < u_end; ++u) {
+                const WorkUnit wu = P.units[u];
+                const int n = wu.tile_end - wu.tile_begin;
+                if (n <= 0) continue;
+                mbar_wait(bar(kBarQFull), ph_q);
+                ph_q ^= 1;
+                if (wu.mode == kModePair) {
+                    uint32_t ks = take();
+                    tc_fence_after();
+                    qk(0, 0, ks);
+                    qk(1, 1, ks);
+                    umma_commit(bar(kBarKvEmpty + ks));
+                    if (n == 1) umma_commit(bar(kBarQEmpty));
+                    for (int j = 0; j < n; ++j) {
+                        const uint32_t vs = take();
+                        pv(0, vs, j == 0);
+                        if (j == n - 1) umma_commit(bar(kBarOFull + 0));
+                        if (j + 1 < n) {
+                            ks = take();
+                            tc_fence_after();
+                            qk(0, 0, ks);
+                        }
+                        pv(1, vs, j == 0);
+                        umma_commit(bar(kBarKvEmpty + vs));
+                        if (j == n - 1) umma_commit(bar(kBarOFull + 1));
+                        if (j + 1 < n) {
+                            qk(1, 1, ks);
+                            umma_commit(bar(kBarKvEmpty + ks));
+                            if (j + 2 == n) umma_commit(bar(kBarQEmpty));
+                        }
+                    }
+                } else {
+                    uint32_t ks = take();
+                    tc_fence_after();
+                    qk(0, 0, ks);
+                    umma_commit(bar(kBarKvEmpty + ks));
+                    if (n > 1) {
+                        ks = take();
+                        tc_fence_after();
+                        qk(1, 0, ks);
+                        umma_commit(bar(kBarKvEmpty + ks));
+                    }
+                    if (n <= 2) umma_commit(bar(kBarQEmpty));
+                    for (int j = 0; j < n; ++j) {
+                        const int c = j & 1;
+                        const uint32_t vs = take();
+                        pv(c, vs, j < 2);
+                        umma_commit(bar(kBarKvEmpty + vs));
+                        if (j + 2 >= n) umma_commit(bar(kBarOFull + c));
+                        if (j + 2 < n) {
+                            ks = take();
+                            tc_fence_after();
+                            qk(c, 0, ks);
+                            umma_commit(bar(kBarKvEmpty + ks));
+                            if (j + 3 == n) umma_commit(bar(kBarQEmpty));
+                        }
+                    }
+                }
+            }
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 13) tmem_dealloc(tmem, 512);
+}
+
+}  // namespace msa

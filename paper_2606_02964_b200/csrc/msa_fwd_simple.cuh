@@ -91,10 +91,10 @@ __global__ void __launch_bounds__(128, 1) msa_fwd_simple_kernel(const __grid_con
                 VBlock vb = {0, 0, 0, 0};
                 if (tid < nvb) vb = P.vblocks[wu.vb_begin + tile * kVbPerTile + tid];
                 s_vb[tid] = vb;
-                if (tid == 0) mbar_arrive_expect_tx(bar_load, static_cast<uint32_t>(nvb * 2 * kBlock * D * 2));
-                if (tid < nvb) {
-                    const void *tk = vb.paged ? &P.tm_pool_k : &P.tm_ctg_k;
-                    const void *tv = vb.paged ? &P.tm_pool_v : &P.tm_ctg_v;
+                if (tid == 0) mbar_arrive_expect_tx(bar_load, static_cast<uint32_t>(nvb * 2 * kBlock * D * 2));   // nvb counts real blocks only
+                if (tid < nvb && vb.nvalid > 0) {
+                    const void *tk = vb.paged ? &P.tm_pool_k[0] : &P.tm_ctg_k[0];
+                    const void *tv = vb.paged ? &P.tm_pool_v[0] : &P.tm_ctg_v[0];
                     const int row = vb.paged ? P.block_table[vb.src] * kBlock : vb.src;
 #pragma unroll
                     for (int h = 0; h < C::kHalves; ++h) {

@@ -10,13 +10,16 @@ namespace msa {
 
 struct FwdParams {
     CUtensorMap tm_q;        // bf16 [total_q][Hq*D], box 64 x R
-    CUtensorMap tm_pool_k;   // bf16 [num_blocks*16][Hkv*D], box 64 x 16
-    CUtensorMap tm_pool_v;
-    CUtensorMap tm_ctg_k;    // bf16 [contig_rows][Hkv*D], box 64 x 16
-    CUtensorMap tm_ctg_v;
+    // K/V tensors: pool bf16 [num_blocks*16][Hkv*D], arena bf16 [contig_rows][Hkv*D]; boxes of
+    // 64 elements x {16, 8, 4, 2, 1} rows: a partly filled block loads only its valid rows.
+    CUtensorMap tm_pool_k[5];
+    CUtensorMap tm_ctg_k[5];
+    CUtensorMap tm_pool_v[5];
+    CUtensorMap tm_ctg_v[5];
     const VBlock *vblocks;
     const WorkUnit *units;
     const int32_t *cta_unit_begin;   // [num_ctas+1]
+    const TileInfo *tile_info;
     const int32_t *block_table;
     const int32_t *kv_to_q;          // [Hkv][G] q heads of each kv head
     void *o;                         // bf16 [total_q][Hq][D]
@@ -39,7 +42,7 @@ struct MergeParams {
 enum class FwdVariant : int { Simple = 0, Pipelined = 1 };
 
 cudaError_t launch_fwd(const FwdParams &p, int head_dim, int num_ctas, FwdVariant v, cudaStream_t stream);
-cudaError_t launch_merge(const MergeParams &p, int n_items, cudaStream_t stream);
+cudaError_t launch_merge(const MergeParams &p, int n_items, int max_rows, cudaStream_t stream);
 int fwd_tiles_per_group(FwdVariant v);   // q tiles (of 128 packed rows) one work item covers
 
 }  // namespace msa

@@ -21,10 +21,12 @@ constexpr int kTileM = 128;           // packed (head, token) rows per MMA tile
 
 struct alignas(16) VBlock {
     int32_t src;        // paged: index into block_table; contiguous: first arena row
-    int32_t abs_start;  // absolute position of slot 0
-    int32_t nvalid;     // valid slots, 1..16
+    int32_t abs_start;  // absolute position of slot 0 (INT32_MAX for padding entries)
+    int32_t nvalid;     // valid slots, 1..16 (0 for padding entries)
     int32_t paged;      // 1 = paged pool (row = block_table[src]*16), 0 = contiguous arena
 };
+// Every context's list is padded with {0, INT32_MAX, 0, 0} entries to a multiple of 8, so a
+// KV tile always has 8 readable entries.
 
 // One unit = one q-tile group of one (run, kv head) against a contiguous range of KV tiles.
 struct alignas(16) WorkUnit {
@@ -37,7 +39,20 @@ struct alignas(16) WorkUnit {
     int32_t tile_begin;    // KV tiles [tile_begin, tile_end) of 8 virtual blocks each
     int32_t tile_end;
     int32_t partial_off;   // < 0: writes final O/LSE; else float offset of this unit's partial
-    int32_t reserved[3];
+    int32_t mode;          // kModePair: two q tiles share every KV tile (prefill chunks);
+                           // kModeSplit: one q tile, even/odd KV tiles go to the two softmax
+                           // warpgroups and are merged in the epilogue (short queries)
+    int32_t tile_info_begin;  // index of the context's first TileInfo
+    int32_t reserved;
+};
+
+constexpr int kModePair = 0;
+constexpr int kModeSplit = 1;
+
+// Per context KV tile: what the softmax warps need to decide whether a tile needs masking.
+struct alignas(8) TileInfo {
+    int32_t max_abs;       // largest absolute position of a valid slot in the tile (-1 if none)
+    int32_t ragged;        // 1 if any of the 8 virtual blocks has fewer than 16 valid slots
 };
 
 // Items whose KV range was split: the merge kernel combines their partials in tile order.

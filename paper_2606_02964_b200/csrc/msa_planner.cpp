@@ -15,11 +15,13 @@ namespace {
 
 struct Ctx {
     int32_t vb_begin = 0;
-    int32_t vb_count = 0;
+    int32_t vb_count = 0;      // real (unpadded) virtual blocks
+    int32_t ti_begin = 0;      // first TileInfo of the context
 };
 
 struct Item {
-    int32_t q_row0, n_tok, q_abs0, kvh, vb_begin, vb_count, n_tiles;
+    int32_t q_row0, n_tok, q_abs0, kvh, vb_begin, vb_count, n_tiles, mode, ti_begin;
+    int32_t cost;              // schedule cost of one KV tile of this item
 };
 
 // sum_{i=0}^{T-1} clamp(c0 + i, 0, n)
@@ -109,13 +111,25 @@ int build_plan(const PlannerConfig &cfg, const msa_request *req, int32_t n_req, 
             }
             if (sg.kind == MSA_SEG_PAGED) hp.uses_paged = true; else hp.uses_contig = true;
         }
-        if (hp.vblocks.size() > static_cast<size_t>(INT32_MAX)) return MSA_ERR_OUT_OF_RANGE;
         c.vb_count = static_cast<int32_t>(hp.vblocks.size()) - c.vb_begin;
+        while ((hp.vblocks.size() - c.vb_begin) % kVbPerTile != 0) hp.vblocks.push_back(VBlock{0, INT32_MAX, 0, 0});
+        if (hp.vblocks.size() > static_cast<size_t>(INT32_MAX)) return MSA_ERR_OUT_OF_RANGE;
+        c.ti_begin = static_cast<int32_t>(hp.tile_info.size());
+        for (size_t t = c.vb_begin; t < hp.vblocks.size(); t += kVbPerTile) {
+            TileInfo ti{-1, 0};
+            for (int b = 0; b < kVbPerTile; ++b) {
+                const VBlock &vb = hp.vblocks[t + b];
+                if (vb.nvalid < kBlock) ti.ragged = 1;
+                if (vb.nvalid > 0) ti.max_abs = std::max(ti.max_abs, vb.abs_start + vb.nvalid - 1);
+            }
+            hp.tile_info.push_back(ti);
+        }
         ctxs[key] = c;
     }
 
     // ---- work items: (run, kv head, q-tile group), horizon folded in ------------------
-    const int group_tok = cfg.tiles_per_group * cfg.R;
+    // tiles_per_group == 2: groups of 2R tokens run as kModePair (two q tiles share each KV
+    // tile); a remainder of <= R tokens (and every short run) runs as kModeSplit.
     std::vector<Item> items;
     int64_t pairs = 0;
     for (int32_t r = 0; r < n_req; ++r) {
@@ -125,13 +139,23 @@ int build_plan(const PlannerConfig &cfg, const msa_request *req, int32_t n_req, 
         for (int32_t s = rq.seg_begin; s < rq.seg_begin + rq.seg_count; ++s)
             pairs += clamp_sum(static_cast<int64_t>(rq.q_abs_start) - seg[s].abs_start + 1, rq.q_len, seg[s].len);
         for (int kvh = 0; kvh < cfg.Hkv; ++kvh) {
-            for (int32_t t0 = 0; t0 < rq.q_len; t0 += group_tok) {
+            int32_t t0 = 0;
+            while (t0 < rq.q_len) {
                 Item it;
-                it.n_tok = std::min<int32_t>(group_tok, rq.q_len - t0);
+                const int32_t left = rq.q_len - t0;
+                if (cfg.tiles_per_group >= 2 && left > cfg.R) {
+                    it.mode = kModePair;
+                    it.n_tok = std::min<int32_t>(2 * cfg.R, left);
+                } else {
+                    it.mode = cfg.tiles_per_group >= 2 ? kModeSplit : kModePair;
+                    it.n_tok = std::min<int32_t>(cfg.R, left);
+                }
+                it.cost = (cfg.tiles_per_group >= 2 && it.mode == kModePair) ? 2 : 1;
                 it.q_row0 = rq.q_row_start + t0;
                 it.q_abs0 = rq.q_abs_start + t0;
                 it.kvh = kvh;
                 it.vb_begin = c.vb_begin;
+                it.ti_begin = c.ti_begin;
                 const int32_t p_max = it.q_abs0 + it.n_tok - 1;
                 // virtual blocks are in ascending abs_start: count those starting at or before p_max
                 const VBlock *b0 = hp.vblocks.data() + c.vb_begin;
@@ -140,15 +164,17 @@ int build_plan(const PlannerConfig &cfg, const msa_request *req, int32_t n_req, 
                 it.vb_count = static_cast<int32_t>(ub - b0);
                 it.n_tiles = (it.vb_count + kVbPerTile - 1) / kVbPerTile;
                 items.push_back(it);
+                t0 += it.n_tok;
             }
         }
     }
 
-    // ---- persistent schedule: equal contiguous shares of the global tile sequence ------
-    // (stream-K style: only the items a share boundary falls into are split along KV.)
+    // ---- persistent schedule: equal contiguous shares of the global (cost-weighted) tile
+    // sequence (stream-K style: only the items a share boundary falls into are split along KV).
     const int64_t n_items = static_cast<int64_t>(items.size());
     std::vector<int64_t> start(n_items + 1, 0);
-    for (int64_t i = 0; i < n_items; ++i) start[i + 1] = start[i] + std::max<int32_t>(items[i].n_tiles, 1);
+    for (int64_t i = 0; i < n_items; ++i)
+        start[i + 1] = start[i] + static_cast<int64_t>(std::max<int32_t>(items[i].n_tiles, 1)) * items[i].cost;
     const int64_t W = start[n_items];
     int n_used = 0;
     std::vector<int64_t> bound;
@@ -159,8 +185,12 @@ int build_plan(const PlannerConfig &cfg, const msa_request *req, int32_t n_req, 
         for (int c = 1; c < n_used; ++c) {
             const int64_t b = bound[c];
             const int64_t i = std::upper_bound(start.begin(), start.end(), b) - start.begin() - 1;   // item holding b
-            if (b - start[i] <= cfg.snap_tiles) bound[c] = start[i];
-            else if (start[i + 1] - b <= cfg.snap_tiles) bound[c] = start[i + 1];
+            const int64_t cost = items[i].cost;
+            const int64_t n_i = std::max<int32_t>(items[i].n_tiles, 1);
+            int64_t tcut = (b - start[i] + cost / 2) / cost;             // nearest tile boundary inside the item
+            if (tcut <= cfg.snap_tiles) tcut = 0;
+            else if (n_i - tcut <= cfg.snap_tiles) tcut = n_i;
+            bound[c] = start[i] + tcut * cost;
         }
         for (int c = 1; c <= n_used; ++c) bound[c] = std::max(bound[c], bound[c - 1]);
     }
@@ -215,11 +245,13 @@ int build_plan(const PlannerConfig &cfg, const msa_request *req, int32_t n_req, 
                 u.kvh = it.kvh;
                 u.vb_begin = it.vb_begin;
                 u.vb_count = it.vb_count;
+                u.mode = it.mode;
+                u.tile_info_begin = it.ti_begin;
                 if (it.n_tiles == 0) {
                     u.tile_begin = u.tile_end = 0;
                 } else {
-                    u.tile_begin = static_cast<int32_t>(a - start[j]);
-                    u.tile_end = static_cast<int32_t>(b - start[j]);
+                    u.tile_begin = static_cast<int32_t>((a - start[j]) / it.cost);
+                    u.tile_end = static_cast<int32_t>((b - start[j]) / it.cost);
                 }
                 if (pieces[j] > 1) {
                     const int64_t rows = static_cast<int64_t>(it.n_tok) * cfg.G;

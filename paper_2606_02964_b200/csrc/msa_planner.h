@@ -24,6 +24,7 @@ struct HostPlan {
     std::vector<WorkUnit> units;
     std::vector<int32_t> cta_unit_begin;   // [num_ctas_used + 1]
     std::vector<MergeItem> merge_items;
+    std::vector<TileInfo> tile_info;
     msa_plan_info info{};
     int64_t workspace_floats = 0;
     bool uses_paged = false, uses_contig = false;

@@ -101,7 +101,11 @@ def _check_plan(p):
         us = sorted(us, key=lambda u: int(u["tile_begin"]))
         r = next(i for i in range(p.n_req) if p.req[i, 0] <= q_row0 < p.req[i, 0] + max(1, p.req[i, 1]))
         t0 = q_row0 - int(p.req[r, 0])
-        assert t0 % Rtok == 0 and us[0]["n_tok"] == min(Rtok, int(p.req[r, 1]) - t0)
+        left = int(p.req[r, 1]) - t0
+        # groups of 2R tokens run as "pair" units; a remainder of <= R tokens as a "split" unit
+        assert t0 % (2 * Rtok) == 0
+        assert us[0]["n_tok"] == (min(2 * Rtok, left) if left > Rtok else left)
+        assert all(int(u["mode"]) == (0 if left > Rtok else 1) for u in us)
         assert us[0]["q_abs0"] == int(p.req[r, 2]) + t0
         p_max = int(us[0]["q_abs0"]) + int(us[0]["n_tok"]) - 1
         blocks = vb[int(us[0]["vb_begin"]):]
@@ -152,10 +156,18 @@ def _check_plan(p):
                     assert e["paged"] == 0 and e["src"] == p.seg_row_off[s] + 16 * b
                 i += 1
     # balance of the persistent schedule: shares differ by at most one item's snap window
-    per_cta = np.array([sum(max(1, int(u["tile_end"]) - int(u["tile_begin"])) for u in units[cta[c]:cta[c + 1]])
-                        for c in range(info["num_ctas"])])
-    if info["num_ctas"] > 1 and per_cta.sum() >= 148 * 8:
-        assert per_cta.max() - per_cta.min() <= 6, (per_cta.min(), per_cta.max())
+    per_cta = np.array([sum(max(1, int(u["tile_end"]) - int(u["tile_begin"])) * (2 if u["mode"] == 0 else 1)
+                            for u in units[cta[c]:cta[c + 1]]) for c in range(info["num_ctas"])])
+    if info["num_ctas"] > 1 and per_cta.sum() >= 148 * 16:
+        assert per_cta.max() - per_cta.min() <= 12, (per_cta.min(), per_cta.max())
+    # per-tile mask summaries agree with the (padded) virtual block list
+    ti = msa_plan_export(plan, 4)
+    assert len(vb) % 8 == 0 and len(ti) == len(vb) // 8
+    for k in range(len(ti)):
+        blk = vb[8 * k:8 * k + 8]
+        valid = blk[blk["nvalid"] > 0]
+        assert ti[k]["ragged"] == int((blk["nvalid"] < 16).any())
+        assert ti[k]["max_abs"] == (int((valid["abs_start"] + valid["nvalid"] - 1).max()) if len(valid) else -1)
     msa_plan_destroy(plan)
     msa_destroy(h)
     return info
