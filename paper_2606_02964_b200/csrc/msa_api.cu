@@ -382,6 +382,8 @@ int msa_forward(msa_handle h, msa_plan p, const void *q, int64_t total_q, const 
         if ((rc = encode_2d(h, &fp.tm_ctg_k[i], ck, cin, crow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
         if ((rc = encode_2d(h, &fp.tm_ctg_v[i], cv, cin, crow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
     }
+    if ((rc = encode_2d(h, &fp.tm_ctg_k128, ck, cin, crow, kTileN)) != MSA_OK) return rc;
+    if ((rc = encode_2d(h, &fp.tm_ctg_v128, cv, cin, crow, kTileN)) != MSA_OK) return rc;
     fp.vblocks = p->d_vblocks;
     fp.units = p->d_units;
     fp.cta_unit_begin = p->d_cta_begin;

@@ -4,16 +4,18 @@
 //   warps 0-3   softmax warpgroup of chain 0   (one thread per packed (head, token) row)
 //   warps 4-7   softmax warpgroup of chain 1
 //   warps 8-11  epilogue warpgroup (O / l -> bf16, LSE, split-KV partials; in-CTA merge)
-//   warp  12    loader: virtual blocks -> TMA boxes (paged and contiguous alike)
+//   warp  12    loader of Q and K tiles: virtual blocks -> TMA boxes (paged and contiguous alike)
 //   warp  13    MMA issuer: tcgen05.mma for S = Q K^T and O += P V, accumulators in TMEM
-//   warps 14-15 idle (they only complete the 4-warp group setmaxnreg needs)
+//   warp  14    loader of V tiles (same code path as warp 12)
+//   warp  15    idle (it only completes the 4-warp group setmaxnreg needs)
 //
 // Two independent "chains" keep the tensor core busy while the other chain's softmax runs:
 //   kModePair   chain c owns q tile c of the unit; both chains consume every KV tile
 //   kModeSplit  one q tile; chain c owns KV tiles c, c+2, ... with its own (m, l, O);
 //               the epilogue merges the two partial softmaxes (short / decode-like queries)
 // TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P (bf16) aliases
-// the first 64 columns of its S.  Shared memory: Q 2 tiles, one ring of 5 K/V tile slots.
+// the first 64 columns of its S.  Shared memory: Q 2 tiles, one ring of 5 tile slots in which
+// K and V tiles alternate (entry 2i = K of the CTA's i-th KV tile, 2i+1 = its V).
 //
 // Invalid KV slots (block tails, blocks past a context's end) never reach O: their scores
 // are replaced by -inf, and their K/V rows are never written by TMA -- partly filled blocks
@@ -57,10 +59,11 @@ enum PipeBar : int {
 
 struct RingPos {
     uint32_t slot, phase;
-    __device__ __forceinline__ void advance(int stages)
+    __device__ __forceinline__ void advance2(int stages)   // K and V entries alternate in the ring
     {
-        if (++slot == static_cast<uint32_t>(stages)) {
-            slot = 0;
+        slot += 2;
+        if (slot >= static_cast<uint32_t>(stages)) {
+            slot -= stages;
             phase ^= 1;
         }
     }
@@ -68,8 +71,7 @@ struct RingPos {
 
 struct ResolvedVb {
     int32_t row;      // first row in the pool / arena row space
-    int32_t nvalid;   // 0: nothing to load
-    int32_t paged;
+    int32_t nvp;      // valid slots (0: nothing to load) | paged << 8
 };
 
 template <int D>
@@ -345,27 +347,38 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
         }
     } else {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
-        if (warp == 12) {
-            // ======================================================= loader warp
-            RingPos rp{0, 1};
+        if (warp == 12 || warp == 14) {
+            // ======================================================= loader warps (12: Q and K, 14: V)
+            // Ring sequence: K of the CTA's i-th KV tile is entry 2i, its V entry 2i+1.
+            const int which = warp == 12 ? 0 : 1;
+            const CUtensorMap *tm_pool = which ? P.tm_pool_v : P.tm_pool_k;
+            const CUtensorMap *tm_ctg = which ? P.tm_ctg_v : P.tm_ctg_k;
+            const CUtensorMap *tm_ctg128 = which ? &P.tm_ctg_v128 : &P.tm_ctg_k128;
+            RingPos rp{static_cast<uint32_t>(which), 1};
             uint32_t ph_qempty = 1;
             for (int u = u_begin; u < u_end; ++u) {
                 const WorkUnit wu = P.units[u];
                 const int n = wu.tile_end - wu.tile_begin;
                 if (n <= 0) continue;
-                const bool pair = wu.mode == kModePair;
-                const int nq = pair ? 2 : 1;
-                mbar_wait(bar(kBarQEmpty), ph_qempty);
-                ph_qempty ^= 1;
-                if (lane == 0) mbar_arrive_expect_tx(bar(kBarQFull), static_cast<uint32_t>(nq * G * R * D * 2));
-                if (lane < G) {
-                    const int hq = P.kv_to_q[wu.kvh * G + lane];
-                    for (int c = 0; c < nq; ++c)
+                if (which == 0) {
+                    const int nq = wu.mode == kModePair ? 2 : 1;
+                    mbar_wait(bar(kBarQEmpty), ph_qempty);
+                    ph_qempty ^= 1;
+                    if (elect_one()) {
+                        mbar_arrive_expect_tx(bar(kBarQFull), static_cast<uint32_t>(nq * G * R * D * 2));
+                        for (int g = 0; g < G; ++g) {
+                            const int hq = __ldg(P.kv_to_q + wu.kvh * G + g);
+                            for (int c = 0; c < nq; ++c)
 #pragma unroll
-                        for (int h = 0; h < C::kHalves; ++h)
-                            tma_load_2d(sQ + c * C::kTileBytes + h * C::kHalfBytes + lane * R * 128, &P.tm_q, bar(kBarQFull),
-                                        hq * D + h * 64, wu.q_row0 + c * R);
+                                for (int h = 0; h < C::kHalves; ++h)
+                                    tma_load_2d(sQ + c * C::kTileBytes + h * C::kHalfBytes + g * R * 128, &P.tm_q,
+                                                bar(kBarQFull), hq * D + h * 64, wu.q_row0 + c * R);
+                        }
+                    }
+                    __syncwarp();
                 }
+                const int c0 = wu.kvh * D;
+                // lane b < 8 owns virtual block b of a tile: fetch its entry, then resolve its row
                 auto fetch = [&](int tile) -> int4 {
                     int4 e = make_int4(0, 0, 0, 0);
                     if (lane < kVbPerTile && tile < wu.tile_end && tile * kVbPerTile + lane < wu.vb_count)
@@ -374,64 +387,94 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                 };
                 auto resolve = [&](const int4 &e) -> ResolvedVb {
                     ResolvedVb r;
-                    r.nvalid = e.z;
-                    r.paged = e.w;
+                    r.nvp = e.z | (e.w << 8);
                     r.row = (e.z > 0 && e.w) ? __ldg(P.block_table + e.x) * kBlock : e.x;
                     return r;
                 };
-                // One K or V tile into the next ring slot.  A full block is one 16-row box per
-                // 64-element half; a partly filled block loads only its valid rows through the
-                // 8/4/2/1-row boxes, so nothing outside a segment ever enters shared memory.
-                auto emit = [&](const ResolvedVb &r, const CUtensorMap *tm_pool, const CUtensorMap *tm_ctg) {
+                ResolvedVb cur = resolve(fetch(wu.tile_begin));
+                ResolvedVb nxt = resolve(fetch(wu.tile_begin + 1));
+                int4 raw = fetch(wu.tile_begin + 2);
+#pragma unroll 1
+                for (int j = 0; j < n; ++j) {
+                    // One K (or V) tile into its ring slot, issued by one elected lane.  A full
+                    // block is one 16-row box per 64-element half; eight full, consecutive arena
+                    // blocks are one 128-row box; a partly filled block loads only its valid rows
+                    // through the 8/4/2/1-row boxes: nothing outside a segment enters shared memory.
+                    const int nv = cur.nvp & 0xff;
+                    const uint32_t m_any = __ballot_sync(0xffffffffu, nv > 0) & 0xffu;
+                    const uint32_t m_full = __ballot_sync(0xffffffffu, nv == kBlock) & 0xffu;
+                    const uint32_t m_paged = __ballot_sync(0xffffffffu, (cur.nvp >> 8) != 0) & 0xffu;
+                    int rows_b[kVbPerTile];
+#pragma unroll
+                    for (int b = 0; b < kVbPerTile; ++b) rows_b[b] = __shfl_sync(0xffffffffu, cur.row, b);
+                    const bool run = m_full == 0xffu && m_paged == 0 &&
+                                     __all_sync(0xffffffffu, lane >= kVbPerTile || cur.row == rows_b[0] + lane * kBlock);
                     mbar_wait(bar(kBarKvEmpty + rp.slot), rp.phase);
-                    const uint32_t rows = __reduce_add_sync(0xffffffffu, static_cast<uint32_t>(r.nvalid));
-                    if (lane == 0) mbar_arrive_expect_tx(bar(kBarKvFull + rp.slot), rows * D * 2);
-                    if (r.nvalid > 0) {
-                        const CUtensorMap *tm = r.paged ? tm_pool : tm_ctg;
-                        const uint32_t dst0 = sRing + rp.slot * C::kTileBytes + lane * (kBlock * 128);
-                        int off = 0;
+                    const uint32_t full = bar(kBarKvFull + rp.slot);
+                    const uint32_t dst = sRing + rp.slot * C::kTileBytes;
+                    if (run) {
+                        if (elect_one()) {
+                            mbar_arrive_expect_tx(full, static_cast<uint32_t>(kTileN * D * 2));
 #pragma unroll
-                        for (int i = 0; i < 5; ++i) {
-                            const int rows_i = kBlock >> i;
-                            if (r.nvalid & rows_i) {
+                            for (int h = 0; h < C::kHalves; ++h)
+                                tma_load_2d(dst + h * C::kHalfBytes, tm_ctg128, full, c0 + h * 64, rows_b[0]);
+                        }
+                    } else if (m_any == m_full) {
+                        if (elect_one()) {
+                            mbar_arrive_expect_tx(full, static_cast<uint32_t>(__popc(m_any) * kBlock * D * 2));
 #pragma unroll
-                                for (int h = 0; h < C::kHalves; ++h)
-                                    tma_load_2d(dst0 + h * C::kHalfBytes + off * 128, tm + i, bar(kBarKvFull + rp.slot),
-                                                wu.kvh * D + h * 64, r.row + off);
-                                off += rows_i;
+                            for (int b = 0; b < kVbPerTile; ++b) {
+                                if (m_any >> b & 1) {
+                                    const CUtensorMap *tm = (m_paged >> b & 1) ? tm_pool : tm_ctg;
+#pragma unroll
+                                    for (int h = 0; h < C::kHalves; ++h)
+                                        tma_load_2d(dst + b * (kBlock * 128) + h * C::kHalfBytes, tm, full, c0 + h * 64, rows_b[b]);
+                                }
+                            }
+                        }
+                    } else {
+                        const uint32_t rows = __reduce_add_sync(0xffffffffu, static_cast<uint32_t>(nv));
+                        if (elect_one()) mbar_arrive_expect_tx(full, rows * D * 2);
+                        __syncwarp();
+                        if (nv > 0) {     // rare path: each lane issues the boxes of its own block
+                            const CUtensorMap *tm = (cur.nvp >> 8) ? tm_pool : tm_ctg;
+                            int off = 0;
+#pragma unroll 1
+                            for (int i = 0; i < 5; ++i) {
+                                const int rows_i = kBlock >> i;
+                                if (nv & rows_i) {
+#pragma unroll 1
+                                    for (int h = 0; h < C::kHalves; ++h)
+                                        tma_load_2d(dst + lane * (kBlock * 128) + h * C::kHalfBytes + off * 128, tm + i, full,
+                                                    c0 + h * 64, cur.row + off);
+                                    off += rows_i;
+                                }
                             }
                         }
                     }
-                    rp.advance(C::kStages);
-                };
-                auto emit_k = [&](const ResolvedVb &r) { emit(r, P.tm_pool_k, P.tm_ctg_k); };
-                auto emit_v = [&](const ResolvedVb &r) { emit(r, P.tm_pool_v, P.tm_ctg_v); };
-                ResolvedVb cur = resolve(fetch(wu.tile_begin));
-                ResolvedVb nxt = resolve(fetch(wu.tile_begin + 1));
-                emit_k(cur);
-                for (int j = 0; j < n; ++j) {
-                    const int4 raw2 = fetch(wu.tile_begin + j + 2);
-                    if (pair) {
-                        emit_v(cur);
-                        if (j + 1 < n) emit_k(nxt);
-                    } else {
-                        if (j + 1 < n) emit_k(nxt);
-                        emit_v(cur);
-                    }
+                    __syncwarp();
+                    rp.advance2(C::kStages);
                     cur = nxt;
-                    nxt = resolve(raw2);
+                    nxt = resolve(raw);
+                    raw = fetch(wu.tile_begin + j + 3);
                 }
             }
-        } else if (warp == 13 && lane == 0) {
+        } else if (warp == 13 && elect_one()) {
             // ======================================================= MMA issuer (one thread)
             constexpr uint32_t idesc_s = make_idesc(128, 128, false);
             constexpr uint32_t idesc_o = make_idesc(128, D, true);
-            RingPos rp{0, 0};
+            RingPos rk{0, 0}, rv{1, 0};
             uint32_t ph_q = 0, ph_p[2] = {0, 0}, ph_ofree[2] = {1, 1};
-            auto take = [&]() -> uint32_t {
-                const uint32_t slot = rp.slot;
-                mbar_wait(bar(kBarKvFull + slot), rp.phase);
-                rp.advance(C::kStages);
+            auto take_k = [&]() -> uint32_t {
+                const uint32_t slot = rk.slot;
+                mbar_wait(bar(kBarKvFull + slot), rk.phase);
+                rk.advance2(C::kStages);
+                return slot;
+            };
+            auto take_v = [&]() -> uint32_t {
+                const uint32_t slot = rv.slot;
+                mbar_wait(bar(kBarKvFull + slot), rv.phase);
+                rv.advance2(C::kStages);
                 return slot;
             };
             auto qk = [&](int c, int qtile, uint32_t kslot) {
@@ -465,18 +508,18 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                 mbar_wait(bar(kBarQFull), ph_q);
                 ph_q ^= 1;
                 if (wu.mode == kModePair) {
-                    uint32_t ks = take();
+                    uint32_t ks = take_k();
                     tc_fence_after();
                     qk(0, 0, ks);
                     qk(1, 1, ks);
                     umma_commit(bar(kBarKvEmpty + ks));
                     if (n == 1) umma_commit(bar(kBarQEmpty));
                     for (int j = 0; j < n; ++j) {
-                        const uint32_t vs = take();
+                        const uint32_t vs = take_v();
                         pv(0, vs, j == 0);
                         if (j == n - 1) umma_commit(bar(kBarOFull + 0));
                         if (j + 1 < n) {
-                            ks = take();
+                            ks = take_k();
                             tc_fence_after();
                             qk(0, 0, ks);
                         }
@@ -490,12 +533,12 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                         }
                     }
                 } else {
-                    uint32_t ks = take();
+                    uint32_t ks = take_k();
                     tc_fence_after();
                     qk(0, 0, ks);
                     umma_commit(bar(kBarKvEmpty + ks));
                     if (n > 1) {
-                        ks = take();
+                        ks = take_k();
                         tc_fence_after();
                         qk(1, 0, ks);
                         umma_commit(bar(kBarKvEmpty + ks));
@@ -503,12 +546,12 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     if (n <= 2) umma_commit(bar(kBarQEmpty));
                     for (int j = 0; j < n; ++j) {
                         const int c = j & 1;
-                        const uint32_t vs = take();
+                        const uint32_t vs = take_v();
                         pv(c, vs, j < 2);
                         umma_commit(bar(kBarKvEmpty + vs));
                         if (j + 2 >= n) umma_commit(bar(kBarOFull + c));
                         if (j + 2 < n) {
-                            ks = take();
+                            ks = take_k();
                             tc_fence_after();
                             qk(c, 0, ks);
                             umma_commit(bar(kBarKvEmpty + ks));

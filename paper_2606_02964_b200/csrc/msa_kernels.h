@@ -16,6 +16,7 @@ struct FwdParams {
     CUtensorMap tm_ctg_k[5];
     CUtensorMap tm_pool_v[5];
     CUtensorMap tm_ctg_v[5];
+    CUtensorMap tm_ctg_k128, tm_ctg_v128;   // arena, box 64 x 128: eight full consecutive blocks at once
     const VBlock *vblocks;
     const WorkUnit *units;
     const int32_t *cta_unit_begin;   // [num_ctas+1]
