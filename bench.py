@@ -47,12 +47,17 @@ def measured_peaks():
 
 
 def committed_traffic(workload: str):
-    """dram bytes per launch of the dominant kernel from the committed ncu capture, or None."""
+    """dram bytes per launch of the dominant kernel from the committed ncu capture
+    (profiles/roofline_traffic.csv, copied by hand from the `ncu --set full` summaries), or None."""
+    import csv
     try:
-        with open(os.path.join(ROOT, "profiles", "roofline_traffic.json")) as f:
-            return json.load(f).get(workload)
+        with open(os.path.join(ROOT, "profiles", "roofline_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload:
+                    return float(row["dram_bytes_per_launch"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
