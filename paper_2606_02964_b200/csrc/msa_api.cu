@@ -66,6 +66,7 @@ struct msa_handle_s {
     int num_sms = 0;
     bool planning_only = false;
     FwdVariant variant = FwdVariant::Simple;
+    int emu = kDefaultEmu;             // debug env MSA_EMU overrides (tuning sweeps)
     std::vector<int32_t> kv_to_q;      // [Hkv][G]
     int32_t *d_kv_to_q = nullptr;
     EncodeTiledFn encode = nullptr;
@@ -142,6 +143,7 @@ int msa_create(const msa_config *cfg, msa_handle *out)
     }
     const char *kv = getenv("MSA_KERNEL");
     h->variant = (kv && strcmp(kv, "simple") == 0) ? FwdVariant::Simple : FwdVariant::Pipelined;
+    if (const char *em = getenv("MSA_EMU")) h->emu = atoi(em);
 
     if (cfg->device < 0) {
         // planning-only handle: descriptor validation and scheduling on the host; every
@@ -402,7 +404,7 @@ int msa_forward(msa_handle h, msa_plan p, const void *q, int64_t total_q, const 
     const bool rec = h->timing && static_cast<size_t>(h->ev_steps) * 3 + 3 <= h->ev.size();
     cudaEvent_t *ev = rec ? &h->ev[static_cast<size_t>(h->ev_steps) * 3] : nullptr;
     if (rec) MSA_CUDA(cudaEventRecord(ev[0], stream));
-    MSA_CUDA(launch_fwd(fp, D, hp.info.num_ctas, h->variant, stream));
+    MSA_CUDA(launch_fwd(fp, D, hp.info.num_ctas, h->variant, h->emu, stream));
     if (rec) MSA_CUDA(cudaEventRecord(ev[1], stream));
     h->last_launches = 1;
     if (!hp.merge_items.empty()) {

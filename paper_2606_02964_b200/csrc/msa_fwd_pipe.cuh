@@ -26,8 +26,41 @@
 
 #include "msa_kernels.h"
 #include "msa_ptx.cuh"
+#include "msa_softmax.cuh"
 
 namespace msa {
+
+// Optional role-level cycle counters (build with -DMSA_PROF; never in the shipped library):
+// lane 0 of one warp per role accumulates clock64() deltas into g_prof[cta][slot].
+#ifdef MSA_PROF
+__device__ unsigned long long g_prof[160][32];
+__device__ long long g_trace[3][64][8];
+#define PROF_TRACE(role, step, ev) \
+    do { if (blockIdx.x == 0 && u == u_begin && (step) < 64) g_trace[role][step][ev] = clock64(); } while (0)
+#if MSA_PROF == 2   /* event trace only: no accumulators in the hot loops */
+#define PROF_DECL()
+#define PROF_T0()
+#define PROF_ADD(slot)
+#define PROF_INC(slot, v)
+#define PROF_FLUSH(lo, hi)
+#else
+#define PROF_DECL() unsigned long long prof_acc[32] = {}
+#define PROF_T0() const long long prof_t0_ = clock64()
+#define PROF_ADD(slot) prof_acc[slot] += static_cast<unsigned long long>(clock64() - prof_t0_)
+#define PROF_INC(slot, v) prof_acc[slot] += static_cast<unsigned long long>(v)
+#define PROF_FLUSH(lo, hi)                                                             \
+    do {                                                                               \
+        _Pragma("unroll") for (int i_ = (lo); i_ < (hi); ++i_) g_prof[blockIdx.x][i_] += prof_acc[i_]; \
+    } while (0)
+#endif
+#else
+#define PROF_TRACE(role, step, ev)
+#define PROF_DECL()
+#define PROF_T0()
+#define PROF_ADD(slot)
+#define PROF_INC(slot, v)
+#define PROF_FLUSH(lo, hi)
+#endif
 
 template <int D>
 struct PipeCfg {
@@ -49,12 +82,13 @@ enum PipeBar : int {
     kBarKvFull = 2,      // [5]
     kBarKvEmpty = 7,     // [5]
     kBarSFull = 12,      // [2]
-    kBarPFull = 14,      // [2]
+    kBarPLo = 14,        // [2] P of keys 0-63 in TMEM
     kBarOFull = 16,      // [2]
     kBarOFree = 18,      // [2]
     kBarStFull = 20,     // [2]
     kBarStFree = 22,     // [2]
-    kBarCount = 24
+    kBarPHi = 24,        // [2] P of keys 64-127 in TMEM
+    kBarCount = 26
 };
 
 struct RingPos {
@@ -74,7 +108,10 @@ struct ResolvedVb {
     int32_t nvp;      // valid slots (0: nothing to load) | paged << 8
 };
 
-template <int D>
+// EMU: of every 8 element pairs of a softmax row, how many take 2^x from ex2_poly2 (FMA/ALU
+// pipes) instead of MUFU.EX2; -1 disables the stale-max fast path altogether (two-phase
+// max-then-exp on every tile, all MUFU).
+template <int D, int EMU>
 __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_constant__ FwdParams P)
 {
     using C = PipeCfg<D>;
@@ -104,7 +141,8 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
         }
         for (int c = 0; c < 2; ++c) {
             mbar_init(bar(kBarSFull + c), 1);
-            mbar_init(bar(kBarPFull + c), 4);
+            mbar_init(bar(kBarPLo + c), 4);
+            mbar_init(bar(kBarPHi + c), 4);
             mbar_init(bar(kBarOFull + c), 1);
             mbar_init(bar(kBarOFree + c), 4);
             mbar_init(bar(kBarStFull + c), 4);
@@ -134,6 +172,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
         const uint32_t tS = trow + C::kColS + c * C::kChainCols;
         const uint32_t tO = trow + C::kColO + c * C::kChainCols;
         uint32_t ph_s = 0, ph_stfree = 1;
+        PROF_DECL();
         for (int u = u_begin; u < u_end; ++u) {
             const WorkUnit wu = P.units[u];
             const int n = wu.tile_end - wu.tile_begin;
@@ -143,86 +182,140 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             if (steps <= 0) continue;
             const int p_row = wu.q_abs0 + (pair ? c * R : 0) + t;
             const int p_min = wu.q_abs0 + (pair ? c * R : 0);
-            float m = -INFINITY, l = 0.f;
+            // Row state: integer reference `ref` (log2 units), l = sum of 2^(s*sl - ref) so far,
+            // m_run = running max of the raw scores.  See msa_softmax.cuh.
+            float ref = 0.f, l = 0.f, m_run = -INFINITY;
+            // Moves the reference up to ceil(m_run*sl) once it lags by more than the lazy
+            // threshold: l and O (in TMEM) are multiplied by an exact power of two.  O may be
+            // touched here because S of this tile is complete, hence so is PV of the last one.
+            auto move_reference = [&](bool have_o) {
+                const float tgt = (m_run == -INFINITY) ? ref : ceilf(m_run * sl);
+                const bool grow = tgt - ref > C::kRescaleThreshold;
+                if (__any_sync(0xffffffffu, grow)) {
+                    const float alpha = grow ? exp2_int(ref - tgt) : 1.f;
+                    l *= alpha;
+                    if (grow) ref = tgt;
+                    if (have_o) {
+#pragma unroll
+                        for (int q = 0; q < D / 16; ++q) {
+                            uint32_t orr[16];
+                            tmem_ld16(tO + q * 16, orr);
+                            tmem_wait_ld();
+#pragma unroll
+                            for (int j = 0; j < 16; ++j) orr[j] = __float_as_uint(__uint_as_float(orr[j]) * alpha);
+                            tmem_st16(tO + q * 16, orr);
+                        }
+                    }
+                }
+            };
+            // tile summaries are fetched one tile ahead: the L2 round trip stays off the
+            // P -> PV -> QK -> S critical loop of the chain
+            const int2 *tip = reinterpret_cast<const int2 *>(P.tile_info + wu.tile_info_begin + wu.tile_begin + (pair ? 0 : c));
+            const int ti_stride = pair ? 1 : 2;
+            int2 ti_raw = __ldg(tip);
             for (int s = 0; s < steps; ++s) {
                 const int tile = wu.tile_begin + (pair ? s : 2 * s + c);
-                const TileInfo ti = P.tile_info[wu.tile_info_begin + tile];
+                TileInfo ti;
+                ti.max_abs = ti_raw.x;
+                ti.ragged = ti_raw.y;
+                if (s + 1 < steps) ti_raw = __ldg(tip + (s + 1) * ti_stride);
                 const bool need_mask = ti.ragged != 0 || ti.max_abs > p_min;
-                mbar_wait(bar(kBarSFull + c), ph_s);
+                {
+                    PROF_T0();
+                    mbar_wait(bar(kBarSFull + c), ph_s);
+                    PROF_ADD(0);
+                }
+                if ((threadIdx.x & 127) == 0) PROF_TRACE(1 + c, s, 0);
                 ph_s ^= 1;
                 tc_fence_after();
-                uint32_t sr[128];
+                PROF_T0();
+                bool done = false;
+                if (EMU >= 0 && !need_mask && s > 0) {
+                    // fast path: stale reference, tile max found alongside, P handed over in halves
+                    move_reference(true);
+                    float tile_sum, tile_max;
+                    done = softmax_fast_tile<(EMU < 0 ? 0 : EMU)>(tS, sl, ref, tile_sum, tile_max, [&]() {
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(bar(kBarPLo + c));
+                        if ((threadIdx.x & 127) == 0) PROF_TRACE(1 + c, s, 4);
+                    }, [&](int ev) {
+                        if ((threadIdx.x & 127) == 0) PROF_TRACE(1 + c, s, ev);
+                    });
+                    if (done) {
+                        l += tile_sum;
+                        m_run = fmaxf(m_run, tile_max);
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(bar(kBarPHi + c));
+                    }
+                    PROF_ADD(20);
+                }
+                if (!done) {
+                    // exact path (first tile of a unit, masked / ragged tiles, guard failures):
+                    // all of S, mask, row max, reference moved BEFORE p is formed
+                    uint32_t sr[128];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) tmem_ld32(tS + q * 32, *reinterpret_cast<uint32_t(*)[32]>(&sr[q * 32]));
-                tmem_wait_ld();
-                if (need_mask) {
-                    const VBlock *vbp = P.vblocks + wu.vb_begin + tile * kVbPerTile;
+                    for (int q = 0; q < 4; ++q) tmem_ld32(tS + q * 32, *reinterpret_cast<uint32_t(*)[32]>(&sr[q * 32]));
+                    tmem_wait_ld();
+                    if (need_mask) {
+                        const VBlock *vbp = P.vblocks + wu.vb_begin + tile * kVbPerTile;
 #pragma unroll
-                    for (int b = 0; b < kVbPerTile; ++b) {
-                        const int4 e = __ldg(reinterpret_cast<const int4 *>(vbp + b));   // {src, abs_start, nvalid, paged}
-                        int lim = min(e.z, p_row - e.y + 1);
-                        if (tile * kVbPerTile + b >= wu.vb_count) lim = 0;               // past the causal horizon: not loaded
+                        for (int b = 0; b < kVbPerTile; ++b) {
+                            const int4 e = __ldg(reinterpret_cast<const int4 *>(vbp + b));   // {src, abs_start, nvalid, paged}
+                            int lim = min(e.z, p_row - e.y + 1);
+                            if (tile * kVbPerTile + b >= wu.vb_count) lim = 0;               // past the causal horizon: not loaded
 #pragma unroll
-                        for (int j = 0; j < kBlock; ++j)
-                            if (j >= lim) sr[b * kBlock + j] = 0xff800000u;             // -inf
+                            for (int j = 0; j < kBlock; ++j)
+                                if (j >= lim) sr[b * kBlock + j] = 0xff800000u;             // -inf
+                        }
+                    }
+                    float mx0 = -INFINITY, mx1 = -INFINITY;
+#pragma unroll
+                    for (int j = 0; j < 128; j += 4) {
+                        mx0 = fmaxf(mx0, fmaxf(__uint_as_float(sr[j]), __uint_as_float(sr[j + 1])));
+                        mx1 = fmaxf(mx1, fmaxf(__uint_as_float(sr[j + 2]), __uint_as_float(sr[j + 3])));
+                    }
+                    m_run = fmaxf(m_run, fmaxf(mx0, mx1));
+                    move_reference(s > 0);
+                    float sum0 = 0.f, sum1 = 0.f;
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        uint32_t pk[16];
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) {
+                            const float p0 = ex2_approx(fmaf(__uint_as_float(sr[q * 32 + 2 * j]), sl, -ref));
+                            const float p1 = ex2_approx(fmaf(__uint_as_float(sr[q * 32 + 2 * j + 1]), sl, -ref));
+                            sum0 += p0;
+                            sum1 += p1;
+                            pk[j] = pack_bf16x2(p0, p1);
+                        }
+                        tmem_st16(tS + q * 16, pk);
+                    }
+                    l += sum0 + sum1;
+                    tmem_wait_st();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) {
+                        mbar_arrive(bar(kBarPLo + c));
+                        mbar_arrive(bar(kBarPHi + c));
                     }
                 }
-                float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
-#pragma unroll
-                for (int j = 0; j < 128; j += 4) {
-                    mx0 = fmaxf(mx0, __uint_as_float(sr[j]));
-                    mx1 = fmaxf(mx1, __uint_as_float(sr[j + 1]));
-                    mx2 = fmaxf(mx2, __uint_as_float(sr[j + 2]));
-                    mx3 = fmaxf(mx3, __uint_as_float(sr[j + 3]));
-                }
-                const float m_new = fmaxf(m, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)));
-                // lazy rescale: keep a stale max while the new one is within 2^8 of it
-                const bool grow = (m_new - m) * sl > C::kRescaleThreshold;
-                float alpha = 1.f;
-                if (grow) {
-                    alpha = ex2_approx((m - m_new) * sl);      // m = -inf -> 0
-                    l *= alpha;
-                    m = m_new;
-                }
-                if (s > 0 && __any_sync(0xffffffffu, grow)) {
-#pragma unroll
-                    for (int q = 0; q < D / 16; ++q) {
-                        uint32_t orr[16];
-                        tmem_ld16(tO + q * 16, orr);
-                        tmem_wait_ld();
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) orr[j] = __float_as_uint(__uint_as_float(orr[j]) * alpha);
-                        tmem_st16(tO + q * 16, orr);
-                    }
-                }
-                const float neg_ms = (m == -INFINITY) ? 0.f : -m * sl;
-                float sum0 = 0.f, sum1 = 0.f;
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    uint32_t pk[16];
-#pragma unroll
-                    for (int j = 0; j < 16; ++j) {
-                        const float p0 = ex2_approx(fmaf(__uint_as_float(sr[q * 32 + 2 * j]), sl, neg_ms));
-                        const float p1 = ex2_approx(fmaf(__uint_as_float(sr[q * 32 + 2 * j + 1]), sl, neg_ms));
-                        sum0 += p0;
-                        sum1 += p1;
-                        pk[j] = pack_bf16x2(p0, p1);
-                    }
-                    tmem_st16(tS + q * 16, pk);
-                }
-                l += sum0 + sum1;
-                tmem_wait_st();
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar(kBarPFull + c));
+                PROF_ADD(2);
+                if ((threadIdx.x & 127) == 0) PROF_TRACE(1 + c, s, 6);
+                PROF_INC(4, 1);
+                PROF_INC(6, done ? 1 : 0);
             }
-            // hand (l, m) of my row to the epilogue
+            // hand (l, ref) of my row to the epilogue
             mbar_wait(bar(kBarStFree + c), ph_stfree);
             ph_stfree ^= 1;
-            stats[c * kTileM + row] = make_float2(l, m);
+            stats[c * kTileM + row] = make_float2(l, ref);
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(kBarStFull + c));
         }
+#if defined(MSA_PROF) && MSA_PROF != 2
+        if ((threadIdx.x & 127) == 0) {
+            for (int i : {0, 2, 4, 6, 18, 20}) g_prof[blockIdx.x][i + c] += prof_acc[i];
+        }
+#endif
     } else if (warp < 12) {
         // =========================================================== epilogue warpgroup
         asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
@@ -265,13 +358,14 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                         __syncwarp();
                         if (lane == 0) mbar_arrive(bar(kBarStFree + 1));
                     }
-                    const float mm = fmaxf(m0, m1);
-                    w0 = (l0 > 0.f) ? ex2_approx((m0 - mm) * sl) : 0.f;
-                    w1 = (l1 > 0.f) ? ex2_approx((m1 - mm) * sl) : 0.f;
+                    // (l, ref) of each active chain; an inactive or empty chain weighs 0
+                    const float mm = fmaxf((act0 && l0 > 0.f) ? m0 : -INFINITY, (act1 && l1 > 0.f) ? m1 : -INFINITY);
+                    w0 = (act0 && l0 > 0.f) ? exp2_int(m0 - mm) : 0.f;
+                    w1 = (act1 && l1 > 0.f) ? exp2_int(m1 - mm) : 0.f;
                     const float lt = w0 * l0 + w1 * l1;
                     if (lt > 0.f) {
                         inv_l = 1.f / lt;
-                        lse_val = (mm * sl + log2f(lt)) * 0.6931471805599453f;
+                        lse_val = (mm + log2f(lt)) * 0.6931471805599453f;
                     }
                     w0 *= inv_l;
                     w1 *= inv_l;
@@ -356,6 +450,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             const CUtensorMap *tm_ctg128 = which ? &P.tm_ctg_v128 : &P.tm_ctg_k128;
             RingPos rp{static_cast<uint32_t>(which), 1};
             uint32_t ph_qempty = 1;
+            PROF_DECL();
             for (int u = u_begin; u < u_end; ++u) {
                 const WorkUnit wu = P.units[u];
                 const int n = wu.tile_end - wu.tile_begin;
@@ -409,7 +504,11 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     for (int b = 0; b < kVbPerTile; ++b) rows_b[b] = __shfl_sync(0xffffffffu, cur.row, b);
                     const bool run = m_full == 0xffu && m_paged == 0 &&
                                      __all_sync(0xffffffffu, lane >= kVbPerTile || cur.row == rows_b[0] + lane * kBlock);
-                    mbar_wait(bar(kBarKvEmpty + rp.slot), rp.phase);
+                    {
+                        PROF_T0();
+                        mbar_wait(bar(kBarKvEmpty + rp.slot), rp.phase);
+                        PROF_ADD(16);
+                    }
                     const uint32_t full = bar(kBarKvFull + rp.slot);
                     const uint32_t dst = sRing + rp.slot * C::kTileBytes;
                     if (run) {
@@ -459,21 +558,32 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     raw = fetch(wu.tile_begin + j + 3);
                 }
             }
+#if defined(MSA_PROF) && MSA_PROF != 2
+            if (lane == 0) g_prof[blockIdx.x][16 + which] += prof_acc[16];
+#endif
         } else if (warp == 13 && elect_one()) {
             // ======================================================= MMA issuer (one thread)
             constexpr uint32_t idesc_s = make_idesc(128, 128, false);
             constexpr uint32_t idesc_o = make_idesc(128, D, true);
             RingPos rk{0, 0}, rv{1, 0};
             uint32_t ph_q = 0, ph_p[2] = {0, 0}, ph_ofree[2] = {1, 1};
+            PROF_DECL();
+#if defined(MSA_PROF) && MSA_PROF != 2
+            const long long prof_mma_start = clock64();
+#endif
             auto take_k = [&]() -> uint32_t {
                 const uint32_t slot = rk.slot;
+                PROF_T0();
                 mbar_wait(bar(kBarKvFull + slot), rk.phase);
+                PROF_ADD(8);
                 rk.advance2(C::kStages);
                 return slot;
             };
             auto take_v = [&]() -> uint32_t {
                 const uint32_t slot = rv.slot;
+                PROF_T0();
                 mbar_wait(bar(kBarKvFull + slot), rv.phase);
+                PROF_ADD(9);
                 rv.advance2(C::kStages);
                 return slot;
             };
@@ -487,25 +597,43 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                 }
                 umma_commit(bar(kBarSFull + c));
             };
+            // O += P V in two halves: keys 0-63 as soon as the softmax warps have published the
+            // first half of P, keys 64-127 after the second.
             auto pv = [&](int c, uint32_t vslot, bool first) {
-                mbar_wait(bar(kBarPFull + c), ph_p[c]);
-                ph_p[c] ^= 1;
+                {
+                    PROF_T0();
+                    mbar_wait(bar(kBarPLo + c), ph_p[c]);
+                    if (c == 0) PROF_ADD(10); else PROF_ADD(11);
+                }
                 if (first) {
+                    PROF_T0();
                     mbar_wait(bar(kBarOFree + c), ph_ofree[c]);
+                    PROF_ADD(12);
                     ph_ofree[c] ^= 1;
                 }
                 tc_fence_after();
                 const uint32_t va = sRing + vslot * C::kTileBytes;
 #pragma unroll
-                for (int k = 0; k < kTileN / 16; ++k)
+                for (int k = 0; k < kTileN / 32; ++k)
                     umma_ts(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
                             make_smem_desc(va + k * (kBlock * 128), C::kHalfBytes, 1024), idesc_o, (!first || k > 0) ? 1u : 0u);
+                mbar_wait(bar(kBarPHi + c), ph_p[c]);
+                ph_p[c] ^= 1;
+                tc_fence_after();
+#pragma unroll
+                for (int k = kTileN / 32; k < kTileN / 16; ++k)
+                    umma_ts(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
+                            make_smem_desc(va + k * (kBlock * 128), C::kHalfBytes, 1024), idesc_o, 1u);
             };
             for (int u = u_begin; u < u_end; ++u) {
                 const WorkUnit wu = P.units[u];
                 const int n = wu.tile_end - wu.tile_begin;
                 if (n <= 0) continue;
-                mbar_wait(bar(kBarQFull), ph_q);
+                {
+                    PROF_T0();
+                    mbar_wait(bar(kBarQFull), ph_q);
+                    PROF_ADD(13);
+                }
                 ph_q ^= 1;
                 if (wu.mode == kModePair) {
                     uint32_t ks = take_k();
@@ -515,19 +643,26 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     umma_commit(bar(kBarKvEmpty + ks));
                     if (n == 1) umma_commit(bar(kBarQEmpty));
                     for (int j = 0; j < n; ++j) {
+                        PROF_TRACE(0, j, 0);
                         const uint32_t vs = take_v();
+                        PROF_TRACE(0, j, 1);
                         pv(0, vs, j == 0);
+                        PROF_TRACE(0, j, 2);
                         if (j == n - 1) umma_commit(bar(kBarOFull + 0));
                         if (j + 1 < n) {
                             ks = take_k();
                             tc_fence_after();
+                            PROF_TRACE(0, j, 3);
                             qk(0, 0, ks);
+                            PROF_TRACE(0, j, 4);
                         }
                         pv(1, vs, j == 0);
+                        PROF_TRACE(0, j, 5);
                         umma_commit(bar(kBarKvEmpty + vs));
                         if (j == n - 1) umma_commit(bar(kBarOFull + 1));
                         if (j + 1 < n) {
                             qk(1, 1, ks);
+                            PROF_TRACE(0, j, 6);
                             umma_commit(bar(kBarKvEmpty + ks));
                             if (j + 2 == n) umma_commit(bar(kBarQEmpty));
                         }
@@ -560,6 +695,10 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     }
                 }
             }
+#if defined(MSA_PROF) && MSA_PROF != 2
+            prof_acc[14] = static_cast<unsigned long long>(clock64() - prof_mma_start);
+            PROF_FLUSH(8, 15);
+#endif
         }
     }
 

@@ -249,6 +249,66 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi)
     asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
     return r;
 }
+// Packed fp32 pairs (sm_100 FFMA2 / FADD2): one issue slot for two lanes of the softmax row.
+__device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c)
+{
+    uint64_t d;
+    asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;"
+        : "=l"(d)
+        : "l"(*reinterpret_cast<uint64_t *>(&a)), "l"(*reinterpret_cast<uint64_t *>(&b)),
+          "l"(*reinterpret_cast<uint64_t *>(&c)));
+    return *reinterpret_cast<float2 *>(&d);
+}
+__device__ __forceinline__ float2 fadd2(float2 a, float2 b)
+{
+    uint64_t d;
+    asm("add.rn.ftz.f32x2 %0, %1, %2;"
+        : "=l"(d)
+        : "l"(*reinterpret_cast<uint64_t *>(&a)), "l"(*reinterpret_cast<uint64_t *>(&b)));
+    return *reinterpret_cast<float2 *>(&d);
+}
+__device__ __forceinline__ float2 fadd2_rm(float2 a, float2 b)   // round toward -inf
+{
+    uint64_t d;
+    asm("add.rm.ftz.f32x2 %0, %1, %2;"
+        : "=l"(d)
+        : "l"(*reinterpret_cast<uint64_t *>(&a)), "l"(*reinterpret_cast<uint64_t *>(&b)));
+    return *reinterpret_cast<float2 *>(&d);
+}
+// 2^x for a pair, on the FMA / ALU pipes instead of the 16-lane MUFU: x = n + f with
+// n = floor(x) taken from the mantissa of x + 1.5*2^23 (rounded down), 2^f by a degree-3
+// polynomial with p(0) = 1 (minimax relative error 8.6e-5 on [0,1), mean bias 7e-6 -- far
+// below the bf16 rounding of P, 2^-9), and n added into the exponent field.  Valid for
+// finite x <= 127; x below -126 is clamped (result 2^-126 instead of a denormal / 0).
+__device__ __forceinline__ float2 ex2_poly2(float2 x)
+{
+    constexpr float kMagic = 12582912.f;   // 1.5 * 2^23
+    x.x = fmaxf(x.x, -126.f);
+    x.y = fmaxf(x.y, -126.f);
+    const float2 r = fadd2_rm(x, make_float2(kMagic, kMagic));
+    const float2 fl = fadd2(r, make_float2(-kMagic, -kMagic));
+    const float2 f = fadd2(x, make_float2(-fl.x, -fl.y));
+    float2 p = ffma2(f, make_float2(0.07706724107265472f, 0.07706724107265472f),
+                     make_float2(0.22764497995376587f, 0.22764497995376587f));
+    p = ffma2(p, f, make_float2(0.6951166391372681f, 0.6951166391372681f));
+    p = ffma2(p, f, make_float2(1.f, 1.f));
+    p.x = __uint_as_float(__float_as_uint(p.x) + (__float_as_uint(r.x) << 23));
+    p.y = __uint_as_float(__float_as_uint(p.y) + (__float_as_uint(r.y) << 23));
+    return p;
+}
+// wait::ld that also names the 32 destination registers, so no consumer of them can be
+// scheduled above the wait by the compiler.
+__device__ __forceinline__ void tmem_wait_ld_regs(uint32_t *r)
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]),
+                   "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]),
+                   "+r"(r[15]), "+r"(r[16]), "+r"(r[17]), "+r"(r[18]), "+r"(r[19]), "+r"(r[20]), "+r"(r[21]),
+                   "+r"(r[22]), "+r"(r[23]), "+r"(r[24]), "+r"(r[25]), "+r"(r[26]), "+r"(r[27]), "+r"(r[28]),
+                   "+r"(r[29]), "+r"(r[30]), "+r"(r[31])
+                 :
+                 : "memory");
+}
 __device__ __forceinline__ uint32_t elect_one()
 {
     uint32_t pred;
