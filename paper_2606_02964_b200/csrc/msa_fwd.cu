@@ -44,9 +44,7 @@ static cudaError_t launch_pipe_emu(const FwdParams &p, int num_ctas, int emu, cu
 {
     switch (emu) {
     case -1: return launch_pipe<D, -1>(p, num_ctas, stream);
-    case 0: return launch_pipe<D, 0>(p, num_ctas, stream);
     case 2: return launch_pipe<D, 2>(p, num_ctas, stream);
-    case 4: return launch_pipe<D, 4>(p, num_ctas, stream);
     default: return launch_pipe<D, kDefaultEmu>(p, num_ctas, stream);
     }
 }

@@ -185,16 +185,20 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             // Row state: integer reference `ref` (log2 units), l = sum of 2^(s*sl - ref) so far,
             // m_run = running max of the raw scores.  See msa_softmax.cuh.
             float ref = 0.f, l = 0.f, m_run = -INFINITY;
+            bool has_ref = false;
             // Moves the reference up to ceil(m_run*sl) once it lags by more than the lazy
             // threshold: l and O (in TMEM) are multiplied by an exact power of two.  O may be
             // touched here because S of this tile is complete, hence so is PV of the last one.
             auto move_reference = [&](bool have_o) {
                 const float tgt = (m_run == -INFINITY) ? ref : ceilf(m_run * sl);
-                const bool grow = tgt - ref > C::kRescaleThreshold;
+                // a row that has seen no key yet (l = 0, O = 0) takes its first reference as is
+                const bool first = !has_ref && m_run != -INFINITY;
+                const bool grow = first || tgt - ref > C::kRescaleThreshold;
                 if (__any_sync(0xffffffffu, grow)) {
-                    const float alpha = grow ? exp2_int(ref - tgt) : 1.f;
+                    const float alpha = (grow && !first) ? exp2_int(ref - tgt) : 1.f;
                     l *= alpha;
                     if (grow) ref = tgt;
+                    has_ref = has_ref || first;
                     if (have_o) {
 #pragma unroll
                         for (int q = 0; q < D / 16; ++q) {
@@ -230,7 +234,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                 tc_fence_after();
                 PROF_T0();
                 bool done = false;
-                if (EMU >= 0 && !need_mask && s > 0) {
+                if (EMU >= 0 && !need_mask && s > 0 && __all_sync(0xffffffffu, has_ref)) {
                     // fast path: stale reference, tile max found alongside, P handed over in halves
                     move_reference(true);
                     float tile_sum, tile_max;

@@ -44,7 +44,7 @@ enum class FwdVariant : int { Simple = 0, Pipelined = 1 };
 
 // emu: softmax exp2 emulation level of the pipelined kernel (see msa_fwd_pipe.cuh); values
 // without an instantiation fall back to kDefaultEmu.
-constexpr int kDefaultEmu = 3;
+constexpr int kDefaultEmu = 0;
 cudaError_t launch_fwd(const FwdParams &p, int head_dim, int num_ctas, FwdVariant v, int emu, cudaStream_t stream);
 cudaError_t launch_merge(const MergeParams &p, int n_items, int max_rows, cudaStream_t stream);
 int fwd_tiles_per_group(FwdVariant v);   // q tiles (of 128 packed rows) one work item covers

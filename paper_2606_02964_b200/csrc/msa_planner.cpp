@@ -169,43 +169,131 @@ int build_plan(const PlannerConfig &cfg, const msa_request *req, int32_t n_req, 
         }
     }
 
-    // ---- persistent schedule: equal contiguous shares of the global (cost-weighted) tile
-    // sequence (stream-K style: only the items a share boundary falls into are split along KV).
+    // ---- persistent schedule ------------------------------------------------------------
+    // Every CTA gets the same share of the global (cost-weighted) tile count.  Two passes:
+    //  1. whole items, block by block (a block = the q-tile groups of one (run, kv head), which
+    //     all stream the SAME K/V), heaviest blocks first, each member onto one of the currently
+    //     least loaded CTAs.  Equal loads mean equal start times, so the members of a block walk
+    //     their common K/V tiles at the same time on different SMs and all but one of them hit in
+    //     L2 (the contiguous-share schedule this replaces ran them back to back on ONE SM, a full
+    //     pass of every other SM's traffic apart: 5.7x the algorithmic DRAM bytes on cfg2).
+    //  2. the items that fit nowhere whole are cut along KV, stream-K style, into the capacity
+    //     that is left, in CTA order; only those items need the merge kernel.
     const int64_t n_items = static_cast<int64_t>(items.size());
-    std::vector<int64_t> start(n_items + 1, 0);
-    for (int64_t i = 0; i < n_items; ++i)
-        start[i + 1] = start[i] + static_cast<int64_t>(std::max<int32_t>(items[i].n_tiles, 1)) * items[i].cost;
-    const int64_t W = start[n_items];
+    std::vector<int64_t> icost(n_items);
+    int64_t W = 0;
+    for (int64_t i = 0; i < n_items; ++i) {
+        icost[i] = static_cast<int64_t>(std::max<int32_t>(items[i].n_tiles, 1)) * items[i].cost;
+        W += icost[i];
+    }
+    struct Piece { int64_t item; int32_t tb, te; };
     int n_used = 0;
-    std::vector<int64_t> bound;
+    std::vector<std::vector<Piece>> queue;
+    std::vector<int32_t> pieces(n_items, 0);
     if (W > 0) {
         n_used = static_cast<int>(std::min<int64_t>(cfg.num_ctas, std::max<int64_t>(1, W / std::max(1, cfg.min_tiles_per_cta))));
-        bound.resize(n_used + 1);
-        for (int c = 0; c <= n_used; ++c) bound[c] = (W * c) / n_used;
-        for (int c = 1; c < n_used; ++c) {
-            const int64_t b = bound[c];
-            const int64_t i = std::upper_bound(start.begin(), start.end(), b) - start.begin() - 1;   // item holding b
-            const int64_t cost = items[i].cost;
-            const int64_t n_i = std::max<int32_t>(items[i].n_tiles, 1);
-            int64_t tcut = (b - start[i] + cost / 2) / cost;             // nearest tile boundary inside the item
-            if (tcut <= cfg.snap_tiles) tcut = 0;
-            else if (n_i - tcut <= cfg.snap_tiles) tcut = n_i;
-            bound[c] = start[i] + tcut * cost;
+        queue.resize(n_used);
+        std::vector<int64_t> cap(n_used), load(n_used, 0);
+        for (int c = 0; c < n_used; ++c) cap[c] = (W * (c + 1)) / n_used - (W * c) / n_used;
+        // blocks of consecutive items that share (context, kv head)
+        struct Block { int64_t b0, b1, cost; };
+        std::vector<Block> blocks;
+        for (int64_t i = 0; i < n_items;) {
+            int64_t j = i;
+            int64_t cst = 0;
+            while (j < n_items && items[j].vb_begin == items[i].vb_begin && items[j].kvh == items[i].kvh &&
+                   (j == i || items[j].q_row0 > items[j - 1].q_row0)) {
+                cst += icost[j];
+                ++j;
+            }
+            blocks.push_back(Block{i, j, cst});
+            i = j;
         }
-        for (int c = 1; c <= n_used; ++c) bound[c] = std::max(bound[c], bound[c - 1]);
+        std::stable_sort(blocks.begin(), blocks.end(), [](const Block &x, const Block &y) {
+            return x.cost * (y.b1 - y.b0) > y.cost * (x.b1 - x.b0);          // mean member cost, descending
+        });
+        std::vector<int> order(n_used);
+        std::vector<int64_t> leftover;
+        for (const Block &bl : blocks) {
+            for (int64_t m0 = bl.b0; m0 < bl.b1; m0 += n_used) {
+                const int64_t k = std::min<int64_t>(bl.b1 - m0, n_used);
+                for (int c = 0; c < n_used; ++c) order[c] = c;
+                std::partial_sort(order.begin(), order.begin() + k, order.end(),
+                                  [&](int x, int y) { return load[x] != load[y] ? load[x] < load[y] : x < y; });
+                for (int64_t j = 0; j < k; ++j) {
+                    const int64_t it = m0 + j;
+                    const int c = order[j];
+                    if (load[c] + icost[it] <= cap[c] + cfg.snap_tiles) {
+                        queue[c].push_back(Piece{it, 0, std::max<int32_t>(items[it].n_tiles, 0)});
+                        load[c] += icost[it];
+                        pieces[it] = 1;
+                    } else {
+                        leftover.push_back(it);
+                    }
+                }
+            }
+        }
+        std::sort(leftover.begin(), leftover.end());
+        // pass 2: the leftover items form one sequence; CTA c takes the range whose cost matches
+        // the room it has left (cuts at the nearest tile boundary; a cut closer than snap_tiles to
+        // an item edge moves onto the edge)
+        const int64_t n_left = static_cast<int64_t>(leftover.size());
+        std::vector<int64_t> lstart(n_left + 1, 0);
+        for (int64_t k = 0; k < n_left; ++k) lstart[k + 1] = lstart[k] + icost[leftover[k]];
+        const int64_t Wl = lstart[n_left];
+        if (Wl > 0) {
+            std::vector<int64_t> room(n_used);
+            int64_t room_sum = 0;
+            for (int c = 0; c < n_used; ++c) {
+                room[c] = std::max<int64_t>(0, cap[c] - load[c]);
+                room_sum += room[c];
+            }
+            std::vector<int64_t> bound(n_used + 1, 0);
+            int64_t acc = 0;
+            for (int c = 0; c < n_used; ++c) {
+                acc += room[c];
+                bound[c + 1] = room_sum > 0 ? (Wl * acc) / room_sum : (c + 1 == n_used ? Wl : 0);
+            }
+            bound[n_used] = Wl;
+            for (int c = 1; c < n_used; ++c) {
+                const int64_t bnd = bound[c];
+                if (bnd <= 0 || bnd >= Wl) continue;
+                const int64_t k = std::upper_bound(lstart.begin(), lstart.end(), bnd) - lstart.begin() - 1;   // item holding bnd
+                const int64_t cost = items[leftover[k]].cost;
+                const int64_t n_i = std::max<int32_t>(items[leftover[k]].n_tiles, 1);
+                int64_t tcut = (bnd - lstart[k] + cost / 2) / cost;          // nearest tile boundary inside the item
+                if (tcut <= cfg.snap_tiles) tcut = 0;
+                else if (n_i - tcut <= cfg.snap_tiles) tcut = n_i;
+                bound[c] = lstart[k] + tcut * cost;
+            }
+            for (int c = 1; c <= n_used; ++c) bound[c] = std::max(bound[c], bound[c - 1]);
+            // two cuts inside one item closer than the snap window: drop the later one (the CTA
+            // between them had next to no room anyway)
+            for (int c = 1; c < n_used; ++c) {
+                const int64_t k0 = std::upper_bound(lstart.begin(), lstart.end(), bound[c - 1]) - lstart.begin() - 1;
+                if (k0 >= n_left || bound[c] <= bound[c - 1] || bound[c] >= lstart[k0 + 1]) continue;
+                if (bound[c] - bound[c - 1] <= cfg.snap_tiles * static_cast<int64_t>(items[leftover[k0]].cost)) bound[c] = bound[c - 1];
+            }
+            int64_t k = 0;
+            for (int c = 0; c < n_used; ++c) {
+                const int64_t lo = bound[c], hi = bound[c + 1];
+                while (k < n_left && lstart[k + 1] <= lo) ++k;
+                for (int64_t j = k; j < n_left && lstart[j] < hi; ++j) {
+                    const int64_t a = std::max(lo, lstart[j]), b2 = std::min(hi, lstart[j + 1]);
+                    if (b2 <= a) continue;
+                    const Item &it = items[leftover[j]];
+                    Piece pc{leftover[j], 0, 0};
+                    if (it.n_tiles > 0) {
+                        pc.tb = static_cast<int32_t>((a - lstart[j]) / it.cost);
+                        pc.te = static_cast<int32_t>((b2 - lstart[j]) / it.cost);
+                    }
+                    queue[c].push_back(pc);
+                    ++pieces[leftover[j]];
+                }
+            }
+        }
     }
 
-    // pieces per item
-    std::vector<int32_t> pieces(n_items, 0);
-    {
-        int64_t i = 0;
-        for (int c = 0; c < n_used; ++c) {
-            const int64_t lo = bound[c], hi = bound[c + 1];
-            while (i < n_items && start[i + 1] <= lo) ++i;
-            for (int64_t j = i; j < n_items && start[j] < hi; ++j)
-                if (std::min(hi, start[j + 1]) > std::max(lo, start[j])) ++pieces[j];
-        }
-    }
     std::vector<int64_t> item_first_off(n_items, -1);
     std::vector<int32_t> item_emitted(n_items, 0);
     int64_t ws = 0;
@@ -228,44 +316,33 @@ int build_plan(const PlannerConfig &cfg, const msa_request *req, int32_t n_req, 
     if (ws > static_cast<int64_t>(INT32_MAX)) return MSA_ERR_OUT_OF_RANGE;   // partial_off is int32 (floats)
 
     hp.cta_unit_begin.assign(n_used + 1, 0);
-    {
-        int64_t i = 0;
-        for (int c = 0; c < n_used; ++c) {
-            hp.cta_unit_begin[c] = static_cast<int32_t>(hp.units.size());
-            const int64_t lo = bound[c], hi = bound[c + 1];
-            while (i < n_items && start[i + 1] <= lo) ++i;
-            for (int64_t j = i; j < n_items && start[j] < hi; ++j) {
-                const int64_t a = std::max(lo, start[j]), b = std::min(hi, start[j + 1]);
-                if (b <= a) continue;
-                const Item &it = items[j];
-                WorkUnit u{};
-                u.q_row0 = it.q_row0;
-                u.n_tok = it.n_tok;
-                u.q_abs0 = it.q_abs0;
-                u.kvh = it.kvh;
-                u.vb_begin = it.vb_begin;
-                u.vb_count = it.vb_count;
-                u.mode = it.mode;
-                u.tile_info_begin = it.ti_begin;
-                if (it.n_tiles == 0) {
-                    u.tile_begin = u.tile_end = 0;
-                } else {
-                    u.tile_begin = static_cast<int32_t>((a - start[j]) / it.cost);
-                    u.tile_end = static_cast<int32_t>((b - start[j]) / it.cost);
-                }
-                if (pieces[j] > 1) {
-                    const int64_t rows = static_cast<int64_t>(it.n_tok) * cfg.G;
-                    const int64_t stride = (rows * (cfg.D + 1) + 3) / 4 * 4;
-                    u.partial_off = static_cast<int32_t>(item_first_off[j] + stride * item_emitted[j]);
-                    ++item_emitted[j];
-                } else {
-                    u.partial_off = -1;
-                }
-                hp.units.push_back(u);
+    for (int c = 0; c < n_used; ++c) {
+        hp.cta_unit_begin[c] = static_cast<int32_t>(hp.units.size());
+        for (const Piece &pc : queue[c]) {
+            const Item &it = items[pc.item];
+            WorkUnit u{};
+            u.q_row0 = it.q_row0;
+            u.n_tok = it.n_tok;
+            u.q_abs0 = it.q_abs0;
+            u.kvh = it.kvh;
+            u.vb_begin = it.vb_begin;
+            u.vb_count = it.vb_count;
+            u.mode = it.mode;
+            u.tile_info_begin = it.ti_begin;
+            u.tile_begin = pc.tb;
+            u.tile_end = pc.te;
+            if (pieces[pc.item] > 1) {
+                const int64_t rows = static_cast<int64_t>(it.n_tok) * cfg.G;
+                const int64_t stride = (rows * (cfg.D + 1) + 3) / 4 * 4;
+                u.partial_off = static_cast<int32_t>(item_first_off[pc.item] + stride * item_emitted[pc.item]);
+                ++item_emitted[pc.item];
+            } else {
+                u.partial_off = -1;
             }
+            hp.units.push_back(u);
         }
-        hp.cta_unit_begin[n_used] = static_cast<int32_t>(hp.units.size());
     }
+    hp.cta_unit_begin[n_used] = static_cast<int32_t>(hp.units.size());
 
     hp.workspace_floats = ws;
     hp.info.num_ctas = n_used;

@@ -86,20 +86,24 @@ __device__ __forceinline__ bool softmax_fast_tile(uint32_t tS, float sl, float r
     mark(1);
     float mx = fmaxf(chunk_max(c0), chunk_max(c1));
     softmax_chunk<EMU>(c0, sl2, nr2, sa, sb, pk0);
-    softmax_chunk<EMU>(c1, sl2, nr2, sa, sb, pk1);
-    mark(2);
+    // the second half has landed by now: its row max is found among the arithmetic of chunk 1,
+    // so the guard is ready as soon as the first half of P is
     tmem_wait_ld_regs(c2);
     tmem_wait_ld_regs(c3);
     mx = fmaxf(mx, fmaxf(chunk_max(c2), chunk_max(c3)));
+    softmax_chunk<EMU>(c1, sl2, nr2, sa, sb, pk1);
+    mark(2);
     tile_max = mx;
     if (__any_sync(0xffffffffu, !(fmaf(mx, sl, -ref) <= kGuardLog2))) return false;
     mark(3);
     tmem_st16(tS, pk0);
     tmem_st16(tS + 16, pk1);
+    // the first half is published one chunk later: its stores have completed by then (no stall),
+    // and O += P V of keys 0-63 still finishes long before the second half is ready
+    softmax_chunk<EMU>(c2, sl2, nr2, sa, sb, pk0);
     tmem_wait_st();
     tc_fence_before();
     arrive_lo();
-    softmax_chunk<EMU>(c2, sl2, nr2, sa, sb, pk0);
     tmem_st16(tS + 32, pk0);
     softmax_chunk<EMU>(c3, sl2, nr2, sa, sb, pk1);
     tmem_st16(tS + 48, pk1);

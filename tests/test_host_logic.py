@@ -155,11 +155,16 @@ def _check_plan(p):
                 else:
                     assert e["paged"] == 0 and e["src"] == p.seg_row_off[s] + 16 * b
                 i += 1
-    # balance of the persistent schedule: shares differ by at most one item's snap window
+    # balance of the persistent schedule (whole items first, leftovers cut into the room that is left):
+    # shares differ by a few snap windows at most
     per_cta = np.array([sum(max(1, int(u["tile_end"]) - int(u["tile_begin"])) * (2 if u["mode"] == 0 else 1)
                             for u in units[cta[c]:cta[c + 1]]) for c in range(info["num_ctas"])])
     if info["num_ctas"] > 1 and per_cta.sum() >= 148 * 16:
-        assert per_cta.max() - per_cta.min() <= 12, (per_cta.min(), per_cta.max())
+        assert per_cta.max() - per_cta.min() <= max(24, 0.01 * per_cta.mean()), (per_cta.min(), per_cta.max())
+    # no sliver pieces: a split item is never cut within two tiles of its ends
+    for (q_row0, kvh), us in items.items():
+        if len(us) > 1:
+            assert all(int(u["tile_end"]) - int(u["tile_begin"]) > 2 for u in us), (q_row0, kvh)
     # per-tile mask summaries agree with the (padded) virtual block list
     ti = msa_plan_export(plan, 4)
     assert len(vb) % 8 == 0 and len(ti) == len(vb) // 8
