@@ -122,6 +122,35 @@ def test_split_kv_merge_path_and_determinism():
         compare(p, o1.float().cpu().numpy().astype(np.float64), l1.cpu().numpy().astype(np.float64))
 
 
+def _contig_problem(L, T, seed):
+    ctx = ContextSpec([(SEG_CONTIG, 0, L), (SEG_SELF, L, T)])
+    return build_problem("extreme", 8, 2, 128, [ctx], [RunSpec(0, L, T)], seed=seed, device=DEV, keep_dense=False)
+
+
+def test_all_scores_far_below_zero():
+    """Every score ~ -100 (log2 units -150): the row reference must follow the scores DOWN on the
+    first tile, otherwise every p underflows and l = 0."""
+    p = _contig_problem(700, 70, 41)
+    p.q.copy_((p.q.float().abs() * 16).to(torch.bfloat16))
+    p.contig_k.copy_((-p.contig_k.float().abs()).to(torch.bfloat16))
+    o, lse, _ = gpu_forward(p)
+    assert np.all(np.isfinite(lse)) and lse.max() < -50.0
+    compare(p, o, lse, strict=False)
+
+
+def test_score_jump_beyond_the_fast_path_guard():
+    """Keys 0..255 score ~ +3, every later key ~ +115 nats (a jump of ~2^160 between two KV tiles):
+    the stale-reference fast path must refuse the tile (overflow guard) and redo it exactly."""
+    p = _contig_problem(900, 70, 42)
+    p.q.copy_((p.q.float().abs() * 16).to(torch.bfloat16))
+    k = p.contig_k.float().abs()
+    k[:256] *= 2.0 ** -6
+    p.contig_k.copy_(k.to(torch.bfloat16))
+    o, lse, _ = gpu_forward(p)
+    assert lse.min() > 50.0
+    compare(p, o, lse, strict=False)
+
+
 def test_empty_batch_and_zero_length_run():
     p = W.random_problem(5, n_req=2, Hq=4, Hkv=2, D=64, device=DEV)
     h = msa_create(p.Hq, p.Hkv, p.D)
