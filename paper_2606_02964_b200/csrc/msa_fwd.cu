@@ -24,28 +24,30 @@ static cudaError_t launch_simple(const FwdParams &p, int num_ctas, cudaStream_t 
     return cudaGetLastError();
 }
 
-template <int D, int EMU>
+template <int D, int EMU, int EMU_HI>
 static cudaError_t launch_pipe(const FwdParams &p, int num_ctas, cudaStream_t stream)
 {
     using C = PipeCfg<D>;
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(msa_fwd_pipe_kernel<D, EMU>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(msa_fwd_pipe_kernel<D, EMU, EMU_HI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              C::kSmemBytes);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    msa_fwd_pipe_kernel<D, EMU><<<num_ctas, 512, C::kSmemBytes, stream>>>(p);
+    msa_fwd_pipe_kernel<D, EMU, EMU_HI><<<num_ctas, 512, C::kSmemBytes, stream>>>(p);
     return cudaGetLastError();
 }
 
+// emu = 10 * (pairs of 8 emulated in the first half of a tile) + (same for the second half); -1: exact path only
 template <int D>
 static cudaError_t launch_pipe_emu(const FwdParams &p, int num_ctas, int emu, cudaStream_t stream)
 {
     switch (emu) {
-    case -1: return launch_pipe<D, -1>(p, num_ctas, stream);
-    case 2: return launch_pipe<D, 2>(p, num_ctas, stream);
-    default: return launch_pipe<D, kDefaultEmu>(p, num_ctas, stream);
+    case -1: return launch_pipe<D, -1, 0>(p, num_ctas, stream);
+    case 0: return launch_pipe<D, 0, 0>(p, num_ctas, stream);
+    case 22: return launch_pipe<D, 2, 2>(p, num_ctas, stream);
+    default: return launch_pipe<D, kDefaultEmu / 10, kDefaultEmu % 10>(p, num_ctas, stream);
     }
 }
 

@@ -111,7 +111,7 @@ struct ResolvedVb {
 // EMU: of every 8 element pairs of a softmax row, how many take 2^x from ex2_poly2 (FMA/ALU
 // pipes) instead of MUFU.EX2; -1 disables the stale-max fast path altogether (two-phase
 // max-then-exp on every tile, all MUFU).
-template <int D, int EMU>
+template <int D, int EMU, int EMU_HI>
 __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_constant__ FwdParams P)
 {
     using C = PipeCfg<D>;
@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     // fast path: stale reference, tile max found alongside, P handed over in halves
                     move_reference(true);
                     float tile_sum, tile_max;
-                    done = softmax_fast_tile<(EMU < 0 ? 0 : EMU)>(tS, sl, ref, tile_sum, tile_max, [&]() {
+                    done = softmax_fast_tile<(EMU < 0 ? 0 : EMU), EMU_HI>(tS, sl, ref, tile_sum, tile_max, [&]() {
                         __syncwarp();
                         if (lane == 0) mbar_arrive(bar(kBarPLo + c));
                         if ((threadIdx.x & 127) == 0) PROF_TRACE(1 + c, s, 4);
@@ -603,7 +603,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             };
             // O += P V in two halves: keys 0-63 as soon as the softmax warps have published the
             // first half of P, keys 64-127 after the second.
-            auto pv = [&](int c, uint32_t vslot, bool first) {
+            auto pv_lo = [&](int c, uint32_t vslot, bool first) {
                 {
                     PROF_T0();
                     mbar_wait(bar(kBarPLo + c), ph_p[c]);
@@ -621,13 +621,20 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                 for (int k = 0; k < kTileN / 32; ++k)
                     umma_ts(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
                             make_smem_desc(va + k * (kBlock * 128), C::kHalfBytes, 1024), idesc_o, (!first || k > 0) ? 1u : 0u);
+            };
+            auto pv_hi = [&](int c, uint32_t vslot) {
                 mbar_wait(bar(kBarPHi + c), ph_p[c]);
                 ph_p[c] ^= 1;
                 tc_fence_after();
+                const uint32_t va = sRing + vslot * C::kTileBytes;
 #pragma unroll
                 for (int k = kTileN / 32; k < kTileN / 16; ++k)
                     umma_ts(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
                             make_smem_desc(va + k * (kBlock * 128), C::kHalfBytes, 1024), idesc_o, 1u);
+            };
+            auto pv = [&](int c, uint32_t vslot, bool first) {
+                pv_lo(c, vslot, first);
+                pv_hi(c, vslot);
             };
             for (int u = u_begin; u < u_end; ++u) {
                 const WorkUnit wu = P.units[u];
@@ -650,12 +657,17 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                         PROF_TRACE(0, j, 0);
                         const uint32_t vs = take_v();
                         PROF_TRACE(0, j, 1);
-                        pv(0, vs, j == 0);
-                        PROF_TRACE(0, j, 2);
-                        if (j == n - 1) umma_commit(bar(kBarOFull + 0));
+                        // the K tile of the next step is taken while the second half of P is still
+                        // being formed, so QK follows PV without a barrier round trip in between
+                        pv_lo(0, vs, j == 0);
                         if (j + 1 < n) {
                             ks = take_k();
                             tc_fence_after();
+                        }
+                        pv_hi(0, vs);
+                        PROF_TRACE(0, j, 2);
+                        if (j == n - 1) umma_commit(bar(kBarOFull + 0));
+                        if (j + 1 < n) {
                             PROF_TRACE(0, j, 3);
                             qk(0, 0, ks);
                             PROF_TRACE(0, j, 4);

@@ -69,7 +69,7 @@ __device__ __forceinline__ void softmax_chunk(const uint32_t (&sr)[32], float2 s
 // first half and the caller arrives for the second.  `mark(i)` is a profiling hook (no-op in
 // the shipped build).  tile_sum = sum of p against `ref`,
 // tile_max = max raw score.
-template <int EMU, class ArriveLo, class Mark>
+template <int EMU, int EMU_HI, class ArriveLo, class Mark>
 __device__ __forceinline__ bool softmax_fast_tile(uint32_t tS, float sl, float ref, float &tile_sum, float &tile_max,
                                                   ArriveLo &&arrive_lo, Mark &&mark)
 {
@@ -100,12 +100,12 @@ __device__ __forceinline__ bool softmax_fast_tile(uint32_t tS, float sl, float r
     tmem_st16(tS + 16, pk1);
     // the first half is published one chunk later: its stores have completed by then (no stall),
     // and O += P V of keys 0-63 still finishes long before the second half is ready
-    softmax_chunk<EMU>(c2, sl2, nr2, sa, sb, pk0);
+    softmax_chunk<EMU_HI>(c2, sl2, nr2, sa, sb, pk0);
     tmem_wait_st();
     tc_fence_before();
     arrive_lo();
     tmem_st16(tS + 32, pk0);
-    softmax_chunk<EMU>(c3, sl2, nr2, sa, sb, pk1);
+    softmax_chunk<EMU_HI>(c3, sl2, nr2, sa, sb, pk1);
     tmem_st16(tS + 48, pk1);
     tile_sum = (sa.x + sb.x) + (sa.y + sb.y);
     mark(5);
