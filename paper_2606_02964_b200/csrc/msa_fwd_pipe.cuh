@@ -11,11 +11,13 @@
 //
 // Two independent "chains" keep the tensor core busy while the other chain's softmax runs:
 //   kModePair   chain c owns q tile c of the unit; both chains consume every KV tile
-//   kModeSplit  one q tile; chain c owns KV tiles c, c+2, ... with its own (m, l, O);
+//   kModeSplit  one q tile; chain c owns KV tiles c, c+2, ... with its own (ref, l, O);
 //               the epilogue merges the two partial softmaxes (short / decode-like queries)
 // TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P (bf16) aliases
-// the first 64 columns of its S.  Shared memory: Q 2 tiles, one ring of 5 tile slots in which
-// K and V tiles alternate (entry 2i = K of the CTA's i-th KV tile, 2i+1 = its V).
+// the first 64 columns of its S and is handed to the MMA warp in two halves (keys 0-63, 64-127).
+// Shared memory: Q 2 tiles, one ring of 5 tile slots in which K and V tiles alternate (entry
+// 2i = K of the CTA's i-th KV tile, 2i+1 = its V).  The softmax arithmetic, its integer row
+// reference and the overflow guard of the fast path are described in msa_softmax.cuh.
 //
 // Invalid KV slots (block tails, blocks past a context's end) never reach O: their scores
 // are replaced by -inf, and their K/V rows are never written by TMA -- partly filled blocks
