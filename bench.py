@@ -160,7 +160,7 @@ def run_mine(args, rank: int, world: int, local_rank: int):
 
     def bench_workload(name: str, steps: int, warmup: int, do_e2e: bool):
         metric, unit, bound = metric_of(name)
-        p = W.CONFIGS[name](device=dev)
+        p = {**W.CONFIGS, **W.EXTRA_CONFIGS}[name](device=dev)
         alg = p.algorithmic()
         units_per_step = alg["flops"] / 1e12 if bound == "tensor" else alg["bytes"] / 1e9
         s = MsaSession(p, device=local_rank)
@@ -286,8 +286,9 @@ def run_reference(args, rank: int, world: int):
     p = W.CONFIGS[args.workload](device="cpu") if args.workload in ("cfg1_tiny",) else None
     if p is None:
         # values on the CPU; only the requests sampled are ever read
-        small = dict(cfg2_llama8b=dict(n_req=2), cfg4_mixed=dict(n_req=4), cfg5_short_query=dict(n_req=8))
-        p = W.CONFIGS[args.workload](device="cpu", **small.get(args.workload, {}))
+        small = dict(cfg2_llama8b=dict(n_req=2), cfg4_mixed=dict(n_req=4), cfg5_short_query=dict(n_req=8),
+                     f1_hybrid_pod=dict(n_prefill=1, n_decode=2))
+        p = {**W.CONFIGS, **W.EXTRA_CONFIGS}[args.workload](device="cpu", **small.get(args.workload, {}))
     reqs = list(range(min(2, p.n_req)))
     dt, fl, pairs, n = oracle_sample(p, 8, 1, reqs)
     total = max(1, args.steps + args.warmup)
@@ -319,7 +320,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="mine", choices=["mine", "reference"])
     ap.add_argument("--workload", default="cfg2_llama8b",
-                    choices=["cfg2_llama8b", "cfg3_70b_long", "cfg4_mixed", "cfg5_short_query"])
+                    choices=["cfg2_llama8b", "cfg3_70b_long", "cfg4_mixed", "cfg5_short_query", "f1_hybrid_pod"])
     ap.add_argument("--no-secondary", action="store_true")
     args = ap.parse_args()
     rank, world, local_rank = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)

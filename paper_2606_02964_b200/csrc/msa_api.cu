@@ -208,6 +208,7 @@ int msa_plan_create(msa_handle h, const msa_request *requests, int32_t n_req, co
     pc.R = h->R;
     pc.tiles_per_group = fwd_tiles_per_group(h->variant);
     pc.num_ctas = h->num_sms;
+    if (const char *nc = getenv("MSA_NUM_CTAS")) pc.num_ctas = std::max(1, std::min(h->num_sms, atoi(nc)));   // debug: scaling experiments
     msa_plan p = new (std::nothrow) msa_plan_s();
     if (!p) return MSA_ERR_INVALID_ARG;
     p->h = h;

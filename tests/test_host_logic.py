@@ -187,6 +187,12 @@ def test_planner_on_the_five_configs(name):
         assert info["num_ctas"] == 148 and info["num_split_items"] <= 148
 
 
+def test_planner_on_the_hybrid_prefill_plus_decode_workload():
+    """several runs share one segment list, decode rows ride in the same launch."""
+    info = _check_plan(W.f1_hybrid_pod(layout_only=True))
+    assert info["num_ctas"] == 148 and info["num_split_items"] <= 148
+
+
 @pytest.mark.parametrize("seed,kw", [(1, dict()), (2, dict(gaps=True, hybrid=True)), (3, dict(Hq=6, Hkv=2, max_ctx=3000)),
                                      (4, dict(n_req=9, max_q=5, max_ctx=50)), (5, dict(Hq=16, Hkv=1, D=128))])
 def test_planner_on_random_problems(seed, kw):

@@ -206,7 +206,7 @@ def test_forward_host_matches_forward_and_error_codes():
 
 # ------------------------------------------------------------------ configs 2-5 at full size (sampled rows)
 def _full_config(name, n_req_sample, n_random, seed):
-    p = W.CONFIGS[name](device=DEV)
+    p = {**W.CONFIGS, **W.EXTRA_CONFIGS}[name](device=DEV)
     o, lse, info = gpu_forward(p)
     rng = np.random.default_rng(seed)
     reqs = sorted(int(x) for x in rng.choice(p.n_req, size=min(n_req_sample, p.n_req), replace=False))
@@ -230,3 +230,8 @@ def test_cfg4_mixed_full_size_sampled_rows():
 
 def test_cfg5_short_query_full_size_sampled_rows():
     _full_config("cfg5_short_query", 24, 0, 5)
+
+
+def test_f1_hybrid_prefill_plus_decode_full_size_sampled_rows():
+    """Hybrid chunks (compute -> cached -> compute sharing one segment list) and 128 decode rows in ONE launch."""
+    _full_config("f1_hybrid_pod", 40, 2, 6)

@@ -543,5 +543,49 @@ def cfg5_short_query(device="cpu", layout_only=False, n_req: int = 256) -> MsaPr
                          pool_blocks=int(1.02 * cached_blocks) + 1, layout_only=layout_only)
 
 
+def f1_hybrid_pod(device="cpu", layout_only=False, n_prefill: int = 16, n_decode: int = 128) -> MsaProblem:
+    """SURVEY.md section 8 (f1): hybrid chunks and decode rows in ONE launch (PAPER.md:92 step 5, :247;
+    the POD-Attention setting of PAPER.md:310).  Llama-3-8B shape.  Each prefill request: prior context
+    L = 16 * U{256..512} tokens in 4 segments alternating cached-paged / recomputed-contiguous, then a
+    chunk of 512 positions of which the middle 128 are already cached: compute run A (256 tokens),
+    cached run (128, paged), compute run B (128 tokens); both runs share one segment list.  Each decode
+    request: one query token behind U[1024, 8192] cached tokens (paged, one contiguous tail <= 64)."""
+    rng = np.random.default_rng(1006)
+    ctxs, runs = [], []
+    cached_blocks = 0
+    for r in range(n_prefill):
+        L = BLOCK * int(rng.integers(256, 513))
+        cuts = np.sort(rng.choice(np.arange(1, L // BLOCK), size=3, replace=False)) * BLOCK
+        bounds = np.concatenate([[0], cuts, [L]]).astype(np.int64)
+        segs = []
+        for j in range(4):
+            kind = SEG_PAGED if j % 2 == 0 else SEG_CONTIG
+            n = int(bounds[j + 1] - bounds[j])
+            segs.append((kind, int(bounds[j]), n))
+            if kind == SEG_PAGED:
+                cached_blocks += (n + BLOCK - 1) // BLOCK
+        segs += [(SEG_SELF, L, 256), (SEG_PAGED, L + 256, 128), (SEG_SELF, L + 384, 128)]
+        cached_blocks += 128 // BLOCK
+        ci = len(ctxs)
+        ctxs.append(ContextSpec(segs))
+        runs.append(RunSpec(ci, L, 256))
+        runs.append(RunSpec(ci, L + 384, 128))
+    for r in range(n_decode):
+        L = int(rng.integers(1024, 8193))
+        tail = int(rng.integers(0, 65))
+        segs = [(SEG_PAGED, 0, L - tail)]
+        cached_blocks += (L - tail + BLOCK - 1) // BLOCK
+        if tail:
+            segs.append((SEG_CONTIG, L - tail, tail))
+        segs.append((SEG_SELF, L, 1))
+        ci = len(ctxs)
+        ctxs.append(ContextSpec(segs))
+        runs.append(RunSpec(ci, L, 1))
+    return build_problem("f1_hybrid_pod", 32, 8, 128, ctxs, runs, seed=1006, device=device,
+                         pool_blocks=int(1.1 * cached_blocks) + 1, layout_only=layout_only)
+
+
 CONFIGS = dict(cfg1_tiny=cfg1_tiny, cfg2_llama8b=cfg2_llama8b, cfg3_70b_long=cfg3_70b_long,
                cfg4_mixed=cfg4_mixed, cfg5_short_query=cfg5_short_query)
+# workloads beyond BASELINE.json's five (SURVEY.md section 8 (f) "next" rows)
+EXTRA_CONFIGS = dict(f1_hybrid_pod=f1_hybrid_pod)
