@@ -46,6 +46,15 @@ def measured_peaks():
         return 1590.0, 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def sustained_tflops():
+    """Seconds-long cuBLAS bf16 loop under the power cap (context for launches that run back to back for long)."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["bf16_tflops_sustained"])
+    except Exception:
+        return 1400.0
+
+
 def committed_traffic(workload: str):
     """dram bytes per launch of the dominant kernel from the committed ncu capture
     (profiles/roofline_traffic.csv, copied by hand from the `ncu --set full` summaries), or None."""
@@ -202,7 +211,8 @@ def run_mine(args, rank: int, world: int, local_rank: int):
                                  frac=(achieved / peak) if achieved else None, traffic=traffic,
                                  kernel="msa_fwd", kernel_ms=fwd_ms, merge_ms=merge_ms, steps_timed=n_rec,
                                  peak_source=peak_label,
-                                 frac_of_nominal=(achieved / (2250.0 if bound == "tensor" else 8000.0)) if achieved else None),
+                                 frac_of_nominal=(achieved / (2250.0 if bound == "tensor" else 8000.0)) if achieved else None,
+                                 frac_of_sustained=(achieved / sustained_tflops()) if (achieved and bound == "tensor") else None),
                    clocks=clocks, plan=s.info, algorithmic=alg)
         if do_e2e:
             qh = p.q.cpu().pin_memory()
