@@ -284,6 +284,80 @@ def run_mine(args, rank: int, world: int, local_rank: int):
         print(json.dumps(line))
 
 
+def run_fig13(args):
+    """SURVEY.md section 8 (f2), the shape of the paper's Fig. 13: N cached tokens + 128 new tokens,
+    Llama-3-8B heads.  One fused msa_forward over both segments against the same kernel called once per segment
+    with a host synchronisation after each call and an LSE merge of the two partial results (torch ops)."""
+    import torch
+    import workloads as W
+    from paper_2606_02964_b200 import (make_descriptors, msa_create, msa_destroy, msa_forward, msa_plan_create,
+                                       msa_plan_destroy, msa_workspace_bytes)
+    import __graft_entry__ as ge
+    ge.build()
+    dev = "cuda:0"
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream().cuda_stream
+    rows = []
+    for N in (1024, 2048, 4096, 8192, 10240):
+        ctx = W.ContextSpec([(W.SEG_PAGED, 0, N), (W.SEG_SELF, N, 128)])
+        p = W.build_problem(f"fig13_{N}", 32, 8, 128, [ctx], [W.RunSpec(0, N, 128)], seed=1300 + N, device=dev)
+        h = msa_create(p.Hq, p.Hkv, p.D, p.q_to_kv, device=0)
+
+        def plan_of(lo, hi):
+            req = np.array([[0, 128, N, 0, hi - lo]], np.int32)
+            R, n, S, m = make_descriptors(req, p.seg_kind[lo:hi], p.seg_abs_start[lo:hi], p.seg_len[lo:hi],
+                                          p.seg_block_off[lo:hi], p.seg_row_off[lo:hi])
+            pl = msa_plan_create(h, R, n, S, m)
+            nb = msa_workspace_bytes(pl)
+            ws = torch.empty(max(nb, 16), dtype=torch.uint8, device=dev) if nb else None
+            return pl, ws, torch.zeros_like(p.q), torch.zeros(p.total_q, p.Hq, dtype=torch.float32, device=dev)
+
+        plans = [plan_of(0, 2), plan_of(0, 1), plan_of(1, 2)]
+
+        def fwd(k):
+            pl, ws, o, lse = plans[k]
+            msa_forward(h, pl, p.q, p.pool_k, p.pool_v, p.block_table, p.contig_k, p.contig_v, p.scale, o, lse, ws, stream)
+            return o, lse
+
+        def fused():
+            o, lse = fwd(0)
+            torch.cuda.synchronize()
+            return o, lse
+
+        def per_segment():
+            oa, la = fwd(1)
+            torch.cuda.synchronize()
+            ob, lb = fwd(2)
+            torch.cuda.synchronize()
+            lse = torch.logaddexp(la, lb)
+            o = (torch.exp(la - lse).unsqueeze(-1) * oa.float() + torch.exp(lb - lse).unsqueeze(-1) * ob.float()).to(torch.bfloat16)
+            torch.cuda.synchronize()
+            return o, lse
+
+        for _ in range(max(3, args.warmup)):
+            o1, l1 = fused()
+            o2, l2 = per_segment()
+        d_o = float((o1.float() - o2.float()).abs().max())
+        d_l = float((l1 - l2).abs().max())
+        t = {}
+        for name, fn in (("fused", fused), ("per_segment", per_segment)):
+            t0 = time.perf_counter()
+            for _ in range(args.steps):
+                fn()
+            t[name] = (time.perf_counter() - t0) / args.steps * 1e6
+        rows.append(dict(cached_tokens=N, fused_us=t["fused"], per_segment_us=t["per_segment"],
+                         speedup=t["per_segment"] / t["fused"], max_abs_dO=d_o, max_abs_dLSE=d_l))
+        for pl, _, _, _ in plans:
+            msa_plan_destroy(pl)
+        msa_destroy(h)
+    mean_speedup = float(np.mean([r["speedup"] for r in rows]))
+    print(json.dumps(dict(metric="msa_fused_vs_per_segment_speedup", value=mean_speedup, unit="x", n_gpus=1, steps=args.steps,
+                          warmup=max(3, args.warmup), higher_is_better=True, dtype="bf16", data="synthetic", vs_baseline=None,
+                          config=dict(workload="fig13", Hq=32, Hkv=8, head_dim=128, new_tokens=128,
+                                      timing="host wall clock per call incl. the synchronisation a caller needs"),
+                          fig13=rows, gpu_launches=args.steps * 2)))
+
+
 def run_reference(args, rank: int, world: int):
     """The reference arm of this tier = the fp64 CPU oracle on the box's host cores (rank 0 only)."""
     if rank != 0:
@@ -330,12 +404,15 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="mine", choices=["mine", "reference"])
     ap.add_argument("--workload", default="cfg2_llama8b",
-                    choices=["cfg2_llama8b", "cfg3_70b_long", "cfg4_mixed", "cfg5_short_query", "f1_hybrid_pod"])
+                    choices=["cfg2_llama8b", "cfg3_70b_long", "cfg4_mixed", "cfg5_short_query", "f1_hybrid_pod", "fig13"])
     ap.add_argument("--no-secondary", action="store_true")
     args = ap.parse_args()
     rank, world, local_rank = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
     if args.impl == "reference":
         run_reference(args, rank, world)
+    elif args.workload == "fig13":
+        if rank == 0:
+            run_fig13(args)
     else:
         run_mine(args, rank, world, local_rank)
 
