@@ -145,6 +145,20 @@ def oracle_sample(p, n_rows: int, seed: int, reqs=None):
     return dt, 4.0 * p.D * p.Hq * pairs, pairs, len(rr)
 
 
+def dist_max(value: float, device="cpu") -> float:
+    """Max over ranks of a per-rank scalar (the timing rule: a multi-GPU number is the slowest rank's)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, units_per_step: float, ms: float) -> float:
+    """Replicas only: every rank processes one full batch per step, no exchange on the path."""
+    return world * units_per_step / (ms * 1e-3)
+
+
 def metric_of(workload: str):
     if workload == "cfg5_short_query":
         return "msa_short_query_hbm_gbs", "GB/s", "hbm"
@@ -197,11 +211,8 @@ def run_mine(args, rank: int, world: int, local_rank: int):
         n_rec, fwd_ms, merge_ms = msa_get_timing(s.h)
         msa_set_timing(s.h, 0)
         if world > 1:
-            import torch.distributed as dist
-            t = torch.tensor([ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        value = world * units_per_step / (ms * 1e-3)
+            ms = dist_max(ms, dev)
+        value = whole_job_value(world, units_per_step, ms)
         kern_units = units_per_step          # the forward kernel does all algorithmic work of a step
         achieved = kern_units / (fwd_ms * 1e-3) if fwd_ms > 0 else None
         peak = tfl_peak if bound == "tensor" else gbs_peak
@@ -231,13 +242,10 @@ def run_mine(args, rank: int, world: int, local_rank: int):
             torch.cuda.synchronize()
             ems = e0.elapsed_time(e1) / k_e2e
             if world > 1:
-                import torch.distributed as dist
-                t = torch.tensor([ems], device=dev, dtype=torch.float64)
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-                ems = float(t.item())
+                ems = dist_max(ems, dev)
             h2d = qh.numel() * 2 + ck.numel() * 2 + cv.numel() * 2 + bt.numel() * 4
             d2h = oh.numel() * 2 + lh.numel() * 4
-            out["e2e"] = dict(value=world * units_per_step / (ems * 1e-3), unit=unit, ms_per_step=ems, steps=k_e2e,
+            out["e2e"] = dict(value=whole_job_value(world, units_per_step, ems), unit=unit, ms_per_step=ems, steps=k_e2e,
                               h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
                               note="msa_forward_host: q, block table, contiguous arena from pinned host memory; "
                                    "O and LSE back to host; the paged pool is the resident KV cache")
