@@ -366,6 +366,42 @@ def run_fig13(args):
                           fig13=rows, gpu_launches=args.steps * 2)))
 
 
+def run_evictor(args):
+    """control-plane cost of one eviction (+ the re-insertion that follows) with the O(log n)
+    evictor (Algorithm 1) against the O(n) scan the paper compares with, at 8 K and 100 K cached blocks."""
+    import __graft_entry__ as ge
+    ge.build()
+    from paper_2606_02964_b200 import MsaEvictor
+    rng = np.random.default_rng(7)
+    rows = []
+    for n in (8192, 100_000):
+        for linear in (False, True):
+            ev = MsaEvictor(alpha=600.0, beta=15.0, tau0=540.0, k5=2.5e-9, c0=3.0e-5)
+            pos = rng.integers(0, 32768, size=n) * 16
+            last = rng.uniform(0.0, 3000.0, size=n)
+            for b in range(n):
+                ev.add(b, int(pos[b]), float(last[b]))
+            ops = 20000 if not linear else (2000 if n <= 8192 else 300)
+            t, nid = 3000.0, n
+            t0 = time.perf_counter()
+            for i in range(ops):
+                t += 0.05
+                ev.evict(t, linear=linear)
+                ev.add(nid, int(pos[i % n]), t)          # the freed block is reused and becomes evictable again
+                nid += 1
+            dt = time.perf_counter() - t0
+            rows.append(dict(blocks=n, strategy="linear scan" if linear else "two ordered sets (Algorithm 1)",
+                             us_per_evict_plus_add=dt / ops * 1e6, ops=ops))
+            ev.close()
+    fast = {r["blocks"]: r["us_per_evict_plus_add"] for r in rows if r["strategy"].startswith("two")}
+    slow = {r["blocks"]: r["us_per_evict_plus_add"] for r in rows if r["strategy"].startswith("linear")}
+    print(json.dumps(dict(metric="msa_evictor_us_per_eviction", value=fast[100_000], unit="us", n_gpus=0, steps=1, warmup=0,
+                          higher_is_better=False, dtype="f64", data="synthetic", vs_baseline=None,
+                          config=dict(workload="evictor", note="host only; includes the ctypes call overhead of both strategies alike"),
+                          evictor=rows, speedup_8k=slow[8192] / fast[8192], speedup_100k=slow[100_000] / fast[100_000],
+                          gpu_launches=0)))
+
+
 def run_reference(args, rank: int, world: int):
     """The reference arm of this tier = the fp64 CPU oracle on the box's host cores (rank 0 only)."""
     if rank != 0:
@@ -412,7 +448,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="mine", choices=["mine", "reference"])
     ap.add_argument("--workload", default="cfg2_llama8b",
-                    choices=["cfg2_llama8b", "cfg3_70b_long", "cfg4_mixed", "cfg5_short_query", "f1_hybrid_pod", "fig13"])
+                    choices=["cfg2_llama8b", "cfg3_70b_long", "cfg4_mixed", "cfg5_short_query", "f1_hybrid_pod", "fig13", "evictor"])
     ap.add_argument("--no-secondary", action="store_true")
     args = ap.parse_args()
     rank, world, local_rank = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
@@ -421,6 +457,9 @@ def main():
     elif args.workload == "fig13":
         if rank == 0:
             run_fig13(args)
+    elif args.workload == "evictor":
+        if rank == 0:
+            run_evictor(args)
     else:
         run_mine(args, rank, world, local_rank)
 

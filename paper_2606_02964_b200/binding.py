@@ -58,6 +58,13 @@ _LIB: Optional[ctypes.CDLL] = None
 EXPORTS = ["msa_create", "msa_destroy", "msa_plan_create", "msa_plan_destroy", "msa_plan_get_info",
            "msa_plan_export", "msa_workspace_bytes", "msa_forward", "msa_forward_host",
            "msa_last_launch_count", "msa_set_timing", "msa_get_timing", "msa_strerror", "msa_last_cuda_error", "msa_version"]
+EVICTOR_EXPORTS = ["msa_evictor_create", "msa_evictor_destroy", "msa_evictor_add", "msa_evictor_remove", "msa_evictor_evict",
+                   "msa_evictor_evict_linear", "msa_evictor_set_lambda", "msa_evictor_size", "msa_evictor_weight"]
+
+
+class MsaEvictorConfig(ctypes.Structure):
+    _fields_ = [("alpha", ctypes.c_double), ("beta", ctypes.c_double), ("tau0", ctypes.c_double),
+                ("lambda_", ctypes.c_double), ("k5", ctypes.c_double), ("c0", ctypes.c_double)]
 
 
 def _lib() -> ctypes.CDLL:
@@ -87,6 +94,19 @@ def _lib() -> ctypes.CDLL:
         for f in ("msa_strerror", "msa_last_cuda_error", "msa_version"):
             getattr(lib, f).restype = ctypes.c_char_p
         lib.msa_strerror.argtypes = [ctypes.c_int]
+        f64 = ctypes.c_double
+        lib.msa_evictor_create.argtypes = [ctypes.POINTER(MsaEvictorConfig), ctypes.POINTER(vp)]
+        lib.msa_evictor_destroy.argtypes = [vp]
+        lib.msa_evictor_destroy.restype = None
+        lib.msa_evictor_add.argtypes = [vp, i64, i64, f64]
+        lib.msa_evictor_remove.argtypes = [vp, i64]
+        lib.msa_evictor_evict.argtypes = [vp, f64, ctypes.POINTER(i64)]
+        lib.msa_evictor_evict_linear.argtypes = [vp, f64, ctypes.POINTER(i64)]
+        lib.msa_evictor_set_lambda.argtypes = [vp, f64]
+        lib.msa_evictor_size.argtypes = [vp]
+        lib.msa_evictor_size.restype = i64
+        lib.msa_evictor_weight.argtypes = [vp, i64, f64]
+        lib.msa_evictor_weight.restype = f64
         _LIB = lib
     return _LIB
 
@@ -264,3 +284,46 @@ class MsaSession:
 
     def __exit__(self, *exc):
         self.close()
+
+
+
+# --------------------------------------------------------------------------- block evictor (include/msa_evictor.h)
+class MsaEvictor:
+    """ctypes view of the C++ evictor (Algorithm 1): argument marshalling only."""
+
+    def __init__(self, alpha: float, beta: float, tau0: float, k5: float, c0: float, lambda_: float = 1.0):
+        cfg = MsaEvictorConfig(alpha, beta, tau0, lambda_, k5, c0)
+        self._h = ctypes.c_void_p()
+        _check(_lib().msa_evictor_create(ctypes.byref(cfg), ctypes.byref(self._h)), "msa_evictor_create")
+
+    def add(self, block_id: int, position: int, last_access: float) -> None:
+        _check(_lib().msa_evictor_add(self._h, block_id, position, last_access), "msa_evictor_add")
+
+    def remove(self, block_id: int) -> None:
+        _check(_lib().msa_evictor_remove(self._h, block_id), "msa_evictor_remove")
+
+    def evict(self, t_now: float, linear: bool = False) -> int:
+        out = ctypes.c_int64(0)
+        fn = _lib().msa_evictor_evict_linear if linear else _lib().msa_evictor_evict
+        _check(fn(self._h, t_now, ctypes.byref(out)), "msa_evictor_evict")
+        return int(out.value)
+
+    def set_lambda(self, lambda_: float) -> None:
+        _check(_lib().msa_evictor_set_lambda(self._h, lambda_), "msa_evictor_set_lambda")
+
+    def weight(self, block_id: int, t_now: float) -> float:
+        return float(_lib().msa_evictor_weight(self._h, block_id, t_now))
+
+    def __len__(self) -> int:
+        return int(_lib().msa_evictor_size(self._h))
+
+    def close(self) -> None:
+        if self._h:
+            _lib().msa_evictor_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

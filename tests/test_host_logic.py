@@ -27,6 +27,11 @@ def test_library_exports_every_declared_symbol():
     for name in sorted(declared):
         assert hasattr(lib, name), f"{name} declared in msa.h but not exported"
     assert set(binding.EXPORTS) == declared
+    hdr2 = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "msa_evictor.h")).read(), flags=re.S)
+    declared2 = set(re.findall(r"\b(msa_evictor_[a-z_]+)\s*\(", hdr2))
+    for name in sorted(declared2):
+        assert hasattr(lib, name), f"{name} declared in msa_evictor.h but not exported"
+    assert set(binding.EVICTOR_EXPORTS) == declared2
 
 
 def test_create_rejects_unsupported_shapes_and_reports_no_device():
