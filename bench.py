@@ -159,6 +159,13 @@ def whole_job_value(world: int, units_per_step: float, ms: float) -> float:
     return world * units_per_step / (ms * 1e-3)
 
 
+def all_workloads():
+    """BASELINE.json's configs, the extra rows of SURVEY.md 8(f), and the batch whose residency the evictor decides."""
+    import workloads as W
+    from paper_2606_02964_b200.policy_trace import f3_policy_trace
+    return {**W.CONFIGS, **W.EXTRA_CONFIGS, "f3_policy_trace": f3_policy_trace}
+
+
 def metric_of(workload: str):
     if workload == "cfg5_short_query":
         return "msa_short_query_hbm_gbs", "GB/s", "hbm"
@@ -183,7 +190,7 @@ def run_mine(args, rank: int, world: int, local_rank: int):
 
     def bench_workload(name: str, steps: int, warmup: int, do_e2e: bool):
         metric, unit, bound = metric_of(name)
-        p = {**W.CONFIGS, **W.EXTRA_CONFIGS}[name](device=dev)
+        p = all_workloads()[name](device=dev)
         alg = p.algorithmic()
         units_per_step = alg["flops"] / 1e12 if bound == "tensor" else alg["bytes"] / 1e9
         s = MsaSession(p, device=local_rank)
@@ -402,6 +409,59 @@ def run_evictor(args):
                           gpu_launches=0)))
 
 
+def run_costmodel(args):
+    """refit the attention part of the paper's latency model from measured msa_forward times.
+    Layout of Eq. (4): [cached l1][compute q1][cached l2][compute q2], one request, Llama-3-8B heads.
+    Eq. (4): T = k1 l1 + k2 q1 + k3 l2 + k4 q2 + k5 q1 (l1+q1) + k6 q2 (l1+q1+l2+q2) + b;  Eq. (6) replaces the k5 term by
+    k5 (l1+q1)^2 so that dT_B = 2 k5 pos + const (Eq. (7)).  Least squares over the grid, R^2 of both forms."""
+    import torch
+    import workloads as W
+    from paper_2606_02964_b200 import MsaSession, msa_get_timing, msa_set_timing
+    import __graft_entry__ as ge
+    ge.build()
+    dev = "cuda:0"
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream().cuda_stream
+    grid = [(l1, q1, l2, q2) for l1 in (1024, 4096, 8192, 16384) for q1 in (256, 1024, 2048)
+            for l2 in (1024, 4096, 8192) for q2 in (256, 1024, 2048)]
+    X4, X6, y = [], [], []
+    for (l1, q1, l2, q2) in grid:
+        ctx = W.ContextSpec([(W.SEG_PAGED, 0, l1), (W.SEG_SELF, l1, q1), (W.SEG_PAGED, l1 + q1, l2), (W.SEG_SELF, l1 + q1 + l2, q2)])
+        p = W.build_problem("costmodel", 32, 8, 128, [ctx], [W.RunSpec(0, l1, q1), W.RunSpec(0, l1 + q1 + l2, q2)],
+                            seed=77, device=dev)
+        with MsaSession(p) as sess:
+            for _ in range(3):
+                sess.forward(stream)
+            msa_set_timing(sess.h, 10)
+            for _ in range(10):
+                sess.forward(stream)
+            torch.cuda.synchronize()
+            _, fwd_ms, merge_ms = msa_get_timing(sess.h)
+        lin = [l1, q1, l2, q2]
+        X4.append(lin + [q1 * (l1 + q1), q2 * (l1 + q1 + l2 + q2), 1.0])
+        X6.append(lin + [(l1 + q1) ** 2, q2 * (l1 + q1 + l2 + q2), 1.0])
+        y.append((fwd_ms + merge_ms) * 1e-3)
+        del p
+    y = np.asarray(y)
+
+    def fit(X):
+        X = np.asarray(X, np.float64)
+        k, *_ = np.linalg.lstsq(X, y, rcond=None)
+        r = y - X @ k
+        return k, 1.0 - float(r @ r) / float(((y - y.mean()) ** 2).sum())
+
+    k4, r2_4 = fit(X4)
+    k6, r2_6 = fit(X6)
+    names = ["k1", "k2", "k3", "k4", "k5", "k6", "beta"]
+    print(json.dumps(dict(metric="msa_costmodel_r2_eq4", value=r2_4, unit="R^2", n_gpus=1, steps=10, warmup=3, higher_is_better=True,
+                          dtype="bf16", data="synthetic", vs_baseline=None,
+                          config=dict(workload="costmodel", points=len(grid), seconds_min=float(y.min()), seconds_max=float(y.max())),
+                          eq4=dict(r2=r2_4, coeff=dict(zip(names, map(float, k4)))),
+                          eq6=dict(r2=r2_6, coeff=dict(zip(names, map(float, k6))),
+                                   evictor_k5=float(k6[4]), evictor_c0=float(k6[1] - k6[2] + k6[4])),
+                          gpu_launches=len(grid) * 26)))
+
+
 def run_reference(args, rank: int, world: int):
     """The reference arm of this tier = the fp64 CPU oracle on the box's host cores (rank 0 only)."""
     if rank != 0:
@@ -415,8 +475,8 @@ def run_reference(args, rank: int, world: int):
     if p is None:
         # values on the CPU; only the requests sampled are ever read
         small = dict(cfg2_llama8b=dict(n_req=2), cfg4_mixed=dict(n_req=4), cfg5_short_query=dict(n_req=8),
-                     f1_hybrid_pod=dict(n_prefill=1, n_decode=2))
-        p = {**W.CONFIGS, **W.EXTRA_CONFIGS}[args.workload](device="cpu", **small.get(args.workload, {}))
+                     f1_hybrid_pod=dict(n_prefill=1, n_decode=2), f3_policy_trace=dict(n_sessions=3))
+        p = all_workloads()[args.workload](device="cpu", **small.get(args.workload, {}))
     reqs = list(range(min(2, p.n_req)))
     dt, fl, pairs, n = oracle_sample(p, 8, 1, reqs)
     total = max(1, args.steps + args.warmup)
@@ -448,7 +508,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="mine", choices=["mine", "reference"])
     ap.add_argument("--workload", default="cfg2_llama8b",
-                    choices=["cfg2_llama8b", "cfg3_70b_long", "cfg4_mixed", "cfg5_short_query", "f1_hybrid_pod", "fig13", "evictor"])
+                    choices=["cfg2_llama8b", "cfg3_70b_long", "cfg4_mixed", "cfg5_short_query", "f1_hybrid_pod", "f3_policy_trace",
+                             "fig13", "evictor", "costmodel"])
     ap.add_argument("--no-secondary", action="store_true")
     args = ap.parse_args()
     rank, world, local_rank = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
@@ -460,6 +521,9 @@ def main():
     elif args.workload == "evictor":
         if rank == 0:
             run_evictor(args)
+    elif args.workload == "costmodel":
+        if rank == 0:
+            run_costmodel(args)
     else:
         run_mine(args, rank, world, local_rank)
 

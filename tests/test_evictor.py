@@ -120,3 +120,23 @@ def test_cpp_evictor_error_codes():
     assert e.value.status == MSA_ERR_INVALID_ARG
     assert math.isnan(ev.weight(12345, 0.0))
     assert ev.evict(5.0) == 7 and len(ev) == 0
+
+
+def test_policy_trace_shows_the_two_ended_residency_of_observation_2():
+    """under pressure the shared prefix and the suffixes survive, the middle of a sequence goes."""
+    from paper_2606_02964_b200.policy_trace import f3_policy_trace, policy_residency
+    sessions, summary = policy_residency()
+    assert summary["kept_fraction"] == pytest.approx(0.6, abs=1e-3)
+    three = 0
+    for x in sessions:
+        r = x["resident"]
+        assert r[: 512 // 16].all()                                   # the shared prefix is never the victim
+        flips = int(np.count_nonzero(r[1:] != r[:-1]))
+        assert flips <= 2                                              # at most prefix | evicted middle | suffix
+        if flips == 2:
+            three += 1
+            first_gone = int(np.argmin(r))
+            assert r[np.argmax(~r[first_gone:] == False) + first_gone:].all()
+    assert three >= 8
+    p = f3_policy_trace(layout_only=True)
+    assert p.n_req == 48 and p.policy_summary["segments_per_request_max"] == 3

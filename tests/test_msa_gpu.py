@@ -206,7 +206,8 @@ def test_forward_host_matches_forward_and_error_codes():
 
 # ------------------------------------------------------------------ configs 2-5 at full size (sampled rows)
 def _full_config(name, n_req_sample, n_random, seed):
-    p = {**W.CONFIGS, **W.EXTRA_CONFIGS}[name](device=DEV)
+    from paper_2606_02964_b200.policy_trace import f3_policy_trace
+    p = {**W.CONFIGS, **W.EXTRA_CONFIGS, "f3_policy_trace": f3_policy_trace}[name](device=DEV)
     o, lse, info = gpu_forward(p)
     rng = np.random.default_rng(seed)
     reqs = sorted(int(x) for x in rng.choice(p.n_req, size=min(n_req_sample, p.n_req), replace=False))
@@ -235,3 +236,8 @@ def test_cfg5_short_query_full_size_sampled_rows():
 def test_f1_hybrid_prefill_plus_decode_full_size_sampled_rows():
     """Hybrid chunks (compute -> cached -> compute sharing one segment list) and 128 decode rows in ONE launch."""
     _full_config("f1_hybrid_pod", 40, 2, 6)
+
+
+def test_f3_policy_trace_full_size_sampled_rows():
+    """Residency decided by the evictor (Algorithm 1): shared prefix and suffix cached, middle recomputed."""
+    _full_config("f3_policy_trace", 10, 4, 7)
