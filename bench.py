@@ -462,6 +462,60 @@ def run_costmodel(args):
                           gpu_launches=len(grid) * 26)))
 
 
+def run_kv_append(args):
+    """write the recomputed and own K/V of the cfg2 batch (every CONTIG / SELF segment) into
+    fresh paged blocks.  HBM-bound copy: algorithmic bytes = 2 (read + write) x tokens x Hkv x D x 2 B x 2 (K, V)."""
+    import torch
+    import workloads as W
+    from paper_2606_02964_b200 import msa_append_plan_create, msa_append_plan_destroy, msa_create, msa_destroy, msa_kv_append
+    import __graft_entry__ as ge
+    ge.build()
+    dev = "cuda:0"
+    torch.cuda.set_device(0)
+    _, gbs_peak, peak_label = measured_peaks()
+    p = W.cfg2_llama8b(device=dev)
+    jobs, cursor, tokens = [], int(p.block_table.numel()), 0
+    for sidx in range(len(p.seg_kind)):
+        if int(p.seg_kind[sidx]) != W.SEG_PAGED:
+            n = int(p.seg_len[sidx])
+            jobs.append((int(p.seg_row_off[sidx]), n, cursor))
+            cursor += (n + 15) // 16
+            tokens += n
+    extra = cursor - int(p.block_table.numel())
+    n_pool = int(p.pool_k.shape[0])
+    perm = torch.randperm(extra, generator=torch.Generator().manual_seed(9)).to(torch.int32) + n_pool
+    bt = torch.cat([p.block_table, perm.to(dev)]).contiguous()
+    pool_k = torch.cat([p.pool_k, torch.zeros((extra,) + tuple(p.pool_k.shape[1:]), dtype=torch.bfloat16, device=dev)]).contiguous()
+    pool_v = torch.cat([p.pool_v, torch.zeros((extra,) + tuple(p.pool_v.shape[1:]), dtype=torch.bfloat16, device=dev)]).contiguous()
+    h = msa_create(p.Hq, p.Hkv, p.D, p.q_to_kv, device=0)
+    ap = msa_append_plan_create(h, jobs)
+    stream = torch.cuda.current_stream().cuda_stream
+    for _ in range(max(3, args.warmup)):
+        msa_kv_append(h, ap, p.contig_k, p.contig_v, pool_k, pool_v, bt, stream)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.start()
+    e0.record()
+    for _ in range(args.steps):
+        msa_kv_append(h, ap, p.contig_k, p.contig_v, pool_k, pool_v, bt, stream)
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1) / args.steps
+    nbytes = 2.0 * tokens * p.Hkv * p.D * 2 * 2
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    msa_append_plan_destroy(ap)
+    msa_destroy(h)
+    print(json.dumps(dict(metric="msa_kv_append_hbm_gbs", value=gbs, unit="GB/s", n_gpus=1, steps=args.steps, warmup=max(3, args.warmup),
+                          ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="bf16", data="synthetic",
+                          config=dict(workload="kv_append", tokens=tokens, jobs=len(jobs), bytes_per_step=nbytes,
+                                      l2_policy="working set %.0f MB per step (read + write), larger than L2" % (nbytes / 1e6)),
+                          clocks=clocks, gpu_launches=args.steps,
+                          roofline=dict(bound="hbm", achieved=gbs, peak=gbs_peak, unit="GB/s", frac=gbs / gbs_peak, traffic=None,
+                                        kernel="msa_kv_append", kernel_ms=ms, peak_source=peak_label))))
+
+
 def run_reference(args, rank: int, world: int):
     """The reference arm of this tier = the fp64 CPU oracle on the box's host cores (rank 0 only)."""
     if rank != 0:
@@ -509,7 +563,7 @@ def main():
     ap.add_argument("--impl", default="mine", choices=["mine", "reference"])
     ap.add_argument("--workload", default="cfg2_llama8b",
                     choices=["cfg2_llama8b", "cfg3_70b_long", "cfg4_mixed", "cfg5_short_query", "f1_hybrid_pod", "f3_policy_trace",
-                             "fig13", "evictor", "costmodel"])
+                             "fig13", "evictor", "costmodel", "kv_append"])
     ap.add_argument("--no-secondary", action="store_true")
     args = ap.parse_args()
     rank, world, local_rank = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
@@ -524,6 +578,9 @@ def main():
     elif args.workload == "costmodel":
         if rank == 0:
             run_costmodel(args)
+    elif args.workload == "kv_append":
+        if rank == 0:
+            run_kv_append(args)
     else:
         run_mine(args, rank, world, local_rank)
 

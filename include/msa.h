@@ -182,6 +182,33 @@ int msa_forward_host(msa_handle h, msa_plan p,
                      float softmax_scale,
                      void *o_host, float *lse_host, void *cuda_stream);
 
+/* ---- KV write-back (PAPER.md:92 step 2: recomputed K/V are written into cache blocks) ----
+ * After a step, the K/V rows a request has just (re)computed -- CONTIG and SELF segments of the arena -- are appended
+ * to the paged cache so that the next step can reach them as PAGED segments.  One job copies arena rows
+ * [row_off, row_off + len) into the blocks block_table[block_off + i/16], slot i%16 (the same addressing a PAGED
+ * segment uses: the job starts at slot 0 of its first block; a partly filled last block leaves its tail untouched). */
+typedef struct {
+    int64_t row_off;               /* first arena row                                        */
+    int32_t len;                   /* tokens, >= 1                                           */
+    int32_t block_off;             /* index into block_table of the first destination block  */
+} msa_append;
+
+typedef struct msa_append_plan_s *msa_append_plan;
+
+/* Validates the jobs (host array, copied) and uploads the 16-token copy units.  MSA_ERR_INVALID_ARG for a bad job,
+ * MSA_ERR_OVERLAP if two jobs write the same block-table entry.  n_jobs = 0 is legal (msa_kv_append launches nothing). */
+int msa_append_plan_create(msa_handle h, const msa_append *jobs, int32_t n_jobs, msa_append_plan *out);
+void msa_append_plan_destroy(msa_append_plan ap);
+
+/* Asynchronous on `cuda_stream`, one kernel launch; never allocates or synchronises.  contig_* / pool_* / block_table as
+ * in msa_forward, except that the pool is written.  The destination blocks must not be read by a kernel running
+ * concurrently on another stream.  MSA_ERR_OUT_OF_RANGE if a job exceeds contig_rows or block_table_len (block ids
+ * themselves are trusted, they live on the device); MSA_ERR_MISALIGNED for pointers not 16-byte aligned. */
+int msa_kv_append(msa_handle h, msa_append_plan ap,
+                  const void *contig_k, const void *contig_v, int64_t contig_rows,
+                  void *pool_k, void *pool_v, int64_t num_blocks,
+                  const int32_t *block_table, int64_t block_table_len, void *cuda_stream);
+
 /* Number of kernels the last msa_forward / msa_forward_host on this handle launched. */
 int msa_last_launch_count(msa_handle h);
 

@@ -57,9 +57,14 @@ _LIB: Optional[ctypes.CDLL] = None
 
 EXPORTS = ["msa_create", "msa_destroy", "msa_plan_create", "msa_plan_destroy", "msa_plan_get_info",
            "msa_plan_export", "msa_workspace_bytes", "msa_forward", "msa_forward_host",
-           "msa_last_launch_count", "msa_set_timing", "msa_get_timing", "msa_strerror", "msa_last_cuda_error", "msa_version"]
+           "msa_last_launch_count", "msa_set_timing", "msa_get_timing", "msa_strerror", "msa_last_cuda_error", "msa_version",
+           "msa_append_plan_create", "msa_append_plan_destroy", "msa_kv_append"]
 EVICTOR_EXPORTS = ["msa_evictor_create", "msa_evictor_destroy", "msa_evictor_add", "msa_evictor_remove", "msa_evictor_evict",
                    "msa_evictor_evict_linear", "msa_evictor_set_lambda", "msa_evictor_size", "msa_evictor_weight"]
+
+
+class MsaAppend(ctypes.Structure):
+    _fields_ = [("row_off", ctypes.c_int64), ("len", ctypes.c_int32), ("block_off", ctypes.c_int32)]
 
 
 class MsaEvictorConfig(ctypes.Structure):
@@ -94,6 +99,10 @@ def _lib() -> ctypes.CDLL:
         for f in ("msa_strerror", "msa_last_cuda_error", "msa_version"):
             getattr(lib, f).restype = ctypes.c_char_p
         lib.msa_strerror.argtypes = [ctypes.c_int]
+        lib.msa_append_plan_create.argtypes = [vp, ctypes.POINTER(MsaAppend), i32, ctypes.POINTER(vp)]
+        lib.msa_append_plan_destroy.argtypes = [vp]
+        lib.msa_append_plan_destroy.restype = None
+        lib.msa_kv_append.argtypes = [vp, vp, vp, vp, i64, vp, vp, i64, vp, i64, vp]
         f64 = ctypes.c_double
         lib.msa_evictor_create.argtypes = [ctypes.POINTER(MsaEvictorConfig), ctypes.POINTER(vp)]
         lib.msa_evictor_destroy.argtypes = [vp]
@@ -285,6 +294,31 @@ class MsaSession:
     def __exit__(self, *exc):
         self.close()
 
+
+
+# --------------------------------------------------------------------------- KV write-back
+def msa_append_plan_create(h, jobs):
+    """jobs: iterable of (row_off, len, block_off)."""
+    jobs = list(jobs)
+    arr = (MsaAppend * max(1, len(jobs)))()
+    for i, (row_off, n, block_off) in enumerate(jobs):
+        arr[i] = MsaAppend(int(row_off), int(n), int(block_off))
+    ap = ctypes.c_void_p()
+    _check(_lib().msa_append_plan_create(h, arr, len(jobs), ctypes.byref(ap)), "msa_append_plan_create")
+    return ap
+
+
+def msa_append_plan_destroy(ap) -> None:
+    _lib().msa_append_plan_destroy(ap)
+
+
+def msa_kv_append(h, ap, contig_k, contig_v, pool_k, pool_v, block_table, stream: Optional[int] = None) -> None:
+    """Arena rows -> paged cache blocks (bf16 CUDA tensors; block_table int32 CUDA); asynchronous on `stream`."""
+    rows = 0 if contig_k is None else int(contig_k.shape[0])
+    nb = 0 if pool_k is None else int(pool_k.shape[0])
+    bt_len = 0 if block_table is None else int(block_table.numel())
+    _check(_lib().msa_kv_append(h, ap, _dptr(contig_k), _dptr(contig_v), rows, _dptr(pool_k), _dptr(pool_v), nb,
+                                _dptr(block_table), bt_len, stream), "msa_kv_append")
 
 
 # --------------------------------------------------------------------------- block evictor (include/msa_evictor.h)

@@ -1,5 +1,6 @@
 // C ABI of libmsa (include/msa.h): handle, plan upload, tensor-map encoding and launches.
 #include <cuda.h>
+#include <limits.h>
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
@@ -88,6 +89,14 @@ struct msa_plan_s {
     const int32_t *d_cta_begin = nullptr;
     const MergeItem *d_merge = nullptr;
     const TileInfo *d_tile_info = nullptr;
+};
+
+struct msa_append_plan_s {
+    msa_handle h = nullptr;
+    std::vector<AppendUnit> units;
+    AppendUnit *d_units = nullptr;
+    int64_t max_row = -1;          // extents the jobs need at msa_kv_append
+    int64_t max_bt = -1;
 };
 
 extern "C" {
@@ -471,6 +480,92 @@ int msa_forward_host(msa_handle h, msa_plan p, const void *q_host, int64_t total
         MSA_CUDA(cudaMemcpyAsync(lse_host, h->s_lse.p, b_lse, cudaMemcpyDeviceToHost, stream));
     }
     MSA_CUDA(cudaStreamSynchronize(stream));
+    return MSA_OK;
+}
+
+int msa_append_plan_create(msa_handle h, const msa_append *jobs, int32_t n_jobs, msa_append_plan *out)
+{
+    if (!h || !out || n_jobs < 0 || (n_jobs > 0 && !jobs)) return MSA_ERR_INVALID_ARG;
+    *out = nullptr;
+    msa_append_plan ap = new (std::nothrow) msa_append_plan_s();
+    if (!ap) return MSA_ERR_INVALID_ARG;
+    ap->h = h;
+    std::vector<std::pair<int64_t, int64_t>> spans;      // destination block-table ranges, for the overlap check
+    for (int32_t j = 0; j < n_jobs; ++j) {
+        const msa_append &a = jobs[j];
+        if (a.len < 1 || a.row_off < 0 || a.block_off < 0) {
+            delete ap;
+            return MSA_ERR_INVALID_ARG;
+        }
+        const int nblk = (a.len + kBlock - 1) / kBlock;
+        const int64_t last_bt = static_cast<int64_t>(a.block_off) + nblk - 1;
+        if (last_bt > INT32_MAX || a.row_off + a.len - 1 > INT32_MAX) {
+            delete ap;
+            return MSA_ERR_OUT_OF_RANGE;
+        }
+        spans.emplace_back(a.block_off, last_bt + 1);
+        ap->max_bt = std::max(ap->max_bt, last_bt);
+        ap->max_row = std::max(ap->max_row, a.row_off + a.len - 1);
+        for (int b = 0; b < nblk; ++b) {
+            AppendUnit u;
+            u.src_row = a.row_off + static_cast<int64_t>(b) * kBlock;
+            u.bt_index = a.block_off + b;
+            u.nvalid = std::min(kBlock, a.len - b * kBlock);
+            ap->units.push_back(u);
+        }
+    }
+    std::sort(spans.begin(), spans.end());
+    for (size_t i = 1; i < spans.size(); ++i)
+        if (spans[i].first < spans[i - 1].second) {
+            delete ap;
+            return MSA_ERR_OVERLAP;
+        }
+    if (!h->planning_only && !ap->units.empty()) {
+        cudaError_t e = cudaSetDevice(h->cfg.device);
+        if (e == cudaSuccess) e = cudaMalloc(&ap->d_units, ap->units.size() * sizeof(AppendUnit));
+        if (e == cudaSuccess)
+            e = cudaMemcpy(ap->d_units, ap->units.data(), ap->units.size() * sizeof(AppendUnit), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) {
+            if (ap->d_units) cudaFree(ap->d_units);
+            delete ap;
+            return cuda_fail(e, "msa_append_plan_create: upload");
+        }
+    }
+    *out = ap;
+    return MSA_OK;
+}
+
+void msa_append_plan_destroy(msa_append_plan ap)
+{
+    if (!ap) return;
+    if (ap->d_units) cudaFree(ap->d_units);
+    delete ap;
+}
+
+int msa_kv_append(msa_handle h, msa_append_plan ap, const void *contig_k, const void *contig_v, int64_t contig_rows,
+                  void *pool_k, void *pool_v, int64_t num_blocks, const int32_t *block_table, int64_t block_table_len,
+                  void *cuda_stream)
+{
+    if (!h || !ap || ap->h != h) return MSA_ERR_INVALID_ARG;
+    if (h->planning_only) return MSA_ERR_NO_DEVICE;
+    h->last_launches = 0;
+    if (ap->units.empty()) return MSA_OK;
+    if (!contig_k || !contig_v || !pool_k || !pool_v || !block_table || num_blocks < 1) return MSA_ERR_INVALID_ARG;
+    if (ap->max_row >= contig_rows || ap->max_bt >= block_table_len) return MSA_ERR_OUT_OF_RANGE;
+    if (!aligned16(contig_k) || !aligned16(contig_v) || !aligned16(pool_k) || !aligned16(pool_v) ||
+        (reinterpret_cast<uintptr_t>(block_table) & 3u))
+        return MSA_ERR_MISALIGNED;
+    AppendParams ap_params;
+    ap_params.units = ap->d_units;
+    ap_params.block_table = block_table;
+    ap_params.contig_k = contig_k;
+    ap_params.contig_v = contig_v;
+    ap_params.pool_k = pool_k;
+    ap_params.pool_v = pool_v;
+    ap_params.row_bytes = static_cast<int64_t>(h->cfg.num_kv_heads) * h->cfg.head_dim * 2;
+    ap_params.n_units = static_cast<int32_t>(ap->units.size());
+    MSA_CUDA(launch_append(ap_params, h->num_sms, static_cast<cudaStream_t>(cuda_stream)));
+    h->last_launches = 1;
     return MSA_OK;
 }
 

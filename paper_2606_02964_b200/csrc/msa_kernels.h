@@ -39,6 +39,24 @@ struct MergeParams {
     int32_t Hq, G, D;
 };
 
+// KV write-back: one unit = up to 16 tokens of one job
+struct AppendUnit {
+    int64_t src_row;       // first arena row
+    int32_t bt_index;      // index into block_table of the destination block
+    int32_t nvalid;        // tokens to copy, 1..16 (slots 0..nvalid-1 of the block)
+};
+
+struct AppendParams {
+    const AppendUnit *units;
+    const int32_t *block_table;
+    const void *contig_k, *contig_v;
+    void *pool_k, *pool_v;
+    int64_t row_bytes;     // Hkv * D * 2
+    int32_t n_units;
+};
+
+cudaError_t launch_append(const AppendParams &p, int num_sms, cudaStream_t stream);
+
 // kernel variants (debug env MSA_KERNEL selects; default = the fastest validated one)
 enum class FwdVariant : int { Simple = 0, Pipelined = 1 };
 

@@ -1,0 +1,111 @@
+"""KV write-back (include/msa.h msa_kv_append): oracle pin, host validation, GPU parity (bit-exact)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import workloads as W
+from oracle.append_oracle import kv_append
+from paper_2606_02964_b200 import (MsaError, MSA_ERR_INVALID_ARG, MSA_ERR_OUT_OF_RANGE, MSA_ERR_OVERLAP, MsaSession,
+                                   make_descriptors, msa_append_plan_create, msa_append_plan_destroy, msa_create,
+                                   msa_destroy, msa_forward, msa_kv_append, msa_plan_create, msa_plan_destroy,
+                                   msa_workspace_bytes)
+from workloads import SEG_PAGED
+
+NAN16 = np.uint16(0x7FC0)          # bf16 NaN: whatever is not written must stay exactly this
+
+
+def _jobs_and_redescription(p):
+    """Every CONTIG / SELF segment gets fresh blocks behind the existing block table; returns
+    (jobs, extended block table, extra blocks, seg_kind', seg_block_off')."""
+    bt = p.block_table_np
+    n_pool = int(p.pool_k.shape[0])
+    jobs, kind2, boff2 = [], p.seg_kind.copy(), p.seg_block_off.copy()
+    cursor = len(bt)
+    for s in range(len(p.seg_kind)):
+        if int(p.seg_kind[s]) != SEG_PAGED:
+            n = int(p.seg_len[s])
+            jobs.append((int(p.seg_row_off[s]), n, cursor))
+            kind2[s], boff2[s] = SEG_PAGED, cursor
+            cursor += (n + 15) // 16
+    extra = cursor - len(bt)
+    rng = np.random.default_rng(5)
+    new_ids = n_pool + rng.permutation(extra)                        # shuffled fresh blocks
+    return jobs, np.concatenate([bt, new_ids.astype(np.int32)]), extra, kind2, boff2
+
+
+def test_oracle_append_then_paged_description_equals_contig_description():
+    p = W.random_problem(301, n_req=3, Hq=4, Hkv=2, D=64, max_ctx=300, max_q=40, hybrid=True)
+    a = p.host_arrays()
+    jobs, bt2, extra, kind2, boff2 = _jobs_and_redescription(p)
+    assert jobs
+    a2 = dict(a)
+    for name, arena in (("pool_k", a["contig_k"]), ("pool_v", a["contig_v"])):
+        ext = np.concatenate([a[name], np.full((extra,) + a[name].shape[1:], NAN16, np.uint16)])
+        a2[name] = kv_append(ext, arena, bt2, jobs)
+    a2.update(block_table=bt2, seg_kind=kind2, seg_block_off=boff2)
+    rr = np.concatenate([np.full(int(p.req[r, 1]), r, np.int32) for r in range(p.n_req)])
+    ii = np.concatenate([np.arange(int(p.req[r, 1]), dtype=np.int32) for r in range(p.n_req)])
+    O1, L1 = oracle.forward(a, p.Hq, p.Hkv, p.D, p.scale, rr, ii)
+    O2, L2 = oracle.forward(a2, p.Hq, p.Hkv, p.D, p.scale, rr, ii)
+    assert np.array_equal(O1, O2) and np.array_equal(L1, L2)
+    # a ragged job leaves the tail of its last block alone
+    n_tail = sum(1 for (_, n, _) in jobs if n % 16)
+    assert n_tail > 0 and (a2["pool_k"] == NAN16).any()
+
+
+def test_append_plan_validation():
+    h = msa_create(4, 2, 64, device=-1)
+    msa_append_plan_destroy(msa_append_plan_create(h, [(0, 40, 0), (40, 16, 3)]))
+    msa_append_plan_destroy(msa_append_plan_create(h, []))
+    for jobs, code in [([(0, 40, 0), (40, 16, 2)], MSA_ERR_OVERLAP),          # 40 tokens take blocks 0..2
+                       ([(0, 0, 0)], MSA_ERR_INVALID_ARG), ([(-1, 4, 0)], MSA_ERR_INVALID_ARG),
+                       ([(0, 4, -1)], MSA_ERR_INVALID_ARG)]:
+        with pytest.raises(MsaError) as e:
+            msa_append_plan_create(h, jobs)
+        assert e.value.status == code, jobs
+    msa_destroy(h)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("seed,kw", [(311, dict(Hq=8, Hkv=2, D=128, max_ctx=900, max_q=150)),
+                                     (312, dict(Hq=4, Hkv=4, D=64, max_ctx=300, max_q=33, hybrid=True, n_req=5))])
+def test_kv_append_matches_the_oracle_bit_for_bit_and_forward_sees_the_same_values(seed, kw):
+    dev = "cuda:0"
+    p = W.random_problem(seed, device=dev, fill="nan", **kw)
+    jobs, bt2, extra, kind2, boff2 = _jobs_and_redescription(p)
+    a = p.host_arrays()
+
+    def ext(t):
+        pad = torch.full((extra,) + tuple(t.shape[1:]), float("nan"), dtype=torch.bfloat16, device=dev)
+        return torch.cat([t, pad]).contiguous()
+
+    pool_k, pool_v = ext(p.pool_k), ext(p.pool_v)
+    bt_dev = torch.from_numpy(bt2).to(dev)
+    u16 = lambda t: t.cpu().view(torch.int16).numpy().view(np.uint16)
+    want_k = kv_append(u16(pool_k), a["contig_k"], bt2, jobs)
+    want_v = kv_append(u16(pool_v), a["contig_v"], bt2, jobs)
+    h = msa_create(p.Hq, p.Hkv, p.D, p.q_to_kv)
+    ap = msa_append_plan_create(h, jobs)
+    msa_kv_append(h, ap, p.contig_k, p.contig_v, pool_k, pool_v, bt_dev, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert np.array_equal(u16(pool_k), want_k) and np.array_equal(u16(pool_v), want_v)
+    with pytest.raises(MsaError) as e:
+        msa_kv_append(h, ap, p.contig_k[:3], p.contig_v, pool_k, pool_v, bt_dev)
+    assert e.value.status == MSA_ERR_OUT_OF_RANGE
+    # the forward pass over the written blocks (PAGED description) equals the one over the arena rows
+    with MsaSession(p) as s:
+        o1, l1 = s.forward()
+        o1, l1 = o1.clone(), l1.clone()
+    R, n, S, m = make_descriptors(p.req, kind2, p.seg_abs_start, p.seg_len, boff2, p.seg_row_off)
+    plan = msa_plan_create(h, R, n, S, m)
+    nb = msa_workspace_bytes(plan)
+    ws = torch.empty(max(nb, 16), dtype=torch.uint8, device=dev) if nb else None
+    o2 = torch.zeros_like(p.q)
+    l2 = torch.zeros(p.total_q, p.Hq, dtype=torch.float32, device=dev)
+    msa_forward(h, plan, p.q, pool_k, pool_v, bt_dev, p.contig_k, p.contig_v, p.scale, o2, l2, ws)
+    torch.cuda.synchronize()
+    assert torch.equal(o1, o2) and torch.equal(l1, l2)
+    msa_plan_destroy(plan)
+    msa_append_plan_destroy(ap)
+    msa_destroy(h)
