@@ -162,7 +162,7 @@ def whole_job_value(world: int, units_per_step: float, ms: float) -> float:
 def all_workloads():
     """BASELINE.json's configs, the extra rows of SURVEY.md 8(f), and the batch whose residency the evictor decides."""
     import workloads as W
-    from paper_2606_02964_b200.policy_trace import f3_policy_trace
+    from workloads.policy_trace import f3_policy_trace
     return {**W.CONFIGS, **W.EXTRA_CONFIGS, "f3_policy_trace": f3_policy_trace}
 
 

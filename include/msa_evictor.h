@@ -1,16 +1,16 @@
 /* msa_evictor.h -- C ABI of the computational-aware block evictor (host side, no GPU involved).
  *
  * SURVEY.md section 8 (f3).  The paper's Algorithm 1: every evictable KV-cache block B
- * carries the weight  f_B(t) * dT_B  (Eq. (3), PAPER.md:136-142) and the block with the smallest weight is
+ * carries the weight  f_B(t) * dT_B  (Eq. (3), PAPER.md:135-136) and the block with the smallest weight is
  * evicted, where
- *   dT_B   = 2*k5*pos_B + c0                 recomputation cost, Eq. (7) (PAPER.md:165-167); pos_B = number of
+ *   dT_B   = 2*k5*pos_B + c0                 recomputation cost, Eq. (7) (PAPER.md:173); pos_B = number of
  *                                            tokens in front of the block in its sequence ("l1 + q1")
- *   f_B(t) = min( exp(-tau/alpha), exp(-(tau - tau0)/beta) ),  tau = t - (last access of B)      Eq. (9)
+ *   f_B(t) = min( exp(-tau/alpha), exp(-(tau - tau0)/beta) ),  tau = t - (last access of B)      Eq. (9) (PAPER.md:202)
  * Each branch of f is a single exponential, so the ORDER of the branch weights of two blocks never changes
- * with t (order-preserving rule, Eq. (8)); the evictor keeps one ordered set per branch, keyed by the
+ * with t (order-preserving rule, Eq. (8), PAPER.md:183-184); the evictor keeps one ordered set per branch, keyed by the
  * time-independent part of the log weight, and all three operations are O(log n):
  *   log w1 = -t/alpha + [ last/alpha          + ln dT ]      log w2 = -t/beta + [ (last + tau0)/beta + ln dT ]
- * Evict takes the minimum of each set and returns argmin{ w1(B1), lambda * w2(B2) } (Algorithm 1, line 8).
+ * Evict takes the minimum of each set and returns argmin{ w1(B1), lambda * w2(B2) } (Algorithm 1, line 8, PAPER.md:222).
  *
  * All functions are host-only and thread-compatible (one evictor per thread, or external locking).
  * Return value: MSA_OK (0) or a negative MSA_ERR_* code from msa.h.
@@ -55,7 +55,8 @@ int msa_evictor_evict(msa_evictor ev, double t_now, int64_t *block_id);
  * PAPER.md:235); kept for the measurement and as a cross-check.  Removes the block it returns. */
 int msa_evictor_evict_linear(msa_evictor ev, double t_now, int64_t *block_id);
 
-/* Online adjustment of lambda. */
+/* Online adjustment of lambda: lambda = exp((tau - tau0)/beta - tau/alpha), Eq. (10), moves the
+ * effective turning point of Eq. (9) to the observed lifespan tau; takes effect at the next evict, O(1). */
 int msa_evictor_set_lambda(msa_evictor ev, double lambda);
 
 /* Number of evictable blocks held. */

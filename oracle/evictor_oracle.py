@@ -1,15 +1,18 @@
 """Plain O(n) statement of the paper's eviction rule -- TEST INFRASTRUCTURE ONLY (tests/, bench.py's baseline legs).
 
 Follows the paper line by line, no ordered sets, no log-domain keys:
-  Eq. (7)   dT_B   = 2*k5*pos_B + c0            (pos_B = tokens in front of block B)
-  Eq. (9) (PAPER.md:213)       f_B(t) = min(exp(-tau/alpha), exp(-(tau - tau0)/beta)),  tau = t - last_access(B)
-  Eq. (3) (PAPER.md:136-142)   evict argmin_B f_B(t) * dT_B
-  Algorithm 1 line 8 generalises the argmin with lambda: argmin{ min_B w1, lambda * min_B w2 }.
+  Eq. (7)       dT_B   = 2*k5*pos_B + c0            (pos_B = tokens in front of block B)
+  Eq. (9) (PAPER.md:202)       f_B(t) = min(exp(-tau/alpha), exp(-(tau - tau0)/beta)),  tau = t - last_access(B)
+  Eq. (3) (PAPER.md:135-136)   evict argmin_B f_B(t) * dT_B
+  Algorithm 1 line 8 generalises the argmin with lambda: argmin{ min_B w1, lambda * min_B w2 };
+  Eq. (10) says which lambda moves the turning point to a lifespan tau:
+  lambda = exp((tau - tau0)/beta - tau/alpha), i.e. w1 == lambda*w2 for a block of exactly that age.
 Shares no code with paper_2606_02964_b200/csrc/msa_evictor.cpp (which never forms these exponentials).
 
 Pins (tests/test_evictor.py): constant dT degenerates to LRU; equal recency evicts the cheapest-to-
 recompute block; the two branches of Eq. (9) cross at tau* = tau0*alpha/(alpha-beta); each branch obeys
-the order-preserving rule Eq. (8).
+the order-preserving rule Eq. (8); the lambda branch: with Eq. (10)'s lambda the two branch weights of a
+block of age tau are equal, and the victim flips from the w1-minimum to the w2-minimum as lambda crosses that value.
 """
 from __future__ import annotations
 

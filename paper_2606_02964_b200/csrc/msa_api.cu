@@ -38,6 +38,22 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
+// Makes the handle's device current for the duration of a call and restores the caller's afterwards.
+struct DeviceGuard {
+    int prev = -1;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int device)
+    {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != device) err = cudaSetDevice(device);
+        else if (err == cudaSuccess) prev = -1;       // nothing to restore
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
 struct DevBuf {
     void *p = nullptr;
     size_t cap = 0;
@@ -66,11 +82,23 @@ struct msa_handle_s {
     int G = 0, R = 0;
     int num_sms = 0;
     bool planning_only = false;
-    FwdVariant variant = FwdVariant::Simple;
-    int emu = kDefaultEmu;             // debug env MSA_EMU overrides (tuning sweeps)
     std::vector<int32_t> kv_to_q;      // [Hkv][G]
     int32_t *d_kv_to_q = nullptr;
     EncodeTiledFn encode = nullptr;
+    // Tensor maps depend only on (base pointer, extent) of q / pool / arena: a model calls msa_forward once per
+    // layer with the same few pointer sets step after step, so the 23 encoded maps are kept per pointer set.
+    struct MapKey {
+        const void *q, *pool_k, *pool_v, *contig_k, *contig_v;
+        int64_t total_q, num_blocks, contig_rows;
+        bool operator==(const MapKey &o) const
+        {
+            return q == o.q && pool_k == o.pool_k && pool_v == o.pool_v && contig_k == o.contig_k && contig_v == o.contig_v &&
+                   total_q == o.total_q && num_blocks == o.num_blocks && contig_rows == o.contig_rows;
+        }
+    };
+    struct MapEntry { MapKey key; FwdParams maps; uint64_t stamp; };
+    std::vector<MapEntry> map_cache;   // at most kMapCacheEntries, least recently used replaced
+    uint64_t map_stamp = 0;
     int last_launches = 0;
     // optional per-launch timing (msa_set_timing): 3 events per recorded step
     bool timing = false;
@@ -150,10 +178,6 @@ int msa_create(const msa_config *cfg, msa_handle *out)
         }
         h->kv_to_q[static_cast<size_t>(kv) * G + fill[kv]++] = q;
     }
-    const char *kv = getenv("MSA_KERNEL");
-    h->variant = (kv && strcmp(kv, "simple") == 0) ? FwdVariant::Simple : FwdVariant::Pipelined;
-    if (const char *em = getenv("MSA_EMU")) h->emu = atoi(em);
-
     if (cfg->device < 0) {
         // planning-only handle: descriptor validation and scheduling on the host; every
         // call that would touch the GPU reports MSA_ERR_NO_DEVICE.
@@ -175,7 +199,9 @@ int msa_create(const msa_config *cfg, msa_handle *out)
         return MSA_ERR_NO_DEVICE;
     }
     h->num_sms = prop.multiProcessorCount;
-    cudaError_t e = cudaSetDevice(cfg->device);
+    DeviceGuard guard(cfg->device);
+    cudaError_t e = guard.err;
+    if (e == cudaSuccess) e = configure_fwd(cfg->head_dim);     // per device: a second handle on another GPU sets its own
     if (e == cudaSuccess) e = cudaMalloc(&h->d_kv_to_q, h->kv_to_q.size() * sizeof(int32_t));
     if (e == cudaSuccess)
         e = cudaMemcpy(h->d_kv_to_q, h->kv_to_q.data(), h->kv_to_q.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
@@ -196,6 +222,7 @@ void msa_destroy(msa_handle h)
 {
     if (!h) return;
     if (!h->planning_only) {
+        DeviceGuard guard(h->cfg.device);
         if (h->d_kv_to_q) cudaFree(h->d_kv_to_q);
         for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
         h->s_q.release(); h->s_o.release(); h->s_lse.release(); h->s_ck.release();
@@ -215,9 +242,8 @@ int msa_plan_create(msa_handle h, const msa_request *requests, int32_t n_req, co
     pc.D = h->cfg.head_dim;
     pc.G = h->G;
     pc.R = h->R;
-    pc.tiles_per_group = fwd_tiles_per_group(h->variant);
+    pc.tiles_per_group = kTilesPerGroup;
     pc.num_ctas = h->num_sms;
-    if (const char *nc = getenv("MSA_NUM_CTAS")) pc.num_ctas = std::max(1, std::min(h->num_sms, atoi(nc)));   // debug: scaling experiments
     msa_plan p = new (std::nothrow) msa_plan_s();
     if (!p) return MSA_ERR_INVALID_ARG;
     p->h = h;
@@ -235,7 +261,8 @@ int msa_plan_create(msa_handle h, const msa_request *requests, int32_t n_req, co
         const size_t b_mg = al(hp.merge_items.size() * sizeof(MergeItem));
         const size_t b_ti = al(hp.tile_info.size() * sizeof(TileInfo));
         const size_t total = b_vb + b_un + b_cb + b_mg + b_ti + 256;
-        cudaError_t e = cudaSetDevice(h->cfg.device);
+        DeviceGuard guard(h->cfg.device);
+        cudaError_t e = guard.err;
         if (e == cudaSuccess) e = cudaMalloc(&p->d_buf, total);
         if (e != cudaSuccess) {
             delete p;
@@ -273,7 +300,10 @@ int msa_plan_create(msa_handle h, const msa_request *requests, int32_t n_req, co
 void msa_plan_destroy(msa_plan p)
 {
     if (!p) return;
-    if (p->d_buf) cudaFree(p->d_buf);
+    if (p->d_buf) {
+        DeviceGuard guard(p->h->cfg.device);
+        cudaFree(p->d_buf);
+    }
     delete p;
 }
 
@@ -341,6 +371,57 @@ int encode_2d(msa_handle h, CUtensorMap *tm, const void *base, uint64_t inner_el
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+constexpr size_t kMapCacheEntries = 64;
+
+// The 23 tensor maps of one (q, pool, arena) pointer set, encoded once and kept in the handle.
+int cached_tensor_maps(msa_handle h, const HostPlan &hp, const void *q, int64_t total_q, const void *pool_k, const void *pool_v,
+                       int64_t num_blocks, const void *contig_k, const void *contig_v, int64_t contig_rows, FwdParams *out)
+{
+    const int Hq = h->cfg.num_q_heads, Hkv = h->cfg.num_kv_heads, D = h->cfg.head_dim;
+    // a plan that uses no paged (or no contiguous) segment never dereferences those maps: they are encoded over q
+    msa_handle_s::MapKey key{q, hp.uses_paged ? pool_k : nullptr, hp.uses_paged ? pool_v : nullptr,
+                             hp.uses_contig ? contig_k : nullptr, hp.uses_contig ? contig_v : nullptr,
+                             total_q, hp.uses_paged ? num_blocks : 0, hp.uses_contig ? contig_rows : 0};
+    ++h->map_stamp;
+    for (auto &e : h->map_cache)
+        if (e.key == key) {
+            e.stamp = h->map_stamp;
+            *out = e.maps;
+            return MSA_OK;
+        }
+    FwdParams fp;
+    memset(&fp, 0, sizeof fp);
+    int rc = encode_2d(h, &fp.tm_q, q, static_cast<uint64_t>(Hq) * D, static_cast<uint64_t>(total_q), h->R);
+    if (rc != MSA_OK) return rc;
+    const void *pk = hp.uses_paged ? pool_k : q;
+    const void *pv = hp.uses_paged ? pool_v : q;
+    const uint64_t prow = hp.uses_paged ? static_cast<uint64_t>(num_blocks) * MSA_BLOCK_SIZE : static_cast<uint64_t>(total_q);
+    const uint64_t pin = hp.uses_paged ? static_cast<uint64_t>(Hkv) * D : static_cast<uint64_t>(Hq) * D;
+    for (int i = 0; i < 5; ++i) {
+        if ((rc = encode_2d(h, &fp.tm_pool_k[i], pk, pin, prow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
+        if ((rc = encode_2d(h, &fp.tm_pool_v[i], pv, pin, prow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
+    }
+    const void *ck = hp.uses_contig ? contig_k : q;
+    const void *cv = hp.uses_contig ? contig_v : q;
+    const uint64_t crow = hp.uses_contig ? static_cast<uint64_t>(contig_rows) : static_cast<uint64_t>(total_q);
+    const uint64_t cin = hp.uses_contig ? static_cast<uint64_t>(Hkv) * D : static_cast<uint64_t>(Hq) * D;
+    for (int i = 0; i < 5; ++i) {
+        if ((rc = encode_2d(h, &fp.tm_ctg_k[i], ck, cin, crow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
+        if ((rc = encode_2d(h, &fp.tm_ctg_v[i], cv, cin, crow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
+    }
+    if ((rc = encode_2d(h, &fp.tm_ctg_k128, ck, cin, crow, kTileN)) != MSA_OK) return rc;
+    if ((rc = encode_2d(h, &fp.tm_ctg_v128, cv, cin, crow, kTileN)) != MSA_OK) return rc;
+    if (h->map_cache.size() < kMapCacheEntries) {
+        h->map_cache.push_back({key, fp, h->map_stamp});
+    } else {
+        auto victim = std::min_element(h->map_cache.begin(), h->map_cache.end(),
+                                       [](const msa_handle_s::MapEntry &a, const msa_handle_s::MapEntry &b) { return a.stamp < b.stamp; });
+        *victim = {key, fp, h->map_stamp};
+    }
+    *out = fp;
+    return MSA_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -374,28 +455,11 @@ int msa_forward(msa_handle h, msa_plan p, const void *q, int64_t total_q, const 
     }
 
     const int Hq = h->cfg.num_q_heads, Hkv = h->cfg.num_kv_heads, D = h->cfg.head_dim;
+    DeviceGuard guard(h->cfg.device);      // the caller's current device may be another one
+    if (guard.err != cudaSuccess) return cuda_fail(guard.err, "msa_forward: cudaSetDevice");
     FwdParams fp;
-    memset(&fp, 0, sizeof fp);
-    int rc = encode_2d(h, &fp.tm_q, q, static_cast<uint64_t>(Hq) * D, static_cast<uint64_t>(total_q), h->R);
+    int rc = cached_tensor_maps(h, hp, q, total_q, pool_k, pool_v, num_blocks, contig_k, contig_v, contig_rows, &fp);
     if (rc != MSA_OK) return rc;
-    const void *pk = hp.uses_paged ? pool_k : q;
-    const void *pv = hp.uses_paged ? pool_v : q;
-    const uint64_t prow = hp.uses_paged ? static_cast<uint64_t>(num_blocks) * MSA_BLOCK_SIZE : static_cast<uint64_t>(total_q);
-    const uint64_t pin = hp.uses_paged ? static_cast<uint64_t>(Hkv) * D : static_cast<uint64_t>(Hq) * D;
-    for (int i = 0; i < 5; ++i) {
-        if ((rc = encode_2d(h, &fp.tm_pool_k[i], pk, pin, prow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
-        if ((rc = encode_2d(h, &fp.tm_pool_v[i], pv, pin, prow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
-    }
-    const void *ck = hp.uses_contig ? contig_k : q;
-    const void *cv = hp.uses_contig ? contig_v : q;
-    const uint64_t crow = hp.uses_contig ? static_cast<uint64_t>(contig_rows) : static_cast<uint64_t>(total_q);
-    const uint64_t cin = hp.uses_contig ? static_cast<uint64_t>(Hkv) * D : static_cast<uint64_t>(Hq) * D;
-    for (int i = 0; i < 5; ++i) {
-        if ((rc = encode_2d(h, &fp.tm_ctg_k[i], ck, cin, crow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
-        if ((rc = encode_2d(h, &fp.tm_ctg_v[i], cv, cin, crow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
-    }
-    if ((rc = encode_2d(h, &fp.tm_ctg_k128, ck, cin, crow, kTileN)) != MSA_OK) return rc;
-    if ((rc = encode_2d(h, &fp.tm_ctg_v128, cv, cin, crow, kTileN)) != MSA_OK) return rc;
     fp.vblocks = p->d_vblocks;
     fp.units = p->d_units;
     fp.cta_unit_begin = p->d_cta_begin;
@@ -414,7 +478,7 @@ int msa_forward(msa_handle h, msa_plan p, const void *q, int64_t total_q, const 
     const bool rec = h->timing && static_cast<size_t>(h->ev_steps) * 3 + 3 <= h->ev.size();
     cudaEvent_t *ev = rec ? &h->ev[static_cast<size_t>(h->ev_steps) * 3] : nullptr;
     if (rec) MSA_CUDA(cudaEventRecord(ev[0], stream));
-    MSA_CUDA(launch_fwd(fp, D, hp.info.num_ctas, h->variant, h->emu, stream));
+    MSA_CUDA(launch_fwd(fp, D, hp.info.num_ctas, stream));
     if (rec) MSA_CUDA(cudaEventRecord(ev[1], stream));
     h->last_launches = 1;
     if (!hp.merge_items.empty()) {
@@ -457,7 +521,8 @@ int msa_forward_host(msa_handle h, msa_plan p, const void *q_host, int64_t total
     const size_t b_bt = static_cast<size_t>(block_table_len) * 4;
     const size_t b_ws = static_cast<size_t>(p->hp.workspace_floats) * 4;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-    MSA_CUDA(cudaSetDevice(h->cfg.device));
+    DeviceGuard guard(h->cfg.device);
+    if (guard.err != cudaSuccess) return cuda_fail(guard.err, "msa_forward_host: cudaSetDevice");
     MSA_CUDA(h->s_q.reserve(b_q + 16));
     MSA_CUDA(h->s_o.reserve(b_q + 16));
     MSA_CUDA(h->s_lse.reserve(b_lse + 16));
@@ -521,7 +586,8 @@ int msa_append_plan_create(msa_handle h, const msa_append *jobs, int32_t n_jobs,
             return MSA_ERR_OVERLAP;
         }
     if (!h->planning_only && !ap->units.empty()) {
-        cudaError_t e = cudaSetDevice(h->cfg.device);
+        DeviceGuard guard(h->cfg.device);
+        cudaError_t e = guard.err;
         if (e == cudaSuccess) e = cudaMalloc(&ap->d_units, ap->units.size() * sizeof(AppendUnit));
         if (e == cudaSuccess)
             e = cudaMemcpy(ap->d_units, ap->units.data(), ap->units.size() * sizeof(AppendUnit), cudaMemcpyHostToDevice);
@@ -538,7 +604,10 @@ int msa_append_plan_create(msa_handle h, const msa_append *jobs, int32_t n_jobs,
 void msa_append_plan_destroy(msa_append_plan ap)
 {
     if (!ap) return;
-    if (ap->d_units) cudaFree(ap->d_units);
+    if (ap->d_units) {
+        DeviceGuard guard(ap->h->cfg.device);
+        cudaFree(ap->d_units);
+    }
     delete ap;
 }
 
@@ -555,6 +624,8 @@ int msa_kv_append(msa_handle h, msa_append_plan ap, const void *contig_k, const 
     if (!aligned16(contig_k) || !aligned16(contig_v) || !aligned16(pool_k) || !aligned16(pool_v) ||
         (reinterpret_cast<uintptr_t>(block_table) & 3u))
         return MSA_ERR_MISALIGNED;
+    DeviceGuard guard(h->cfg.device);
+    if (guard.err != cudaSuccess) return cuda_fail(guard.err, "msa_kv_append: cudaSetDevice");
     AppendParams ap_params;
     ap_params.units = ap->d_units;
     ap_params.block_table = block_table;
@@ -575,6 +646,8 @@ int msa_set_timing(msa_handle h, int max_steps)
 {
     if (!h || max_steps < 0) return MSA_ERR_INVALID_ARG;
     if (h->planning_only) return MSA_ERR_NO_DEVICE;
+    DeviceGuard guard(h->cfg.device);
+    if (guard.err != cudaSuccess) return cuda_fail(guard.err, "msa_set_timing: cudaSetDevice");
     for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
     h->ev.clear();
     h->ev_steps = 0;

@@ -14,15 +14,17 @@
 //   kModeSplit  one q tile; chain c owns KV tiles c, c+2, ... with its own (ref, l, O);
 //               the epilogue merges the two partial softmaxes (short / decode-like queries)
 // TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P (bf16) aliases
-// the first 64 columns of its S and is handed to the MMA warp in two halves (keys 0-63, 64-127).
+// the first 64 columns of its S and is handed to the MMA warp in three parts (keys 0-63, 64-95,
+// 96-127), so that O += P V trails the exponentials.
 // Shared memory: Q 2 tiles, one ring of 5 tile slots in which K and V tiles alternate (entry
 // 2i = K of the CTA's i-th KV tile, 2i+1 = its V).  The softmax arithmetic, its integer row
 // reference and the overflow guard of the fast path are described in msa_softmax.cuh.
 //
-// Invalid KV slots (block tails, blocks past a context's end) never reach O: their scores
-// are replaced by -inf, and their K/V rows are never written by TMA -- partly filled blocks
-// load through 8/4/2/1-row boxes -- so those smem rows keep earlier, valid (finite) tile
-// data (the ring is zeroed once at kernel start) and P = 0 times a finite value stays 0.
+// Invalid KV slots (block tails, blocks past a context's end or past the causal horizon) never
+// reach O: their scores are replaced by -inf (P = 0), their K/V rows are never written by TMA --
+// partly filled blocks load through 8/4/2/1-row boxes -- and the V loader zeroes exactly those
+// rows of its ring slot before it arms the tile, so P = 0 never meets stale data (another
+// request's Inf / NaN would otherwise turn 0 * x into NaN).
 #pragma once
 #include <math.h>
 
@@ -36,7 +38,7 @@ namespace msa {
 // lane 0 of one warp per role accumulates clock64() deltas into g_prof[cta][slot].
 #ifdef MSA_PROF
 __device__ unsigned long long g_prof[160][32];
-__device__ long long g_trace[3][64][8];
+__device__ long long g_trace[4][64][12];
 #define PROF_TRACE(role, step, ev) \
     do { if (blockIdx.x == 0 && u == u_begin && (step) < 64) g_trace[role][step][ev] = clock64(); } while (0)
 #if MSA_PROF == 2   /* event trace only: no accumulators in the hot loops */
@@ -89,8 +91,9 @@ enum PipeBar : int {
     kBarOFree = 18,      // [2]
     kBarStFull = 20,     // [2]
     kBarStFree = 22,     // [2]
-    kBarPHi = 24,        // [2] P of keys 64-127 in TMEM
-    kBarCount = 26
+    kBarPQ2 = 24,        // [2] P of keys 64-95 in TMEM
+    kBarPQ3 = 26,        // [2] P of keys 96-127 in TMEM
+    kBarCount = 28
 };
 
 struct RingPos {
@@ -110,10 +113,7 @@ struct ResolvedVb {
     int32_t nvp;      // valid slots (0: nothing to load) | paged << 8
 };
 
-// EMU: of every 8 element pairs of a softmax row, how many take 2^x from ex2_poly2 (FMA/ALU
-// pipes) instead of MUFU.EX2; -1 disables the stale-max fast path altogether (two-phase
-// max-then-exp on every tile, all MUFU).
-template <int D, int EMU, int EMU_HI>
+template <int D>
 __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_constant__ FwdParams P)
 {
     using C = PipeCfg<D>;
@@ -130,10 +130,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
     const int lane = threadIdx.x & 31;
     if ((sbase & 1023u) != 0) __trap();
 
-    // one-time setup: zero the K/V ring (see header), barriers, TMEM
-    for (uint32_t i = threadIdx.x * 16u; i < static_cast<uint32_t>(C::kRingBytes); i += 512u * 16u)
-        *reinterpret_cast<uint4 *>(smem + C::kQBytes + i) = make_uint4(0, 0, 0, 0);
-    fence_proxy_async_smem();
+    // one-time setup: barriers, TMEM
     if (threadIdx.x == 0) {
         mbar_init(bar(kBarQFull), 1);
         mbar_init(bar(kBarQEmpty), 1);
@@ -144,7 +141,8 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
         for (int c = 0; c < 2; ++c) {
             mbar_init(bar(kBarSFull + c), 1);
             mbar_init(bar(kBarPLo + c), 4);
-            mbar_init(bar(kBarPHi + c), 4);
+            mbar_init(bar(kBarPQ2 + c), 4);
+            mbar_init(bar(kBarPQ3 + c), 4);
             mbar_init(bar(kBarOFull + c), 1);
             mbar_init(bar(kBarOFree + c), 4);
             mbar_init(bar(kBarStFull + c), 4);
@@ -163,6 +161,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
     const int u_begin = P.cta_unit_begin[blockIdx.x], u_end = P.cta_unit_begin[blockIdx.x + 1];
     const int G = P.G, R = P.R;
     const float sl = P.scale_log2;
+    const float inv_sl = 1.f / sl;
 
     if (warp < 8) {
         // =========================================================== softmax warpgroups
@@ -236,14 +235,14 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                 tc_fence_after();
                 PROF_T0();
                 bool done = false;
-                if (EMU >= 0 && !need_mask && s > 0 && __all_sync(0xffffffffu, has_ref)) {
-                    // fast path: stale reference, tile max found alongside, P handed over in halves
+                if (!need_mask && s > 0 && __all_sync(0xffffffffu, has_ref)) {
+                    // fast path: stale reference, tile max found alongside, P handed over in parts
                     move_reference(true);
                     float tile_sum, tile_max;
-                    done = softmax_fast_tile<(EMU < 0 ? 0 : EMU), EMU_HI>(tS, sl, ref, tile_sum, tile_max, [&]() {
+                    done = softmax_fast_tile(tS, sl, inv_sl, ref, tile_sum, tile_max, [&](int part) {
                         __syncwarp();
-                        if (lane == 0) mbar_arrive(bar(kBarPLo + c));
-                        if ((threadIdx.x & 127) == 0) PROF_TRACE(1 + c, s, 4);
+                        if (lane == 0) mbar_arrive(bar((part == 0 ? kBarPLo : kBarPQ2) + c));
+                        if ((threadIdx.x & 127) == 0 && part == 0) PROF_TRACE(1 + c, s, 4);
                     }, [&](int ev) {
                         if ((threadIdx.x & 127) == 0) PROF_TRACE(1 + c, s, ev);
                     });
@@ -251,7 +250,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                         l += tile_sum;
                         m_run = fmaxf(m_run, tile_max);
                         __syncwarp();
-                        if (lane == 0) mbar_arrive(bar(kBarPHi + c));
+                        if (lane == 0) mbar_arrive(bar(kBarPQ3 + c));
                     }
                     PROF_ADD(20);
                 }
@@ -302,7 +301,8 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     __syncwarp();
                     if (lane == 0) {
                         mbar_arrive(bar(kBarPLo + c));
-                        mbar_arrive(bar(kBarPHi + c));
+                        mbar_arrive(bar(kBarPQ2 + c));
+                        mbar_arrive(bar(kBarPQ3 + c));
                     }
                 }
                 PROF_ADD(2);
@@ -517,6 +517,21 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     }
                     const uint32_t full = bar(kBarKvFull + rp.slot);
                     const uint32_t dst = sRing + rp.slot * C::kTileBytes;
+                    if (which == 1 && m_full != 0xffu) {
+                        // V rows TMA will not write (block tails, blocks past the end / the horizon): zero them
+                        // (generic-proxy stores, made visible to the tensor core's async proxy before the tile is armed)
+#pragma unroll 1
+                        for (int b = 0; b < kVbPerTile; ++b) {
+                            const int nvb = __shfl_sync(0xffffffffu, nv, b);
+                            const uint32_t off0 = static_cast<uint32_t>(nvb) * 128u;
+#pragma unroll 1
+                            for (int h = 0; h < C::kHalves; ++h)
+                                for (uint32_t off = off0 + lane * 16u; off < kBlock * 128u; off += 512u)
+                                    asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(dst + b * (kBlock * 128) + h * C::kHalfBytes + off), "r"(0u) : "memory");
+                        }
+                        fence_proxy_async_smem();
+                        __syncwarp();
+                    }
                     if (run) {
                         if (elect_one()) {
                             mbar_arrive_expect_tx(full, static_cast<uint32_t>(kTileN * D * 2));
@@ -573,6 +588,8 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             constexpr uint32_t idesc_o = make_idesc(128, D, true);
             RingPos rk{0, 0}, rv{1, 0};
             uint32_t ph_q = 0, ph_p[2] = {0, 0}, ph_ofree[2] = {1, 1};
+            int u = u_begin, tr_step = 0;    // (trace builds: which unit / KV step the issuer is in)
+            (void)tr_step;
             PROF_DECL();
 #if defined(MSA_PROF) && MSA_PROF != 2
             const long long prof_mma_start = clock64();
@@ -603,8 +620,8 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                 }
                 umma_commit(bar(kBarSFull + c));
             };
-            // O += P V in two halves: keys 0-63 as soon as the softmax warps have published the
-            // first half of P, keys 64-127 after the second.
+            // O += P V in three parts: keys 0-63 as soon as the softmax warps have published the
+            // first half of P, then keys 64-95 and 96-127 as they arrive.
             auto pv_lo = [&](int c, uint32_t vslot, bool first) {
                 {
                     PROF_T0();
@@ -625,12 +642,20 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                             make_smem_desc(va + k * (kBlock * 128), C::kHalfBytes, 1024), idesc_o, (!first || k > 0) ? 1u : 0u);
             };
             auto pv_hi = [&](int c, uint32_t vslot) {
-                mbar_wait(bar(kBarPHi + c), ph_p[c]);
+                const uint32_t va = sRing + vslot * C::kTileBytes;
+                mbar_wait(bar(kBarPQ2 + c), ph_p[c]);
+                PROF_TRACE(0, tr_step, 7 + 2 * c);
+                tc_fence_after();
+#pragma unroll
+                for (int k = kTileN / 32; k < 3 * kTileN / 64; ++k)
+                    umma_ts(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
+                            make_smem_desc(va + k * (kBlock * 128), C::kHalfBytes, 1024), idesc_o, 1u);
+                mbar_wait(bar(kBarPQ3 + c), ph_p[c]);
+                PROF_TRACE(0, tr_step, 8 + 2 * c);
                 ph_p[c] ^= 1;
                 tc_fence_after();
-                const uint32_t va = sRing + vslot * C::kTileBytes;
 #pragma unroll
-                for (int k = kTileN / 32; k < kTileN / 16; ++k)
+                for (int k = 3 * kTileN / 64; k < kTileN / 16; ++k)
                     umma_ts(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
                             make_smem_desc(va + k * (kBlock * 128), C::kHalfBytes, 1024), idesc_o, 1u);
             };
@@ -638,7 +663,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                 pv_lo(c, vslot, first);
                 pv_hi(c, vslot);
             };
-            for (int u = u_begin; u < u_end; ++u) {
+            for (u = u_begin; u < u_end; ++u) {
                 const WorkUnit wu = P.units[u];
                 const int n = wu.tile_end - wu.tile_begin;
                 if (n <= 0) continue;
@@ -656,6 +681,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     umma_commit(bar(kBarKvEmpty + ks));
                     if (n == 1) umma_commit(bar(kBarQEmpty));
                     for (int j = 0; j < n; ++j) {
+                        tr_step = j;
                         PROF_TRACE(0, j, 0);
                         const uint32_t vs = take_v();
                         PROF_TRACE(0, j, 1);
@@ -718,6 +744,23 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             PROF_FLUSH(8, 15);
 #endif
         }
+#if defined(MSA_PROF) && MSA_PROF == 2
+        else if (warp == 15 && lane == 0 && blockIdx.x == 0 && u_begin < u_end) {
+            // observer (trace builds only): when does each chain's S become complete in the first unit?
+            const WorkUnit wu = P.units[u_begin];
+            const int n = wu.tile_end - wu.tile_begin;
+            if (wu.mode == kModePair) {
+                uint32_t ph = 0;
+                for (int s = 0; s < n && s < 64; ++s) {
+                    mbar_wait(bar(kBarSFull + 0), ph);
+                    g_trace[3][s][0] = clock64();
+                    mbar_wait(bar(kBarSFull + 1), ph);
+                    g_trace[3][s][1] = clock64();
+                    ph ^= 1;
+                }
+            }
+        }
+#endif
     }
 
     tc_fence_before();

@@ -57,14 +57,11 @@ struct AppendParams {
 
 cudaError_t launch_append(const AppendParams &p, int num_sms, cudaStream_t stream);
 
-// kernel variants (debug env MSA_KERNEL selects; default = the fastest validated one)
-enum class FwdVariant : int { Simple = 0, Pipelined = 1 };
-
-// emu: softmax exp2 emulation level of the pipelined kernel (see msa_fwd_pipe.cuh); values
-// without an instantiation fall back to kDefaultEmu.
-constexpr int kDefaultEmu = 0;
-cudaError_t launch_fwd(const FwdParams &p, int head_dim, int num_ctas, FwdVariant v, int emu, cudaStream_t stream);
+// Forward kernel: persistent, warp-specialised (msa_fwd_pipe.cuh).  configure_fwd sets the kernel's dynamic
+// shared-memory limit on the CURRENT device (once per device and head dim); launch_fwd assumes it was done.
+constexpr int kTilesPerGroup = 2;    // q tiles (of 128 packed rows) one work item covers in pair mode
+cudaError_t configure_fwd(int head_dim);
+cudaError_t launch_fwd(const FwdParams &p, int head_dim, int num_ctas, cudaStream_t stream);
 cudaError_t launch_merge(const MergeParams &p, int n_items, int max_rows, cudaStream_t stream);
-int fwd_tiles_per_group(FwdVariant v);   // q tiles (of 128 packed rows) one work item covers
 
 }  // namespace msa

@@ -42,15 +42,29 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
         : "memory");
     return ok != 0;
 }
+// try_wait with a suspend-time hint: the warp sleeps in hardware until the phase completes (it is woken at
+// once) or the hint (ns) runs out, instead of coming back every few dozen cycles and taking issue slots from
+// the warps of its SM sub-partition that have work.
+__device__ __forceinline__ bool mbar_try_wait_sleep(uint32_t bar, uint32_t parity, uint32_t hint_ns)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity), "r"(hint_ns)
+        : "memory");
+    return ok != 0;
+}
 // Waits for the phase with the given parity to complete.  A wait that lasts longer than
 // ~2 s of SM clocks traps instead of hanging the device (a lost arrive is a bug, not a state).
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     if (mbar_try_wait(bar, parity)) return;
     const long long t0 = clock64();
-    uint32_t spins = 0;
-    while (!mbar_try_wait(bar, parity)) {
-        if ((++spins & 0x3ff) == 0 && clock64() - t0 > 4000000000LL) __trap();
+    while (!mbar_try_wait_sleep(bar, parity, 1000000u)) {
+        if (clock64() - t0 > 4000000000LL) __trap();
     }
 }
 
@@ -67,20 +81,7 @@ __device__ __forceinline__ void tc_fence_after()
 {
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 }
-__device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t nthreads)
-{
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-__device__ __forceinline__ void named_bar_arrive(uint32_t id, uint32_t nthreads)
-{
-    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-
 // ------------------------------------------------------------------ TMA
-__device__ __forceinline__ void tma_prefetch_desc(const void *tmap)
-{
-    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tmap)) : "memory");
-}
 // 2-D tiled load: box lands at smem `dst`, completes `bytes` on mbarrier `bar`.
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const void *tmap, uint32_t bar, int32_t c0, int32_t c1)
 {
@@ -89,28 +90,6 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const void *tmap, uint
         ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(bar), "r"(c0), "r"(c1)
         : "memory");
 }
-__device__ __forceinline__ void tma_load_2d_hint(uint32_t dst, const void *tmap, uint32_t bar, int32_t c0, int32_t c1,
-                                                 uint64_t policy)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
-        " [%0], [%1, {%3, %4}], [%2], %5;"
-        ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(bar), "r"(c0), "r"(c1), "l"(policy)
-        : "memory");
-}
-__device__ __forceinline__ uint64_t l2_policy_evict_first()
-{
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
-__device__ __forceinline__ uint64_t l2_policy_evict_last()
-{
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
-
 // ------------------------------------------------------------------ TMEM
 __device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols)
 {
@@ -205,18 +184,6 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16])
         : "r"(taddr)
         : "memory");
 }
-__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32])
-{
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
-        "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
-        "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
-        ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
-          "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),
-          "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]),
-          "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
-        : "memory");
-}
 __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16])
 {
     asm volatile(
@@ -225,6 +192,48 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16
         ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
           "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
         : "memory");
+}
+// 16x256b / 16x128b: the warp touches 16 TMEM lanes starting at the address's lane (a multiple of 16
+// inside the warp's 32-lane quarter).  Thread t holds, per repetition i (checked on B200 with a probe):
+//   ld 16x256b: r[4i], r[4i+1] = lane t/4,     columns 8i + 2(t%4), 8i + 2(t%4) + 1
+//               r[4i+2], r[4i+3] = lane t/4 + 8, same columns
+//   st 16x128b: r[2i] = lane t/4, column 4i + t%4;  r[2i+1] = lane t/4 + 8, same column
+// so a row's 32-bit pairs packed to bf16x2 land in exactly the thread that computed them.
+__device__ __forceinline__ void tmem_ld_16x256b_x4(uint32_t taddr, uint32_t (&r)[16])
+{
+    asm volatile("tcgen05.ld.sync.aligned.16x256b.x4.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+                   "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                 : "r"(taddr)
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_st_16x256b_x4(uint32_t taddr, const uint32_t (&r)[16])
+{
+    asm volatile("tcgen05.st.sync.aligned.16x256b.x4.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+                 ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+                   "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_st_16x128b_x4(uint32_t taddr, const uint32_t (&r)[8])
+{
+    asm volatile("tcgen05.st.sync.aligned.16x128b.x4.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                 ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+                 : "memory");
+}
+// wait::st that names registers computed by the work that is meant to hide the store latency: the compiler cannot
+// schedule the wait (and the publication that follows it) above that work
+__device__ __forceinline__ void tmem_wait_st_after(uint32_t &a, uint32_t &b, uint32_t &c, uint32_t &d)
+{
+    asm volatile("tcgen05.wait::st.sync.aligned;" : "+r"(a), "+r"(b), "+r"(c), "+r"(d) : : "memory");
+}
+// wait::ld that also names 16 destination registers, so no consumer of them can be scheduled above the wait
+__device__ __forceinline__ void tmem_wait_ld_regs16(uint32_t *r)
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]),
+                   "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15])
+                 :
+                 : "memory");
 }
 __device__ __forceinline__ void tmem_wait_ld()
 {
@@ -267,34 +276,14 @@ __device__ __forceinline__ float2 fadd2(float2 a, float2 b)
         : "l"(*reinterpret_cast<uint64_t *>(&a)), "l"(*reinterpret_cast<uint64_t *>(&b)));
     return *reinterpret_cast<float2 *>(&d);
 }
-__device__ __forceinline__ float2 fadd2_rm(float2 a, float2 b)   // round toward -inf
+__device__ __forceinline__ float2 ffma2_rm(float2 a, float2 b, float2 c)   // round toward -inf
 {
     uint64_t d;
-    asm("add.rm.ftz.f32x2 %0, %1, %2;"
+    asm("fma.rm.ftz.f32x2 %0, %1, %2, %3;"
         : "=l"(d)
-        : "l"(*reinterpret_cast<uint64_t *>(&a)), "l"(*reinterpret_cast<uint64_t *>(&b)));
+        : "l"(*reinterpret_cast<uint64_t *>(&a)), "l"(*reinterpret_cast<uint64_t *>(&b)),
+          "l"(*reinterpret_cast<uint64_t *>(&c)));
     return *reinterpret_cast<float2 *>(&d);
-}
-// 2^x for a pair, on the FMA / ALU pipes instead of the 16-lane MUFU: x = n + f with
-// n = floor(x) taken from the mantissa of x + 1.5*2^23 (rounded down), 2^f by a degree-3
-// polynomial with p(0) = 1 (minimax relative error 8.6e-5 on [0,1), mean bias 7e-6 -- far
-// below the bf16 rounding of P, 2^-9), and n added into the exponent field.  Valid for
-// finite x <= 127; x below -126 is clamped (result 2^-126 instead of a denormal / 0).
-__device__ __forceinline__ float2 ex2_poly2(float2 x)
-{
-    constexpr float kMagic = 12582912.f;   // 1.5 * 2^23
-    x.x = fmaxf(x.x, -126.f);
-    x.y = fmaxf(x.y, -126.f);
-    const float2 r = fadd2_rm(x, make_float2(kMagic, kMagic));
-    const float2 fl = fadd2(r, make_float2(-kMagic, -kMagic));
-    const float2 f = fadd2(x, make_float2(-fl.x, -fl.y));
-    float2 p = ffma2(f, make_float2(0.07706724107265472f, 0.07706724107265472f),
-                     make_float2(0.22764497995376587f, 0.22764497995376587f));
-    p = ffma2(p, f, make_float2(0.6951166391372681f, 0.6951166391372681f));
-    p = ffma2(p, f, make_float2(1.f, 1.f));
-    p.x = __uint_as_float(__float_as_uint(p.x) + (__float_as_uint(r.x) << 23));
-    p.y = __uint_as_float(__float_as_uint(p.y) + (__float_as_uint(r.y) << 23));
-    return p;
 }
 // wait::ld that also names the 32 destination registers, so no consumer of them can be
 // scheduled above the wait by the compiler.

@@ -7,21 +7,23 @@
 // the reference moves; it only has to stay close enough above/below the scores for fp32 / bf16
 // range.  The fast path therefore uses the reference it was handed (stale by up to this tile),
 // finds the tile's own row max alongside, and the caller moves the reference before the next
-// tile.  The only hazard is overflow when a tile's scores exceed the reference by more than
-// ~2^120: a guard over the WHOLE tile is evaluated before anything is stored, so the caller
-// can redo the tile on the exact (max-first) path with S still intact.
+// tile.  The only hazard is overflow when a tile's scores exceed the reference by a lot: a guard
+// over the WHOLE tile (score - ref <= 2^kGuardLog2) is evaluated before anything is stored, so the
+// caller can redo the tile on the exact (max-first) path with S still intact.  The guard leaves
+// headroom for the accumulation that follows: P <= 2^64, a tile adds at most 2^71 to l and
+// 2^71 |V| to O (fp32 holds 2^127).
 //
-// Pipes.  The arithmetic is spread over three pipes so that none of them alone bounds the tile
-// (B200, one softmax warp per SM sub-partition; measured: MUFU.EX2 8.0 cycles per warp
-// instruction, FFMA2/FADD2 2.3, F2FP 2.1):
-//   * x = s*scale_log2 - ref              one FFMA2 per element pair
-//   * 2^x                                  MUFU.EX2, or ex2_poly2 on the FMA/ALU pipes for EMU of
-//                                          every 8 pairs
-//   * row sum from the fp32 p (FADD2), row max of the raw scores (FMNMX3), bf16 pack (F2FP)
+// Pipes (B200, measured with working microbenchmarks, cycles per warp instruction on one SM
+// sub-partition): MUFU.EX2 8.0; FFMA2 / FADD2 2.1; every ALU-pipe instruction (F2FP pack, FMNMX,
+// LEA) 2.0; FFMA / FADD 1.0.  MUFU time overlaps with everything else, FFMA2 and ALU time add up.
+// An all-MUFU tile therefore costs 1024 cycles of MUFU per warp while the tensor core needs 1024
+// per tile and chain: with both chains on one sub-partition MUFU alone would bound the kernel.
+// kEmuMask moves part of the exponentials to the FMA/ALU pipes (ex2_emu_pair: exact range
+// reduction by two FMAs, degree-3 polynomial, exponent added as an integer).
 //
-// Hand-off.  P is published in two halves (keys 0-63, then 64-127): `arrive_lo` is called once
-// the first 32 columns of P are visible to the tensor core, so O += P V starts on the first
-// half while the second half is still being exponentiated.
+// Hand-off.  P is published in three steps (keys 0-63, 64-95, 96-127): `arrive(i)` is called once
+// the corresponding columns of P are visible to the tensor core, so O += P V trails the
+// exponentials and only the last 32 keys remain to be multiplied when the tile is done.
 #pragma once
 #include <math.h>
 
@@ -29,7 +31,50 @@
 
 namespace msa {
 
-constexpr float kGuardLog2 = 120.f;   // largest s*scale_log2 - ref the fast path accepts
+constexpr float kGuardLog2 = 64.f;    // largest s*scale_log2 - ref the fast path accepts
+// bit j: pair j of the 16 element pairs of every 32-column chunk takes 2^x from ex2_emu_pair
+// (FMA / ALU pipes) instead of MUFU.EX2
+#ifndef MSA_EMU_MASK
+#define MSA_EMU_MASK 0x0000u
+#endif
+constexpr uint32_t kEmuMask = MSA_EMU_MASK;
+
+struct SoftmaxRow {
+    float2 sl2;       // scale_log2
+    float2 nr2;       // -ref
+    float2 k2;        // 1.5*2^23 - ref (exact: both are integers below 2^24)
+    float s_floor;    // scores below (ref - 120)/scale_log2 are clamped: their p is < 2^-120 either way
+};
+
+__device__ __forceinline__ SoftmaxRow make_softmax_row(float sl, float inv_sl, float ref)
+{
+    SoftmaxRow r;
+    r.sl2 = make_float2(sl, sl);
+    r.nr2 = make_float2(-ref, -ref);
+    r.k2 = make_float2(12582912.f - ref, 12582912.f - ref);
+    r.s_floor = (ref - 120.f) * inv_sl;
+    return r;
+}
+
+// 2^(s*sl - ref) for a pair on the FMA / ALU pipes, straight from the raw scores:
+//   r = fma.rm(s, sl, magic - ref) = magic + floor(x)      (x = s*sl - ref, |x| < 2^22)
+//   f = fma(s, sl, (magic - ref) - r) = x - floor(x)       one rounding, in [0, 1]
+//   2^f by a degree-3 polynomial with p(0) = 1 (minimax relative error 8.6e-5 on [0,1), far below
+//   the bf16 rounding of P), floor(x) added into the exponent field.
+__device__ __forceinline__ float2 ex2_emu_pair(float s0, float s1, const SoftmaxRow &t)
+{
+    const float2 sc = make_float2(fmaxf(s0, t.s_floor), fmaxf(s1, t.s_floor));
+    const float2 r = ffma2_rm(sc, t.sl2, t.k2);
+    const float2 c = ffma2(r, make_float2(-1.f, -1.f), t.k2);
+    const float2 f = ffma2(sc, t.sl2, c);
+    float2 p = ffma2(f, make_float2(0.07706724107265472f, 0.07706724107265472f),
+                     make_float2(0.22764497995376587f, 0.22764497995376587f));
+    p = ffma2(p, f, make_float2(0.6951166391372681f, 0.6951166391372681f));
+    p = ffma2(p, f, make_float2(1.f, 1.f));
+    p.x = __uint_as_float(__float_as_uint(p.x) + (__float_as_uint(r.x) << 23));
+    p.y = __uint_as_float(__float_as_uint(p.y) + (__float_as_uint(r.y) << 23));
+    return p;
+}
 
 __device__ __forceinline__ float chunk_max(const uint32_t (&sr)[32])
 {
@@ -42,19 +87,20 @@ __device__ __forceinline__ float chunk_max(const uint32_t (&sr)[32])
     return fmaxf(a, b);
 }
 
-// One 32-column chunk: scores -> 16 packed bf16 pairs; two sum accumulators keep the
-// dependent FADD2 chain short.
-template <int EMU>
-__device__ __forceinline__ void softmax_chunk(const uint32_t (&sr)[32], float2 sl2, float2 nr2, float2 &sa, float2 &sb,
+// Pairs [J0, J1) of a 32-column chunk: scores -> packed bf16 pairs; two sum accumulators keep
+// the dependent FADD2 chain short.  MASK bit j: pair j takes 2^x from ex2_emu_pair.
+template <uint32_t MASK, int J0, int J1>
+__device__ __forceinline__ void softmax_pairs(const uint32_t (&sr)[32], const SoftmaxRow &t, float2 &sa, float2 &sb,
                                               uint32_t (&pk)[16])
 {
 #pragma unroll
-    for (int j = 0; j < 16; ++j) {
-        const float2 x = ffma2(make_float2(__uint_as_float(sr[2 * j]), __uint_as_float(sr[2 * j + 1])), sl2, nr2);
+    for (int j = J0; j < J1; ++j) {
+        const float s0 = __uint_as_float(sr[2 * j]), s1 = __uint_as_float(sr[2 * j + 1]);
         float2 pp;
-        if ((j & 7) < EMU) {
-            pp = ex2_poly2(x);
+        if (MASK >> j & 1) {
+            pp = ex2_emu_pair(s0, s1, t);
         } else {
+            const float2 x = ffma2(make_float2(s0, s1), t.sl2, t.nr2);
             pp.x = ex2_approx(x.x);
             pp.y = ex2_approx(x.y);
         }
@@ -65,15 +111,16 @@ __device__ __forceinline__ void softmax_chunk(const uint32_t (&sr)[32], float2 s
 
 // Whole tile.  tS: TMEM address of the row's S (lane already folded in).  Returns false, with
 // nothing stored, if some row of the warp failed the overflow guard.  Otherwise P is complete
-// in TMEM (stores waited for, tcgen05 fence issued): `arrive_lo()` has been called for the
-// first half and the caller arrives for the second.  `mark(i)` is a profiling hook (no-op in
-// the shipped build).  tile_sum = sum of p against `ref`,
-// tile_max = max raw score.
-template <int EMU, int EMU_HI, class ArriveLo, class Mark>
-__device__ __forceinline__ bool softmax_fast_tile(uint32_t tS, float sl, float ref, float &tile_sum, float &tile_max,
-                                                  ArriveLo &&arrive_lo, Mark &&mark)
+// in TMEM (stores waited for, tcgen05 fence issued): `arrive(0)` and `arrive(1)` have been called
+// for keys 0-63 and 64-95 and the caller arrives for the rest.  `mark(i)` is a profiling hook
+// (no-op in the shipped build).  tile_sum = sum of p against `ref`, tile_max = max raw score.
+// The waits for the P stores name registers of the chunk computed in between (tmem_wait_st_after):
+// without that the compiler is free to schedule the wait -- and the stall -- right behind the store.
+template <class Arrive, class Mark>
+__device__ __forceinline__ bool softmax_fast_tile(uint32_t tS, float sl, float inv_sl, float ref, float &tile_sum,
+                                                  float &tile_max, Arrive &&arrive, Mark &&mark)
 {
-    const float2 sl2 = make_float2(sl, sl), nr2 = make_float2(-ref, -ref);
+    const SoftmaxRow t = make_softmax_row(sl, inv_sl, ref);
     float2 sa = make_float2(0.f, 0.f), sb = make_float2(0.f, 0.f);
     uint32_t c0[32], c1[32], c2[32], c3[32];
     uint32_t pk0[16], pk1[16];
@@ -85,27 +132,31 @@ __device__ __forceinline__ bool softmax_fast_tile(uint32_t tS, float sl, float r
     tmem_ld32(tS + 96, c3);
     mark(1);
     float mx = fmaxf(chunk_max(c0), chunk_max(c1));
-    softmax_chunk<EMU>(c0, sl2, nr2, sa, sb, pk0);
+    softmax_pairs<kEmuMask, 0, 16>(c0, t, sa, sb, pk0);
     // the second half has landed by now: its row max is found among the arithmetic of chunk 1,
     // so the guard is ready as soon as the first half of P is
     tmem_wait_ld_regs(c2);
     tmem_wait_ld_regs(c3);
     mx = fmaxf(mx, fmaxf(chunk_max(c2), chunk_max(c3)));
-    softmax_chunk<EMU>(c1, sl2, nr2, sa, sb, pk1);
+    softmax_pairs<kEmuMask, 0, 16>(c1, t, sa, sb, pk1);
     mark(2);
     tile_max = mx;
     if (__any_sync(0xffffffffu, !(fmaf(mx, sl, -ref) <= kGuardLog2))) return false;
     mark(3);
     tmem_st16(tS, pk0);
     tmem_st16(tS + 16, pk1);
-    // the first half is published one chunk later: its stores have completed by then (no stall),
-    // and O += P V of keys 0-63 still finishes long before the second half is ready
-    softmax_chunk<EMU_HI>(c2, sl2, nr2, sa, sb, pk0);
-    tmem_wait_st();
+    // each part is published while the next one is computed: its stores have completed by then
+    // (no stall), and O += P V of the published keys finishes before the next part is ready
+    softmax_pairs<kEmuMask, 0, 16>(c2, t, sa, sb, pk0);
+    tmem_wait_st_after(pk0[12], pk0[13], pk0[14], pk0[15]);
     tc_fence_before();
-    arrive_lo();
+    arrive(0);
     tmem_st16(tS + 32, pk0);
-    softmax_chunk<EMU_HI>(c3, sl2, nr2, sa, sb, pk1);
+    softmax_pairs<kEmuMask, 0, 8>(c3, t, sa, sb, pk1);
+    tmem_wait_st_after(pk1[4], pk1[5], pk1[6], pk1[7]);
+    tc_fence_before();
+    arrive(1);
+    softmax_pairs<kEmuMask, 8, 16>(c3, t, sa, sb, pk1);
     tmem_st16(tS + 48, pk1);
     tile_sum = (sa.x + sb.x) + (sa.y + sb.y);
     mark(5);

@@ -68,6 +68,59 @@ def test_each_branch_obeys_the_order_preserving_rule():
                 assert np.array_equal(s0[np.ix_(a, a)], s[np.ix_(b, b)])
 
 
+def _eq10_lambda(tau, alpha, beta, tau0):
+    """Eq. (10), retyped from the paper (not taken from the oracle)."""
+    return math.exp((tau - tau0) / beta - tau / alpha)
+
+
+@pytest.mark.parametrize("tau", [30.0, 200.0, 553.8461538461538, 900.0])
+def test_eq10_lambda_moves_the_turning_point_to_the_given_lifespan(tau):
+    """Eq. (10): with lambda = exp((tau - tau0)/beta - tau/alpha) the two branch weights of a block of age tau are
+    equal (w1 == lambda * w2); a younger block is still weighed by the slow branch w1 (lambda does NOT touch it), an
+    older one by lambda * w2 (Algorithm 1 line 8: lambda multiplies the SECOND tree's minimum)."""
+    a, b, t0 = P["alpha"], P["beta"], P["tau0"]
+    lam = _eq10_lambda(tau, a, b, t0)
+    if tau == pytest.approx(t0 * a / (a - b)):
+        assert lam == pytest.approx(1.0, rel=1e-9)          # the original turning point needs no correction
+    ev = LinearEvictor(lambda_=lam, **P)
+    t = 5000.0
+    ev.add(0, 4096, t - tau)                 # exactly at the (new) turning point
+    ev.add(1, 4096, t - 0.5 * tau)           # younger: inside the lifespan
+    ev.add(2, 4096, t - (tau + 60.0))        # older: past it
+    d = 2.0 * P["k5"] * 4096 + P["c0"]       # Eq. (7)
+    w1, w2 = ev.weights(0, t)
+    assert w1 == pytest.approx(lam * w2, rel=1e-12)
+    assert ev.weight(0, t) == pytest.approx(w1, rel=1e-12)
+    assert ev.weight(1, t) == pytest.approx(math.exp(-0.5 * tau / a) * d, rel=1e-12)
+    assert ev.weight(2, t) == pytest.approx(lam * math.exp(-(tau + 60.0 - t0) / b) * d, rel=1e-12)
+    assert ev.weight(2, t) < ev.weight(0, t) < ev.weight(1, t)
+    assert [ev.evict(t) for _ in range(3)] == [2, 0, 1]
+
+
+def test_victim_flips_from_the_w1_minimum_to_the_w2_minimum_as_lambda_crosses_w1_over_w2():
+    """Algorithm 1 line 8: i = argmin{B1.w1, lambda * B2.w2}.  A = the w1-minimum (young, cheap), B = the w2-minimum
+    (old, expensive).  The victim is A for lambda > w1(A)/w2(B) and B below it; the crossing is far from 1, so an
+    implementation that put lambda on the other branch (crossing at w2(B)/w1(A)) fails."""
+    t = 5000.0
+    blocks = {7: (0, t - 100.0), 8: (32768 * 16, t - 700.0)}        # id: (pos, last access)
+
+    def victim(lam):
+        ev = LinearEvictor(lambda_=lam, **P)
+        for bid, (pos, last) in blocks.items():
+            ev.add(bid, pos, last)
+        return ev.evict(t)
+
+    dA, dB = 2.0 * P["k5"] * 0 + P["c0"], 2.0 * P["k5"] * 32768 * 16 + P["c0"]
+    w1A, w1B = math.exp(-100.0 / P["alpha"]) * dA, math.exp(-700.0 / P["alpha"]) * dB
+    w2A, w2B = math.exp(-(100.0 - P["tau0"]) / P["beta"]) * dA, math.exp(-(700.0 - P["tau0"]) / P["beta"]) * dB
+    assert w1A < w1B and w2B < w2A                                   # A heads tree 1, B heads tree 2
+    cross = w1A / w2B
+    assert cross > 50.0                                              # nowhere near its own reciprocal
+    assert victim(cross * 1.001) == 7 and victim(cross * 0.999) == 8
+    assert victim(1.0) == 8 and victim(1.0 / cross) == 8             # lambda on the wrong branch would return 7 here
+    assert victim(cross * cross) == 7
+
+
 # ------------------------------------------------------------------ C++ evictor against the oracle
 @pytest.mark.parametrize("seed,lam", [(10, 1.0), (11, 1.0), (12, 0.05), (13, 40.0)])
 def test_cpp_evictor_makes_the_oracles_decisions_on_random_traces(seed, lam):
@@ -124,7 +177,7 @@ def test_cpp_evictor_error_codes():
 
 def test_policy_trace_shows_the_two_ended_residency_of_observation_2():
     """under pressure the shared prefix and the suffixes survive, the middle of a sequence goes."""
-    from paper_2606_02964_b200.policy_trace import f3_policy_trace, policy_residency
+    from workloads.policy_trace import f3_policy_trace, policy_residency
     sessions, summary = policy_residency()
     assert summary["kept_fraction"] == pytest.approx(0.6, abs=1e-3)
     three = 0

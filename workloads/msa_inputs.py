@@ -585,6 +585,35 @@ def f1_hybrid_pod(device="cpu", layout_only=False, n_prefill: int = 16, n_decode
                          pool_blocks=int(1.1 * cached_blocks) + 1, layout_only=layout_only)
 
 
+def f2_fig13(cached_tokens: int, layout: str, device="cpu", new_tokens: int = 128, keep_dense: bool = False,
+             recompute_tokens: Optional[int] = None) -> MsaProblem:
+    """the request shape of the paper's Fig. 13, Llama-3-8B heads:
+    "a variable number of cached tokens [N] and ends with 128 new (uncached) tokens".  The figure itself is missing
+    from PAPER.md, so how long the uncached history is stays a reading (DESIGN.md c18): R = N recomputed tokens.
+
+      'prefix_new'  [cached N][new 128]                   one run of 128 (what remains when nothing was evicted)
+      'prefix'      [cached N][recompute R + new 128]     caching from the prefix: ONE run of R+128 tokens behind N cached
+      'suffix'      [recompute R][cached N][new 128]      caching from the suffix: TWO runs (R tokens at position 0, the
+                                                          128 new ones at R+N) sharing one segment list -- the
+                                                          two-segment instance of Eq. (2)
+    """
+    N, T = int(cached_tokens), int(new_tokens)
+    R = N if recompute_tokens is None else int(recompute_tokens)
+    if layout == "prefix_new":
+        ctx = ContextSpec([(SEG_PAGED, 0, N), (SEG_SELF, N, T)])
+        runs = [RunSpec(0, N, T)]
+    elif layout == "prefix":
+        ctx = ContextSpec([(SEG_PAGED, 0, N), (SEG_SELF, N, R + T)])
+        runs = [RunSpec(0, N, R + T)]
+    elif layout == "suffix":
+        ctx = ContextSpec([(SEG_SELF, 0, R), (SEG_PAGED, R, N), (SEG_SELF, R + N, T)])
+        runs = [RunSpec(0, 0, R), RunSpec(0, R + N, T)]
+    else:
+        raise ValueError(layout)
+    return build_problem(f"f2_fig13_{layout}_{N}", 32, 8, 128, [ctx], runs, seed=1300 + N, device=device,
+                         keep_dense=keep_dense)
+
+
 CONFIGS = dict(cfg1_tiny=cfg1_tiny, cfg2_llama8b=cfg2_llama8b, cfg3_70b_long=cfg3_70b_long,
                cfg4_mixed=cfg4_mixed, cfg5_short_query=cfg5_short_query)
 # workloads beyond BASELINE.json's five (SURVEY.md section 8 (f) "next" rows)

@@ -15,8 +15,7 @@ from typing import Dict, List, Tuple
 
 import numpy as np
 
-import workloads as W
-from .binding import MsaEvictor
+from . import msa_inputs as W
 
 BLOCK = 16
 
@@ -26,6 +25,9 @@ def policy_residency(n_sessions: int = 48, keep_fraction: float = 0.6, seed: int
                      tau0: float = 540.0, prefix_tokens: int = 512) -> Tuple[List[Dict], Dict]:
     """Returns per session {L, T, resident: bool per block} and a summary.  k5 / c0 default to the values refitted from
     measured msa_forward latencies on B200 (bench.py --workload costmodel, Eq. (6)/(7) of the paper)."""
+    # the product's C++ evictor decides the victims (imported here, not at module level: the generator package
+    # itself never depends on the product library)
+    from paper_2606_02964_b200.binding import MsaEvictor
     rng = np.random.default_rng(seed)
     ev = MsaEvictor(alpha=alpha, beta=beta, tau0=tau0, k5=k5, c0=c0)
     t_now = 3000.0
