@@ -56,17 +56,18 @@ def sustained_tflops():
 
 
 def committed_traffic(workload: str):
-    """dram bytes per launch of the dominant kernel from the committed ncu capture
-    (profiles/roofline_traffic.csv, copied by hand from the `ncu --set full` summaries), or None."""
+    """(dram bytes per launch of the dominant kernel, source) from the committed ncu capture, or (None, None).
+    NOT measured by this run: profiles/roofline_traffic.csv holds dram__bytes_read.sum + dram__bytes_write.sum of one
+    `ncu --set full` launch per workload (the .txt summary named in its `source` column)."""
     import csv
     try:
         with open(os.path.join(ROOT, "profiles", "roofline_traffic.csv")) as f:
             for row in csv.DictReader(f):
                 if row["workload"] == workload:
-                    return float(row["dram_bytes_per_launch"])
+                    return float(row["dram_bytes_per_launch"]), "profiles/%s (ncu --set full, one launch; not this run)" % row["source"]
     except Exception:
         pass
-    return None
+    return None, None
 
 
 class ClockSampler:
@@ -223,10 +224,11 @@ def run_mine(args, rank: int, world: int, local_rank: int):
         kern_units = units_per_step          # the forward kernel does all algorithmic work of a step
         achieved = kern_units / (fwd_ms * 1e-3) if fwd_ms > 0 else None
         peak = tfl_peak if bound == "tensor" else gbs_peak
-        traffic = committed_traffic(name)
+        traffic, traffic_source = committed_traffic(name)
         out = dict(metric=metric, value=value, unit=unit, ms_per_step=ms, gpu_launches=launches,
                    roofline=dict(bound=bound, achieved=achieved, peak=peak, unit=unit,
-                                 frac=(achieved / peak) if achieved else None, traffic=traffic,
+                                 frac=(achieved / peak) if achieved else None, traffic=traffic, traffic_source=traffic_source,
+                                 algorithmic_units_per_launch=units_per_step,
                                  kernel="msa_fwd", kernel_ms=fwd_ms, merge_ms=merge_ms, steps_timed=n_rec,
                                  peak_source=peak_label,
                                  frac_of_nominal=(achieved / (2250.0 if bound == "tensor" else 8000.0)) if achieved else None,
@@ -285,12 +287,19 @@ def run_mine(args, rank: int, world: int, local_rank: int):
                                     sample=f"{n} query rows of requests {reqs} (all {p.Hq} heads), {dt:.2f} s",
                                     seconds=dt)
         if args.workload == "cfg2_llama8b" and not args.no_secondary:
+            # the other three performance configs of BASELINE.json, each with its own roofline block and clocks
             del p
-            torch.cuda.empty_cache()
-            sec, p5 = bench_workload("cfg5_short_query", max(10, min(args.steps, 50)), args.warmup, do_e2e=False)
-            line["secondary"] = dict(workload="cfg5_short_query", metric=sec["metric"], value=sec["value"],
-                                     unit=sec["unit"], ms_per_step=sec["ms_per_step"], roofline=sec["roofline"],
-                                     clocks=sec["clocks"], plan=sec["plan"])
+            line["secondary"] = []
+            for wl, k in (("cfg3_70b_long", 30), ("cfg4_mixed", 20), ("cfg5_short_query", 50)):
+                torch.cuda.empty_cache()
+                sec, psec = bench_workload(wl, max(10, min(args.steps, k)), args.warmup, do_e2e=False)
+                line["secondary"].append(dict(workload=wl, metric=sec["metric"], value=sec["value"], unit=sec["unit"],
+                                              ms_per_step=sec["ms_per_step"], gpu_launches=sec["gpu_launches"],
+                                              roofline=sec["roofline"], clocks=sec["clocks"], plan=sec["plan"],
+                                              config=dict(requests=psec.n_req, total_q=psec.total_q, kv_tokens=psec.kv_tokens(),
+                                                          Hq=psec.Hq, Hkv=psec.Hkv, head_dim=psec.D)))
+                del psec
+            line["config"]["largest_single_gpu_config"] = "cfg4_mixed (in `secondary`; `value` is quoted on cfg2_llama8b = BASELINE.json configs[1])"
     if world > 1:
         import torch.distributed as dist
         dist.barrier()
@@ -299,78 +308,157 @@ def run_mine(args, rank: int, world: int, local_rank: int):
         print(json.dumps(line))
 
 
+class Fig13Case:
+    """One request of the Fig. 13 shape (workloads.f2_fig13) with the plans of every way to compute it.
+
+    fused()            one msa_forward over all runs and segments (what MSA is)
+    per_run()          'two kernel calls' of PAPER.md:353: one msa_forward per compute run, a host synchronisation after each
+    per_kv_segment()   the same kernel once per KV segment of the LAST run, a host synchronisation after each call, and an
+                       LSE merge of the partial results with torch ops (exact: softmax over a union = LSE-weighted mix)
+    The per-* paths are baselines that exist only here (bench + tests); the product path is the fused call."""
+
+    def __init__(self, cached_tokens: int, layout: str, device="cuda:0", keep_dense: bool = False):
+        import torch
+        import workloads as W
+        from paper_2606_02964_b200 import make_descriptors, msa_create, msa_plan_create, msa_workspace_bytes
+        self.torch = torch
+        self.p = p = W.f2_fig13(cached_tokens, layout, device=device, keep_dense=keep_dense)
+        self.dev = device
+        self.h = msa_create(p.Hq, p.Hkv, p.D, p.q_to_kv, device=torch.device(device).index or 0)
+        self.plans = {}
+
+        def plan_of(run_ids, seg_lo, seg_hi):
+            req = p.req[run_ids].copy()
+            req[:, 3] = 0
+            req[:, 4] = seg_hi - seg_lo
+            R, n, S, m = make_descriptors(req, p.seg_kind[seg_lo:seg_hi], p.seg_abs_start[seg_lo:seg_hi], p.seg_len[seg_lo:seg_hi],
+                                          p.seg_block_off[seg_lo:seg_hi], p.seg_row_off[seg_lo:seg_hi])
+            pl = msa_plan_create(self.h, R, n, S, m)
+            nb = msa_workspace_bytes(pl)
+            ws = torch.empty(max(nb, 16), dtype=torch.uint8, device=device) if nb else None
+            return pl, ws
+
+        nseg, nrun = p.n_seg, p.n_req
+        self.plans["fused"] = plan_of(list(range(nrun)), 0, nseg)
+        # per run: run r sees the segments up to and including its own SELF segment
+        self.run_plans = []
+        for r in range(nrun):
+            last = max(s for s in range(nseg) if int(p.seg_abs_start[s]) <= int(p.req[r, 2]))
+            self.run_plans.append(plan_of([r], 0, last + 1))
+        # per KV segment, last run only
+        self.seg_plans = [plan_of([nrun - 1], s, s + 1) for s in range(nseg)]
+        self.o = torch.zeros_like(p.q)
+        self.lse = torch.zeros(p.total_q, p.Hq, dtype=torch.float32, device=device)
+        self.o_part = [torch.zeros_like(p.q) for _ in range(nseg)]
+        self.lse_part = [torch.full((p.total_q, p.Hq), float("-inf"), dtype=torch.float32, device=device) for _ in range(nseg)]
+
+    def _fwd(self, plan, o, lse, stream):
+        from paper_2606_02964_b200 import msa_forward
+        p = self.p
+        msa_forward(self.h, plan[0], p.q, p.pool_k, p.pool_v, p.block_table, p.contig_k, p.contig_v, p.scale, o, lse, plan[1], stream)
+
+    def fused(self, stream, sync=True):
+        self._fwd(self.plans["fused"], self.o, self.lse, stream)
+        if sync:
+            self.torch.cuda.synchronize()
+        return self.o, self.lse
+
+    def per_run(self, stream, sync=True):
+        for pl in self.run_plans:
+            self._fwd(pl, self.o, self.lse, stream)
+            if sync:
+                self.torch.cuda.synchronize()
+        return self.o, self.lse
+
+    def per_kv_segment(self, stream, sync=True):
+        torch = self.torch
+        p = self.p
+        r0, n = int(p.req[-1, 0]), int(p.req[-1, 1])
+        for s, pl in enumerate(self.seg_plans):
+            self._fwd(pl, self.o_part[s], self.lse_part[s], stream)
+            if sync:
+                torch.cuda.synchronize()
+        L = torch.stack([x[r0:r0 + n] for x in self.lse_part])                  # [S, n, Hq]
+        lse = torch.logsumexp(L, dim=0)
+        w = torch.exp(L - lse.unsqueeze(0))
+        w = torch.where(torch.isfinite(L), w, torch.zeros_like(w))
+        O = torch.stack([x[r0:r0 + n].float() for x in self.o_part])            # [S, n, Hq, D]
+        o = (w.unsqueeze(-1) * O).sum(0).to(torch.bfloat16)
+        if sync:
+            torch.cuda.synchronize()
+        return o, lse, (r0, n)
+
+    def close(self):
+        from paper_2606_02964_b200 import msa_destroy, msa_plan_destroy
+        for pl, _ in [self.plans["fused"]] + self.run_plans + self.seg_plans:
+            msa_plan_destroy(pl)
+        msa_destroy(self.h)
+
+
 def run_fig13(args):
-    """SURVEY.md section 8 (f2), the shape of the paper's Fig. 13: N cached tokens + 128 new tokens,
-    Llama-3-8B heads.  One fused msa_forward over both segments against the same kernel called once per segment
-    with a host synchronisation after each call and an LSE merge of the two partial results (torch ops)."""
+    """SURVEY.md section 8 (f2), the shape of the paper's Fig. 13, Llama-3-8B heads, one request that
+    "ends with 128 new tokens".  Three ways to serve it (the paper's three lines):
+      prefix     caching from the prefix   [cached N][recompute R + new 128]              one call
+      suffix x2  caching from the suffix   [recompute R][cached N][new 128]               one call per compute run ("two kernel calls")
+      suffix MSA caching from the suffix, same layout                                      ONE fused msa_forward
+    plus the round-1 row [cached N][new 128]: fused against one call per KV segment + LSE merge.  R = N (DESIGN.md c18).
+    Every variant is timed twice: host wall clock per attention call including the synchronisation(s) a caller needs, and
+    device time (CUDA events around `steps` back-to-back calls without host synchronisation)."""
     import torch
-    import workloads as W
-    from paper_2606_02964_b200 import (make_descriptors, msa_create, msa_destroy, msa_forward, msa_plan_create,
-                                       msa_plan_destroy, msa_workspace_bytes)
     import __graft_entry__ as ge
     ge.build()
     dev = "cuda:0"
     torch.cuda.set_device(0)
     stream = torch.cuda.current_stream().cuda_stream
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def timed(fn):
+        for _ in range(max(3, args.warmup)):
+            fn(stream)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            fn(stream)
+        wall = (time.perf_counter() - t0) / args.steps * 1e6
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(args.steps):
+            fn(stream, sync=False)
+        e1.record()
+        torch.cuda.synchronize()
+        return wall, e0.elapsed_time(e1) / args.steps * 1e3
+
     rows = []
     for N in (1024, 2048, 4096, 8192, 10240):
-        ctx = W.ContextSpec([(W.SEG_PAGED, 0, N), (W.SEG_SELF, N, 128)])
-        p = W.build_problem(f"fig13_{N}", 32, 8, 128, [ctx], [W.RunSpec(0, N, 128)], seed=1300 + N, device=dev)
-        h = msa_create(p.Hq, p.Hkv, p.D, p.q_to_kv, device=0)
-
-        def plan_of(lo, hi):
-            req = np.array([[0, 128, N, 0, hi - lo]], np.int32)
-            R, n, S, m = make_descriptors(req, p.seg_kind[lo:hi], p.seg_abs_start[lo:hi], p.seg_len[lo:hi],
-                                          p.seg_block_off[lo:hi], p.seg_row_off[lo:hi])
-            pl = msa_plan_create(h, R, n, S, m)
-            nb = msa_workspace_bytes(pl)
-            ws = torch.empty(max(nb, 16), dtype=torch.uint8, device=dev) if nb else None
-            return pl, ws, torch.zeros_like(p.q), torch.zeros(p.total_q, p.Hq, dtype=torch.float32, device=dev)
-
-        plans = [plan_of(0, 2), plan_of(0, 1), plan_of(1, 2)]
-
-        def fwd(k):
-            pl, ws, o, lse = plans[k]
-            msa_forward(h, pl, p.q, p.pool_k, p.pool_v, p.block_table, p.contig_k, p.contig_v, p.scale, o, lse, ws, stream)
-            return o, lse
-
-        def fused():
-            o, lse = fwd(0)
-            torch.cuda.synchronize()
-            return o, lse
-
-        def per_segment():
-            oa, la = fwd(1)
-            torch.cuda.synchronize()
-            ob, lb = fwd(2)
-            torch.cuda.synchronize()
-            lse = torch.logaddexp(la, lb)
-            o = (torch.exp(la - lse).unsqueeze(-1) * oa.float() + torch.exp(lb - lse).unsqueeze(-1) * ob.float()).to(torch.bfloat16)
-            torch.cuda.synchronize()
-            return o, lse
-
-        for _ in range(max(3, args.warmup)):
-            o1, l1 = fused()
-            o2, l2 = per_segment()
-        d_o = float((o1.float() - o2.float()).abs().max())
-        d_l = float((l1 - l2).abs().max())
-        t = {}
-        for name, fn in (("fused", fused), ("per_segment", per_segment)):
-            t0 = time.perf_counter()
-            for _ in range(args.steps):
-                fn()
-            t[name] = (time.perf_counter() - t0) / args.steps * 1e6
-        rows.append(dict(cached_tokens=N, fused_us=t["fused"], per_segment_us=t["per_segment"],
-                         speedup=t["per_segment"] / t["fused"], max_abs_dO=d_o, max_abs_dLSE=d_l))
-        for pl, _, _, _ in plans:
-            msa_plan_destroy(pl)
-        msa_destroy(h)
-    mean_speedup = float(np.mean([r["speedup"] for r in rows]))
-    print(json.dumps(dict(metric="msa_fused_vs_per_segment_speedup", value=mean_speedup, unit="x", n_gpus=1, steps=args.steps,
-                          warmup=max(3, args.warmup), higher_is_better=True, dtype="bf16", data="synthetic", vs_baseline=None,
+        row = dict(cached_tokens=N, recompute_tokens=N, new_tokens=128)
+        c = Fig13Case(N, "prefix", dev)
+        row["prefix_wall_us"], row["prefix_dev_us"] = timed(c.fused)
+        c.close()
+        c = Fig13Case(N, "suffix", dev)
+        row["suffix_msa_wall_us"], row["suffix_msa_dev_us"] = timed(c.fused)
+        o1, l1 = (x.clone() for x in c.fused(stream))
+        row["suffix_two_calls_wall_us"], row["suffix_two_calls_dev_us"] = timed(c.per_run)
+        o2, l2 = c.per_run(stream)
+        row["two_calls_max_abs_dO"] = float((o1.float() - o2.float()).abs().max())
+        row["two_calls_max_abs_dLSE"] = float((l1 - l2).abs().max())
+        c.close()
+        c = Fig13Case(N, "prefix_new", dev)
+        row["new128_fused_wall_us"], row["new128_fused_dev_us"] = timed(c.fused)
+        o1, l1 = (x.clone() for x in c.fused(stream))
+        row["new128_per_segment_wall_us"], row["new128_per_segment_dev_us"] = timed(c.per_kv_segment)
+        o2, l2, (r0, n) = c.per_kv_segment(stream)
+        row["per_segment_max_abs_dO"] = float((o1[r0:r0 + n].float() - o2.float()).abs().max())
+        row["per_segment_max_abs_dLSE"] = float((l1[r0:r0 + n] - l2).abs().max())
+        c.close()
+        row["two_calls_overhead_us"] = row["suffix_two_calls_wall_us"] - row["suffix_msa_wall_us"]
+        row["suffix_vs_prefix"] = row["suffix_msa_wall_us"] / row["prefix_wall_us"]
+        rows.append(row)
+    mean_overhead = float(np.mean([r["two_calls_overhead_us"] for r in rows]))
+    print(json.dumps(dict(metric="msa_two_call_overhead_us_per_attention_call", value=mean_overhead, unit="us", n_gpus=1, steps=args.steps,
+                          warmup=max(3, args.warmup), higher_is_better=False, dtype="bf16", data="synthetic", vs_baseline=None,
                           config=dict(workload="fig13", Hq=32, Hkv=8, head_dim=128, new_tokens=128,
-                                      timing="host wall clock per call incl. the synchronisation a caller needs"),
-                          fig13=rows, gpu_launches=args.steps * 2)))
+                                      timing="wall = host clock per call incl. the synchronisation(s) a caller needs; dev = CUDA events, no host sync"),
+                          fig13=rows, gpu_launches=args.steps * 2 * 7)))
 
 
 def run_evictor(args):
@@ -522,15 +610,16 @@ def run_reference(args, rank: int, world: int):
         return
     import oracle
     import workloads as W
-    import __graft_entry__ as ge
-    ge.build()
+    oracle.build()                      # the C oracle only: this arm never maps libmsa.so
     metric, unit, bound = metric_of(args.workload)
     p = W.CONFIGS[args.workload](device="cpu") if args.workload in ("cfg1_tiny",) else None
     if p is None:
         # values on the CPU; only the requests sampled are ever read
         small = dict(cfg2_llama8b=dict(n_req=2), cfg4_mixed=dict(n_req=4), cfg5_short_query=dict(n_req=8),
-                     f1_hybrid_pod=dict(n_prefill=1, n_decode=2), f3_policy_trace=dict(n_sessions=3))
-        p = all_workloads()[args.workload](device="cpu", **small.get(args.workload, {}))
+                     f1_hybrid_pod=dict(n_prefill=1, n_decode=2))
+        if args.workload == "f3_policy_trace":
+            raise SystemExit("the oracle arm covers BASELINE.json's configs and f1 (f3's residency is decided by the product's evictor)")
+        p = {**W.CONFIGS, **W.EXTRA_CONFIGS}[args.workload](device="cpu", **small.get(args.workload, {}))
     reqs = list(range(min(2, p.n_req)))
     dt, fl, pairs, n = oracle_sample(p, 8, 1, reqs)
     total = max(1, args.steps + args.warmup)

@@ -30,7 +30,8 @@ def gpu_forward(p):
         return o.float().cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64), s.info
 
 
-def compare(p, o, lse, row_req=None, row_idx=None, strict=True):
+def compare(p, o, lse, row_req=None, row_idx=None, strict=True, v_scale=1.0):
+    """v_scale: the O tolerances are stated for V ~ N(0,1); the error of O is linear in V, so a test that scales V scales them."""
     O, LSE = oracle.forward_problem(p, row_req, row_idx)
     if row_req is not None:
         g = p.req[row_req, 0] + row_idx
@@ -42,10 +43,10 @@ def compare(p, o, lse, row_req=None, row_idx=None, strict=True):
     d_o = np.abs(o - O)
     d_l = np.abs(lse[fin] - LSE[fin]) if fin.any() else np.zeros(1)
     if strict:
-        assert d_o.max() <= TOL_O_MAX, f"max|dO|={d_o.max()}"
+        assert d_o.max() <= TOL_O_MAX * v_scale, f"max|dO|={d_o.max()}"
     else:
-        assert np.all(d_o <= TOL_O_MAX * np.maximum(1.0, np.abs(O) / 2.0)), f"max|dO|={d_o.max()}"
-    assert d_o.mean() <= TOL_O_MEAN, f"mean|dO|={d_o.mean()}"
+        assert np.all(d_o <= TOL_O_MAX * v_scale * np.maximum(1.0, np.abs(O) / (2.0 * v_scale))), f"max|dO|={d_o.max()}"
+    assert d_o.mean() <= TOL_O_MEAN * v_scale, f"mean|dO|={d_o.mean()}"
     assert d_l.max() <= TOL_LSE, f"max|dLSE|={d_l.max()}"
     return d_o.max(), d_o.mean(), d_l.max()
 
@@ -203,6 +204,131 @@ def test_forward_host_matches_forward_and_error_codes():
             msa_forward(s.h, s.plan, mis, p.pool_k, p.pool_v, p.block_table, p.contig_k, p.contig_v, p.scale,
                         s.o, s.lse, s.workspace)
         assert e.value.status == MSA_ERR_MISALIGNED
+
+
+def test_score_jump_just_under_the_fast_path_guard_with_large_v():
+    """A tile whose scores sit ~60 log2 units above the stale reference (inside the 2^64 guard) takes the fast path with
+    P up to 2^60; with |V| ~ 4 over hundreds of keys O += P V must still stay far from fp32 overflow, and the power-of-two
+    rescale that follows must bring it back exactly (the old 2^120 guard left no headroom)."""
+    # scores ~ 115 nats (std 12) for the late keys, x * 115 for keys 0..255: jumps of ~ +58 and ~ +125 log2 units between tiles
+    for jump_scale, lo in ((0.65, 70.0), (0.25, 70.0)):
+        p = _contig_problem(900, 70, 43)
+        p.q.copy_((p.q.float().abs() * 16).to(torch.bfloat16))
+        k = p.contig_k.float().abs()
+        k[:256] *= jump_scale
+        p.contig_k.copy_(k.to(torch.bfloat16))
+        p.contig_v.copy_((p.contig_v.float() * 4).to(torch.bfloat16))
+        o, lse, _ = gpu_forward(p)
+        assert np.all(np.isfinite(o)) and lse.min() > lo
+        compare(p, o, lse, strict=False, v_scale=4.0)
+
+
+def test_nan_in_one_requests_valid_kv_stays_in_that_request():
+    """One request's VALID K/V holds NaN / Inf (a diverged sequence).  Every other request must come out bit-identical
+    to the run without the poison: masked P = 0 never meets another request's stale rows (the V loader zeroes the rows
+    TMA does not write), whatever the persistent schedule puts on the same CTA before it."""
+    kw = dict(seed=301, n_req=6, Hq=8, Hkv=2, D=128, max_ctx=900, max_q=70, min_ctx=300, device=DEV)
+    p = W.random_problem(**kw)
+    o0, l0, _ = gpu_forward(p)
+    victim = 2
+    sb, sc = int(p.req[victim, 3]), int(p.req[victim, 4])
+    shared = set()
+    for r in range(p.n_req):
+        if r != victim:
+            shared.update(range(int(p.req[r, 3]), int(p.req[r, 3]) + int(p.req[r, 4])))
+    assert not shared.intersection(range(sb, sb + sc)), "the victim must own its segments"
+    bad = torch.tensor([float("nan"), float("inf"), float("-inf")], dtype=torch.bfloat16, device=DEV)
+    for s_ in range(sb, sb + sc):
+        n = int(p.seg_len[s_])
+        if int(p.seg_kind[s_]) == SEG_PAGED:
+            ids = torch.from_numpy(p.block_table_np[int(p.seg_block_off[s_]):int(p.seg_block_off[s_]) + (n + 15) // 16].astype(np.int64)).to(DEV)
+            for pool in (p.pool_k, p.pool_v):
+                blk = pool[ids]                                   # [nb, 16, Hkv, D]
+                blk.view(-1)[::7] = bad[0]
+                blk.view(-1)[3::11] = bad[1]
+                pool[ids] = blk
+        else:
+            r0 = int(p.seg_row_off[s_])
+            for arena in (p.contig_k, p.contig_v):
+                arena[r0:r0 + n].view(-1)[::5] = bad[0]
+                arena[r0:r0 + n].view(-1)[2::13] = bad[2]
+    o1, l1, _ = gpu_forward(p)
+    for r in range(p.n_req):
+        a, n = int(p.req[r, 0]), int(p.req[r, 1])
+        if r == victim:
+            continue            # non-finite inputs: that request's own rows are unspecified (DESIGN.md section 2, c19)
+        assert np.array_equal(o0[a:a + n], o1[a:a + n]) and np.array_equal(l0[a:a + n], l1[a:a + n]), f"request {r} changed"
+
+
+def test_many_pointer_sets_through_one_handle():
+    """The handle keeps encoded tensor maps per (q, pool, arena) pointer set (least recently used of 64 replaced):
+    more than 64 distinct q buffers through one handle, revisited, must each give the result of a fresh handle."""
+    p = W.random_problem(77, n_req=2, Hq=4, Hkv=2, D=64, max_ctx=300, max_q=40, device=DEV)
+    with MsaSession(p) as s:
+        o_ref, l_ref = (x.clone() for x in s.forward())
+        torch.cuda.synchronize()
+        qs = [p.q.clone() for _ in range(70)]
+        for rnd in range(2):
+            for i, q in enumerate(qs):
+                s.o.zero_()
+                msa_forward(s.h, s.plan, q, p.pool_k, p.pool_v, p.block_table, p.contig_k, p.contig_v, p.scale, s.o, s.lse, s.workspace)
+                torch.cuda.synchronize()
+                assert torch.equal(s.o, o_ref) and torch.equal(s.lse, l_ref), (rnd, i)
+
+
+@pytest.mark.skipif(torch.cuda.device_count() < 2, reason="needs a second GPU to make another device current")
+def test_forward_with_another_device_current():
+    """msa_forward / msa_kv_append make the handle's device current for the call and restore the caller's."""
+    p = W.random_problem(78, n_req=2, Hq=4, Hkv=2, D=128, max_ctx=300, max_q=40, device=DEV)
+    with MsaSession(p, device=0) as s:
+        o_ref, l_ref = (x.clone() for x in s.forward())
+        torch.cuda.synchronize()
+        torch.cuda.set_device(1)
+        try:
+            s.o.zero_()
+            s.forward(torch.cuda.current_stream(0).cuda_stream)
+            torch.cuda.synchronize(0)
+            assert torch.cuda.current_device() == 1
+            assert torch.equal(s.o, o_ref) and torch.equal(s.lse, l_ref)
+        finally:
+            torch.cuda.set_device(0)
+
+
+# ------------------------------------------------------------------ SURVEY 8 (f2): Fig. 13 layouts, every way to serve them
+@pytest.mark.parametrize("layout,N", [("prefix_new", 1024), ("suffix", 1024), ("suffix", 2048), ("prefix", 1024)])
+def test_f2_fig13_fused_per_run_and_per_segment_paths_against_the_oracle(layout, N):
+    """The fused call, the 'two kernel calls' path (one msa_forward per compute run) and the per-KV-segment + LSE-merge
+    path of bench.py --workload fig13 are each compared with the ORACLE (not with one another)."""
+    from bench import Fig13Case
+    c = Fig13Case(N, layout, DEV)
+    try:
+        p = c.p
+        stream = torch.cuda.current_stream().cuda_stream
+        rows = sorted(set(zip(*[x.tolist() for x in W.pick_rows(p, 40, 5)])))
+        rr = np.asarray([r for r, _ in rows], np.int32)
+        ii = np.asarray([i for _, i in rows], np.int32)
+        O, LSE = oracle.forward_problem(p, rr, ii)
+        g = p.req[rr, 0] + ii
+
+        def check(o, lse, sel=None, off=0):
+            o = o.float().cpu().numpy().astype(np.float64)
+            lse = lse.cpu().numpy().astype(np.float64)
+            idx = np.arange(len(g)) if sel is None else sel
+            d_o = np.abs(o[g[idx] - off] - O[idx])
+            d_l = np.abs(lse[g[idx] - off] - LSE[idx])
+            assert d_o.max() <= TOL_O_MAX and d_o.mean() <= TOL_O_MEAN and d_l.max() <= TOL_LSE, (d_o.max(), d_o.mean(), d_l.max())
+
+        o, lse = c.fused(stream)
+        check(o, lse)
+        c.o.zero_()
+        c.lse.zero_()
+        o, lse = c.per_run(stream)
+        check(o, lse)
+        o, lse, (r0, n) = c.per_kv_segment(stream)                      # rows of the last run only
+        sel = np.flatnonzero(rr == p.n_req - 1)
+        check(o, lse, sel, off=r0)
+    finally:
+        c.close()
 
 
 # ------------------------------------------------------------------ configs 2-5 at full size
