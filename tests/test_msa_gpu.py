@@ -294,6 +294,57 @@ def test_forward_with_another_device_current():
             torch.cuda.set_device(0)
 
 
+# ------------------------------------------------------------------ stand-ins for compute-sanitizer (closed on this GPU pool)
+def test_outputs_and_workspace_stay_inside_their_buffers():
+    """memcheck stand-in: O, LSE and the split-KV workspace sit between canary regions that must come back untouched,
+    on a problem with split items, ragged tails, short runs and partial q tiles."""
+    ctxs = [ContextSpec([(SEG_PAGED, 0, 3000), (SEG_CONTIG, 3000, 1777), (SEG_PAGED, 4777, 1501), (SEG_SELF, 6278, 45)]),
+            ContextSpec([(SEG_PAGED, 0, 333), (SEG_SELF, 333, 3)]),
+            ContextSpec([(SEG_CONTIG, 5, 700), (SEG_SELF, 705, 131)])]
+    p = build_problem("canary", 8, 2, 128, ctxs, [RunSpec(0, 6278, 45), RunSpec(1, 333, 3), RunSpec(2, 705, 131)], seed=9, device=DEV,
+                      keep_dense=True)
+    PAD = 4096
+    with MsaSession(p) as s:
+        assert s.info["num_split_items"] > 0
+        n_o, n_l = p.q.numel(), p.total_q * p.Hq
+        big_o = torch.full((n_o + 2 * PAD,), -7.0, dtype=torch.bfloat16, device=DEV)
+        big_l = torch.full((n_l + 2 * PAD,), -7.0, dtype=torch.float32, device=DEV)
+        nws = 0 if s.workspace is None else s.workspace.numel()
+        big_w = torch.full((nws + 2 * PAD,), 0x5A, dtype=torch.uint8, device=DEV)
+        o = big_o[PAD:PAD + n_o].view_as(p.q)
+        lse = big_l[PAD:PAD + n_l].view(p.total_q, p.Hq)
+        ws = big_w[PAD:PAD + nws] if nws else None
+        msa_forward(s.h, s.plan, p.q, p.pool_k, p.pool_v, p.block_table, p.contig_k, p.contig_v, p.scale, o, lse, ws)
+        torch.cuda.synchronize()
+        for big, n in ((big_o, n_o), (big_l, n_l)):
+            assert bool((big[:PAD] == -7.0).all()) and bool((big[PAD + n:] == -7.0).all())
+        assert bool((big_w[:PAD] == 0x5A).all()) and bool((big_w[PAD + nws:] == 0x5A).all())
+        compare(p, o.float().cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64), strict=False)
+
+
+def test_bit_identical_under_timing_noise():
+    """racecheck stand-in: the same launch, repeated while another stream keeps the SMs, L2 and HBM busy with unrelated work
+    of varying size, must give bit-identical O and LSE every time (the 28-mbarrier pipeline has no timing-dependent result)."""
+    p = W.random_problem(55, n_req=8, Hq=8, Hkv=2, D=128, max_ctx=5000, max_q=300, min_ctx=1500, device=DEV)
+    side = torch.cuda.Stream()
+    a = torch.randn(2048, 2048, device=DEV)
+    big = torch.empty(64 << 20, dtype=torch.uint8, device=DEV)
+    with MsaSession(p) as s:
+        o_ref, l_ref = (x.clone() for x in s.forward())
+        torch.cuda.synchronize()
+        for it in range(12):
+            with torch.cuda.stream(side):
+                for _ in range(1 + it % 4):
+                    (a @ a).sum()
+                    big[: (8 + 5 * it) << 20].fill_(it)
+            s.o.zero_()
+            s.lse.zero_()
+            s.forward()
+            torch.cuda.synchronize()
+            assert torch.equal(s.o, o_ref) and torch.equal(s.lse, l_ref), it
+        compare(p, o_ref.float().cpu().numpy().astype(np.float64), l_ref.cpu().numpy().astype(np.float64), strict=False)
+
+
 # ------------------------------------------------------------------ SURVEY 8 (f2): Fig. 13 layouts, every way to serve them
 @pytest.mark.parametrize("layout,N", [("prefix_new", 1024), ("suffix", 1024), ("suffix", 2048), ("prefix", 1024)])
 def test_f2_fig13_fused_per_run_and_per_segment_paths_against_the_oracle(layout, N):
