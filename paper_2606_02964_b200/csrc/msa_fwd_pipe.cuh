@@ -89,12 +89,14 @@ enum PipeBar : int {
     kBarPLo = 14,        // [2] P of keys 0-63 in TMEM
     kBarOFull = 16,      // [2]
     kBarOFree = 18,      // [2]
-    kBarStFull = 20,     // [2]
+    // 20, 21: free (the stats hand-off is a named barrier: the epilogue warps wait for a whole unit)
     kBarStFree = 22,     // [2]
     kBarPQ2 = 24,        // [2] P of keys 64-95 in TMEM
     kBarPQ3 = 26,        // [2] P of keys 96-127 in TMEM
     kBarCount = 28
 };
+
+constexpr uint32_t kNamedStFull = 1;   // named barriers 1, 2: (l, ref) of chain 0 / 1 are in shared memory (128 + 128 threads)
 
 struct RingPos {
     uint32_t slot, phase;
@@ -145,7 +147,6 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             mbar_init(bar(kBarPQ3 + c), 4);
             mbar_init(bar(kBarOFull + c), 1);
             mbar_init(bar(kBarOFree + c), 4);
-            mbar_init(bar(kBarStFull + c), 4);
             mbar_init(bar(kBarStFree + c), 4);
         }
         fence_mbar_init();
@@ -165,7 +166,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
 
     if (warp < 8) {
         // =========================================================== softmax warpgroups
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 192;");
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 184;");
         const int c = warp >> 2;                       // chain
         const int row = threadIdx.x & 127;
         const int g = row / R, t = row - g * R;
@@ -314,8 +315,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             mbar_wait(bar(kBarStFree + c), ph_stfree);
             ph_stfree ^= 1;
             stats[c * kTileM + row] = make_float2(l, ref);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar(kBarStFull + c));
+            named_bar_arrive(kNamedStFull + c, 256);
         }
 #if defined(MSA_PROF) && MSA_PROF != 2
         if ((threadIdx.x & 127) == 0) {
@@ -328,7 +328,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
         const int row = threadIdx.x & 127;
         const int g = row / R, t = row - g * R;
         const uint32_t trow = tmem + (static_cast<uint32_t>((warp & 3) * 32) << 16);
-        uint32_t ph_st[2] = {0, 0}, ph_o[2] = {0, 0};
+        uint32_t ph_o[2] = {0, 0};
         for (int u = u_begin; u < u_end; ++u) {
             const WorkUnit wu = P.units[u];
             const int n = wu.tile_end - wu.tile_begin;
@@ -347,8 +347,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     act1 = pair ? (qt == 1) : (n >= 2);
                     float l0 = 0.f, m0 = -INFINITY, l1 = 0.f, m1 = -INFINITY;
                     if (act0) {
-                        mbar_wait(bar(kBarStFull + 0), ph_st[0]);
-                        ph_st[0] ^= 1;
+                        named_bar_sync(kNamedStFull + 0, 256);     // blocked in hardware until the chain's softmax warps are done
                         const float2 st = stats[0 * kTileM + row];
                         l0 = st.x;
                         m0 = st.y;
@@ -356,8 +355,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                         if (lane == 0) mbar_arrive(bar(kBarStFree + 0));
                     }
                     if (act1) {
-                        mbar_wait(bar(kBarStFull + 1), ph_st[1]);
-                        ph_st[1] ^= 1;
+                        named_bar_sync(kNamedStFull + 1, 256);     // blocked in hardware until the chain's softmax warps are done
                         const float2 st = stats[1 * kTileM + row];
                         l1 = st.x;
                         m1 = st.y;
@@ -446,7 +444,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             }
         }
     } else {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
         if (warp == 12 || warp == 14) {
             // ======================================================= loader warps (12: Q and K, 14: V)
             // Ring sequence: K of the CTA's i-th KV tile is entry 2i, its V entry 2i+1.
@@ -610,13 +608,22 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                 rv.advance2(C::kStages);
                 return slot;
             };
+            // Descriptors: only the 14-bit start-address field (address >> 4) differs between the operands of one
+            // tile, and it never carries out of its field (shared memory ends below 256 KB), so a tile's descriptor
+            // is formed once and every MMA adds a compile-time constant to it: the issuing thread shares its SM
+            // sub-partition with two softmax warps, and every instruction it does not need shortens the P -> S round trip.
+            const uint64_t q_desc = make_smem_desc(sQ, 16, 1024);
+            const uint64_t k_desc = make_smem_desc(sRing, 16, 1024);
+            const uint64_t v_desc = make_smem_desc(sRing, C::kHalfBytes, 1024);
+            constexpr uint64_t kTileStep = C::kTileBytes >> 4;
             auto qk = [&](int c, int qtile, uint32_t kslot) {
-                const uint32_t qa = sQ + qtile * C::kTileBytes, ka = sRing + kslot * C::kTileBytes;
+                const uint64_t qd = q_desc + qtile * kTileStep, kd = k_desc + kslot * kTileStep;
+                const uint32_t d_tmem = tmem + C::kColS + c * C::kChainCols;
 #pragma unroll
                 for (int k = 0; k < D / 16; ++k) {
-                    const uint32_t off = (k >> 2) * C::kHalfBytes + (k & 3) * 32;
-                    umma_ss(tmem + C::kColS + c * C::kChainCols, make_smem_desc(qa + off, 16, 1024),
-                            make_smem_desc(ka + off, 16, 1024), idesc_s, k > 0);
+                    constexpr uint32_t kHalfStep = C::kHalfBytes >> 4;
+                    const uint64_t off = (k >> 2) * kHalfStep + (k & 3) * 2;          // ((k>>2)*kHalfBytes + (k&3)*32) >> 4
+                    umma_ss(d_tmem, qd + off, kd + off, idesc_s, k > 0);
                 }
                 umma_commit(bar(kBarSFull + c));
             };
@@ -635,21 +642,21 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     ph_ofree[c] ^= 1;
                 }
                 tc_fence_after();
-                const uint32_t va = sRing + vslot * C::kTileBytes;
+                const uint64_t vd = v_desc + vslot * kTileStep;
 #pragma unroll
                 for (int k = 0; k < kTileN / 32; ++k)
                     umma_ts(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
-                            make_smem_desc(va + k * (kBlock * 128), C::kHalfBytes, 1024), idesc_o, (!first || k > 0) ? 1u : 0u);
+                            vd + k * ((kBlock * 128) >> 4), idesc_o, (!first || k > 0) ? 1u : 0u);
             };
             auto pv_hi = [&](int c, uint32_t vslot) {
-                const uint32_t va = sRing + vslot * C::kTileBytes;
+                const uint64_t vd = v_desc + vslot * kTileStep;
                 mbar_wait(bar(kBarPQ2 + c), ph_p[c]);
                 PROF_TRACE(0, tr_step, 7 + 2 * c);
                 tc_fence_after();
 #pragma unroll
                 for (int k = kTileN / 32; k < 3 * kTileN / 64; ++k)
                     umma_ts(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
-                            make_smem_desc(va + k * (kBlock * 128), C::kHalfBytes, 1024), idesc_o, 1u);
+                            vd + k * ((kBlock * 128) >> 4), idesc_o, 1u);
                 mbar_wait(bar(kBarPQ3 + c), ph_p[c]);
                 PROF_TRACE(0, tr_step, 8 + 2 * c);
                 ph_p[c] ^= 1;
@@ -657,7 +664,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
 #pragma unroll
                 for (int k = 3 * kTileN / 64; k < kTileN / 16; ++k)
                     umma_ts(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
-                            make_smem_desc(va + k * (kBlock * 128), C::kHalfBytes, 1024), idesc_o, 1u);
+                            vd + k * ((kBlock * 128) >> 4), idesc_o, 1u);
             };
             auto pv = [&](int c, uint32_t vslot, bool first) {
                 pv_lo(c, vslot, first);

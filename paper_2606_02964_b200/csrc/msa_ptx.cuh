@@ -57,17 +57,18 @@ __device__ __forceinline__ bool mbar_try_wait_sleep(uint32_t bar, uint32_t parit
         : "memory");
     return ok != 0;
 }
-// Waits for the phase with the given parity to complete.  A wait that lasts longer than
-// ~2 s of SM clocks traps instead of hanging the device (a lost arrive is a bug, not a state).
+// Waits for the phase with the given parity to complete.  The loop is kept to a handful of instructions: a
+// sleeping warp is woken by every mbarrier event of its CTA, not only by its own, and each spurious wake-up takes
+// issue slots from the warps of its SM sub-partition that have work.  A wait that goes through ~2^27 wake-ups
+// (seconds) traps instead of hanging the device (a lost arrive is a bug, not a state).
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     if (mbar_try_wait(bar, parity)) return;
-    const long long t0 = clock64();
+    uint32_t spins = 0;
     while (!mbar_try_wait_sleep(bar, parity, 1000000u)) {
-        if (clock64() - t0 > 4000000000LL) __trap();
+        if (++spins == (1u << 27)) __trap();
     }
 }
-
 // ------------------------------------------------------------------ proxies / fences
 __device__ __forceinline__ void fence_proxy_async_smem()
 {
@@ -80,6 +81,16 @@ __device__ __forceinline__ void tc_fence_before()
 __device__ __forceinline__ void tc_fence_after()
 {
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+}
+// Named barriers (hardware, 16 per CTA): a warp blocked in bar.sync takes no issue slots at all, unlike a
+// warp that sleeps on an mbarrier and is woken by every mbarrier event of the CTA.
+__device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t nthreads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ void named_bar_arrive(uint32_t id, uint32_t nthreads)
+{
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 // ------------------------------------------------------------------ TMA
 // 2-D tiled load: box lands at smem `dst`, completes `bytes` on mbarrier `bar`.
