@@ -593,6 +593,32 @@ def run_kv_append(args):
     ms = e0.elapsed_time(e1) / args.steps
     nbytes = 2.0 * tokens * p.Hkv * p.D * 2 * 2
     gbs = nbytes / (ms * 1e-3) / 1e9
+    # the same write-back fused into the forward launch (msa_forward_writeback) against forward + msa_kv_append
+    from paper_2606_02964_b200 import (make_descriptors, msa_forward, msa_forward_writeback, msa_plan_create_writeback,
+                                       msa_plan_destroy, msa_workspace_bytes)
+    R, n, S, m = make_descriptors(p.req, p.seg_kind, p.seg_abs_start, p.seg_len, p.seg_block_off, p.seg_row_off)
+    plan = msa_plan_create_writeback(h, R, n, S, m, jobs)
+    nb = msa_workspace_bytes(plan)
+    ws = torch.empty(max(nb, 16), dtype=torch.uint8, device=dev) if nb else None
+    o = torch.zeros_like(p.q)
+    lse = torch.zeros(p.total_q, p.Hq, dtype=torch.float32, device=dev)
+
+    def timed(fn):
+        for _ in range(max(3, args.warmup)):
+            fn()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(args.steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / args.steps
+
+    fwd_only = timed(lambda: msa_forward(h, plan, p.q, pool_k, pool_v, bt, p.contig_k, p.contig_v, p.scale, o, lse, ws, stream))
+    two = timed(lambda: (msa_forward(h, plan, p.q, pool_k, pool_v, bt, p.contig_k, p.contig_v, p.scale, o, lse, ws, stream),
+                         msa_kv_append(h, ap, p.contig_k, p.contig_v, pool_k, pool_v, bt, stream)))
+    fused = timed(lambda: msa_forward_writeback(h, plan, p.q, pool_k, pool_v, bt, p.contig_k, p.contig_v, p.scale, o, lse, ws, stream))
+    msa_plan_destroy(plan)
     msa_append_plan_destroy(ap)
     msa_destroy(h)
     print(json.dumps(dict(metric="msa_kv_append_hbm_gbs", value=gbs, unit="GB/s", n_gpus=1, steps=args.steps, warmup=max(3, args.warmup),
@@ -600,6 +626,10 @@ def run_kv_append(args):
                           config=dict(workload="kv_append", tokens=tokens, jobs=len(jobs), bytes_per_step=nbytes,
                                       l2_policy="working set %.0f MB per step (read + write), larger than L2" % (nbytes / 1e6)),
                           clocks=clocks, gpu_launches=args.steps,
+                          fused=dict(forward_only_ms=fwd_only, forward_plus_kv_append_ms=two, forward_writeback_ms=fused,
+                                     writeback_cost_ms=fused - fwd_only, separate_cost_ms=two - fwd_only,
+                                     note="cfg2 batch: msa_forward_writeback stores the recomputed + own K/V from the forward "
+                                          "kernel's shared-memory tiles (no second read of the arena, no second launch)"),
                           roofline=dict(bound="hbm", achieved=gbs, peak=gbs_peak, unit="GB/s", frac=gbs / gbs_peak, traffic=None,
                                         kernel="msa_kv_append", kernel_ms=ms, peak_source=peak_label))))
 

@@ -209,6 +209,36 @@ int msa_kv_append(msa_handle h, msa_append_plan ap,
                   void *pool_k, void *pool_v, int64_t num_blocks,
                   const int32_t *block_table, int64_t block_table_len, void *cuda_stream);
 
+/* ---- KV write-back fused into the forward launch ----
+ * The forward kernel already brings every K/V row of a recomputed (CONTIG) or own (SELF) segment into shared memory;
+ * with a write-back plan the unit that loads a tile for the attention also stores it into its cache blocks (one TMA
+ * store per 16-token block and 64-element half, straight from the tile), so no second pass over the arena and no second
+ * launch is needed (PAPER.md:92 step 2 "allocates cache blocks": in the paper's engine the recomputed K/V land in
+ * paged blocks within the same step).
+ *
+ * msa_plan_create_writeback = msa_plan_create + `jobs` (same meaning as in msa_append_plan_create).  Restrictions, each
+ * reported as MSA_ERR_UNSUPPORTED (use msa_kv_append then): every 16-token copy unit of a job must coincide with a
+ * 16-token block of a CONTIG / SELF segment of the batch (same first arena row, same number of tokens), and some query
+ * row of the batch must attend to it (a row nobody reads is never loaded).  MSA_ERR_OVERLAP / MSA_ERR_INVALID_ARG /
+ * MSA_ERR_OUT_OF_RANGE as in msa_append_plan_create.  n_jobs = 0 gives an ordinary plan.
+ *
+ * msa_forward_writeback = msa_forward on such a plan, except that pool_k / pool_v are written: after the call has
+ * completed on the stream, pool[block_table[job.block_off + i/16]][i%16] = arena[job.row_off + i] for every job, bit for
+ * bit, and O / LSE are bit-identical to msa_forward on the same plan.  The destination blocks must not be read by this
+ * or any concurrently running call.  MSA_ERR_INVALID_ARG if the plan has no write-back jobs; MSA_ERR_OUT_OF_RANGE if a
+ * job's block-table slice exceeds block_table_len.  msa_forward on a write-back plan computes O / LSE only. */
+int msa_plan_create_writeback(msa_handle h, const msa_request *requests, int32_t n_req,
+                              const msa_segment *segments, int32_t n_seg,
+                              const msa_append *jobs, int32_t n_jobs, msa_plan *out);
+int msa_forward_writeback(msa_handle h, msa_plan p,
+                          const void *q, int64_t total_q,
+                          void *pool_k, void *pool_v, int64_t num_blocks,
+                          const int32_t *block_table, int64_t block_table_len,
+                          const void *contig_k, const void *contig_v, int64_t contig_rows,
+                          float softmax_scale,
+                          void *o, float *lse,
+                          void *workspace, size_t workspace_bytes, void *cuda_stream);
+
 /* Number of kernels the last msa_forward / msa_forward_host on this handle launched. */
 int msa_last_launch_count(msa_handle h);
 

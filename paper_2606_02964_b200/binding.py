@@ -58,7 +58,8 @@ _LIB: Optional[ctypes.CDLL] = None
 EXPORTS = ["msa_create", "msa_destroy", "msa_plan_create", "msa_plan_destroy", "msa_plan_get_info",
            "msa_plan_export", "msa_workspace_bytes", "msa_forward", "msa_forward_host",
            "msa_last_launch_count", "msa_set_timing", "msa_get_timing", "msa_strerror", "msa_last_cuda_error", "msa_version",
-           "msa_append_plan_create", "msa_append_plan_destroy", "msa_kv_append"]
+           "msa_append_plan_create", "msa_append_plan_destroy", "msa_kv_append",
+           "msa_plan_create_writeback", "msa_forward_writeback"]
 EVICTOR_EXPORTS = ["msa_evictor_create", "msa_evictor_destroy", "msa_evictor_add", "msa_evictor_remove", "msa_evictor_evict",
                    "msa_evictor_evict_linear", "msa_evictor_set_lambda", "msa_evictor_size", "msa_evictor_weight"]
 
@@ -103,6 +104,9 @@ def _lib() -> ctypes.CDLL:
         lib.msa_append_plan_destroy.argtypes = [vp]
         lib.msa_append_plan_destroy.restype = None
         lib.msa_kv_append.argtypes = [vp, vp, vp, vp, i64, vp, vp, i64, vp, i64, vp]
+        lib.msa_plan_create_writeback.argtypes = [vp, ctypes.POINTER(MsaRequest), i32, ctypes.POINTER(MsaSegment), i32,
+                                                  ctypes.POINTER(MsaAppend), i32, ctypes.POINTER(vp)]
+        lib.msa_forward_writeback.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, i64, f32, vp, vp, vp, sz, vp]
         f64 = ctypes.c_double
         lib.msa_evictor_create.argtypes = [ctypes.POINTER(MsaEvictorConfig), ctypes.POINTER(vp)]
         lib.msa_evictor_destroy.argtypes = [vp]
@@ -188,11 +192,13 @@ _EXPORT_DTYPES = {
     0: np.dtype([("src", "<i4"), ("abs_start", "<i4"), ("nvalid", "<i4"), ("paged", "<i4")]),
     1: np.dtype([("q_row0", "<i4"), ("n_tok", "<i4"), ("q_abs0", "<i4"), ("kvh", "<i4"), ("vb_begin", "<i4"),
                  ("vb_count", "<i4"), ("tile_begin", "<i4"), ("tile_end", "<i4"), ("partial_off", "<i4"),
-                 ("mode", "<i4"), ("tile_info_begin", "<i4"), ("r2", "<i4")]),
+                 ("mode", "<i4"), ("tile_info_begin", "<i4"), ("writeback", "<i4")]),
     2: np.dtype("<i4"),
     3: np.dtype([("q_row0", "<i4"), ("n_tok", "<i4"), ("kvh", "<i4"), ("n_partials", "<i4"),
                  ("first_off", "<i8"), ("stride", "<i8")]),
     4: np.dtype([("max_abs", "<i4"), ("ragged", "<i4")]),
+    5: np.dtype("<i4"),
+    6: np.dtype("<i4"),
 }
 
 
@@ -306,6 +312,32 @@ def msa_append_plan_create(h, jobs):
     ap = ctypes.c_void_p()
     _check(_lib().msa_append_plan_create(h, arr, len(jobs), ctypes.byref(ap)), "msa_append_plan_create")
     return ap
+
+
+def msa_plan_create_writeback(h, requests, n_req: int, segments, n_seg: int, jobs) -> ctypes.c_void_p:
+    """jobs: iterable of (row_off, len, block_off), as in msa_append_plan_create."""
+    jobs = list(jobs)
+    arr = (MsaAppend * max(1, len(jobs)))()
+    for i, (row_off, n, block_off) in enumerate(jobs):
+        arr[i] = MsaAppend(int(row_off), int(n), int(block_off))
+    p = ctypes.c_void_p()
+    _check(_lib().msa_plan_create_writeback(h, requests, n_req, segments, n_seg, arr, len(jobs), ctypes.byref(p)),
+           "msa_plan_create_writeback")
+    return p
+
+
+def msa_forward_writeback(h, p, q, pool_k, pool_v, block_table, contig_k, contig_v, softmax_scale: float, o, lse,
+                          workspace=None, stream: Optional[int] = None) -> None:
+    """msa_forward that also writes the plan's write-back jobs into pool_k / pool_v (same launch)."""
+    total_q = int(q.shape[0])
+    num_blocks = 0 if pool_k is None else int(pool_k.shape[0])
+    bt_len = 0 if block_table is None else int(block_table.numel())
+    rows = 0 if contig_k is None else int(contig_k.shape[0])
+    ws_bytes = 0 if workspace is None else int(workspace.numel() * workspace.element_size())
+    _check(_lib().msa_forward_writeback(h, p, _dptr(q), total_q, _dptr(pool_k), _dptr(pool_v), num_blocks,
+                                        _dptr(block_table), bt_len, _dptr(contig_k), _dptr(contig_v), rows,
+                                        ctypes.c_float(softmax_scale), _dptr(o), _dptr(lse), _dptr(workspace), ws_bytes,
+                                        stream), "msa_forward_writeback")
 
 
 def msa_append_plan_destroy(ap) -> None:

@@ -117,6 +117,8 @@ struct msa_plan_s {
     const int32_t *d_cta_begin = nullptr;
     const MergeItem *d_merge = nullptr;
     const TileInfo *d_tile_info = nullptr;
+    const int32_t *d_vb_dst = nullptr;     // write-back plans only
+    const int32_t *d_tile_writer = nullptr;
 };
 
 struct msa_append_plan_s {
@@ -231,8 +233,34 @@ void msa_destroy(msa_handle h)
     delete h;
 }
 
+}  // extern "C"
+
+namespace {
+int plan_create(msa_handle h, const msa_request *requests, int32_t n_req, const msa_segment *segments, int32_t n_seg,
+                const msa_append *jobs, int32_t n_jobs, msa_plan *out);
+}
+
+extern "C" {
+
 int msa_plan_create(msa_handle h, const msa_request *requests, int32_t n_req, const msa_segment *segments,
                     int32_t n_seg, msa_plan *out)
+{
+    return plan_create(h, requests, n_req, segments, n_seg, nullptr, 0, out);
+}
+
+int msa_plan_create_writeback(msa_handle h, const msa_request *requests, int32_t n_req, const msa_segment *segments,
+                              int32_t n_seg, const msa_append *jobs, int32_t n_jobs, msa_plan *out)
+{
+    if (n_jobs < 0 || (n_jobs > 0 && !jobs)) return MSA_ERR_INVALID_ARG;
+    return plan_create(h, requests, n_req, segments, n_seg, jobs, n_jobs, out);
+}
+
+}  // extern "C"
+
+namespace {
+
+int plan_create(msa_handle h, const msa_request *requests, int32_t n_req, const msa_segment *segments, int32_t n_seg,
+                const msa_append *jobs, int32_t n_jobs, msa_plan *out)
 {
     if (!h || !out) return MSA_ERR_INVALID_ARG;
     *out = nullptr;
@@ -247,7 +275,7 @@ int msa_plan_create(msa_handle h, const msa_request *requests, int32_t n_req, co
     msa_plan p = new (std::nothrow) msa_plan_s();
     if (!p) return MSA_ERR_INVALID_ARG;
     p->h = h;
-    int rc = build_plan(pc, requests, n_req, segments, n_seg, &p->hp);
+    int rc = build_plan(pc, requests, n_req, segments, n_seg, &p->hp, jobs, n_jobs);
     if (rc != MSA_OK) {
         delete p;
         return rc;
@@ -260,7 +288,9 @@ int msa_plan_create(msa_handle h, const msa_request *requests, int32_t n_req, co
         const size_t b_cb = al(hp.cta_unit_begin.size() * sizeof(int32_t));
         const size_t b_mg = al(hp.merge_items.size() * sizeof(MergeItem));
         const size_t b_ti = al(hp.tile_info.size() * sizeof(TileInfo));
-        const size_t total = b_vb + b_un + b_cb + b_mg + b_ti + 256;
+        const size_t b_wb = al(hp.vb_dst.size() * sizeof(int32_t));
+        const size_t b_tw = al(hp.tile_writer.size() * sizeof(int32_t));
+        const size_t total = b_vb + b_un + b_cb + b_mg + b_ti + b_wb + b_tw + 256;
         DeviceGuard guard(h->cfg.device);
         cudaError_t e = guard.err;
         if (e == cudaSuccess) e = cudaMalloc(&p->d_buf, total);
@@ -274,6 +304,10 @@ int msa_plan_create(msa_handle h, const msa_request *requests, int32_t n_req, co
         p->d_cta_begin = reinterpret_cast<const int32_t *>(base + b_vb + b_un);
         p->d_merge = reinterpret_cast<const MergeItem *>(base + b_vb + b_un + b_cb);
         p->d_tile_info = reinterpret_cast<const TileInfo *>(base + b_vb + b_un + b_cb + b_mg);
+        if (hp.has_writeback) {
+            p->d_vb_dst = reinterpret_cast<const int32_t *>(base + b_vb + b_un + b_cb + b_mg + b_ti);
+            p->d_tile_writer = reinterpret_cast<const int32_t *>(base + b_vb + b_un + b_cb + b_mg + b_ti + b_wb);
+        }
         if (e == cudaSuccess && !hp.vblocks.empty())
             e = cudaMemcpy(base, hp.vblocks.data(), hp.vblocks.size() * sizeof(VBlock), cudaMemcpyHostToDevice);
         if (e == cudaSuccess && !hp.units.empty())
@@ -287,6 +321,12 @@ int msa_plan_create(msa_handle h, const msa_request *requests, int32_t n_req, co
         if (e == cudaSuccess && !hp.tile_info.empty())
             e = cudaMemcpy(base + b_vb + b_un + b_cb + b_mg, hp.tile_info.data(), hp.tile_info.size() * sizeof(TileInfo),
                            cudaMemcpyHostToDevice);
+        if (e == cudaSuccess && !hp.vb_dst.empty())
+            e = cudaMemcpy(base + b_vb + b_un + b_cb + b_mg + b_ti, hp.vb_dst.data(), hp.vb_dst.size() * sizeof(int32_t),
+                           cudaMemcpyHostToDevice);
+        if (e == cudaSuccess && !hp.tile_writer.empty())
+            e = cudaMemcpy(base + b_vb + b_un + b_cb + b_mg + b_ti + b_wb, hp.tile_writer.data(), hp.tile_writer.size() * sizeof(int32_t),
+                           cudaMemcpyHostToDevice);
         if (e != cudaSuccess) {
             cudaFree(p->d_buf);
             delete p;
@@ -296,6 +336,10 @@ int msa_plan_create(msa_handle h, const msa_request *requests, int32_t n_req, co
     *out = p;
     return MSA_OK;
 }
+
+}  // namespace
+
+extern "C" {
 
 void msa_plan_destroy(msa_plan p)
 {
@@ -324,7 +368,8 @@ int msa_workspace_bytes(msa_plan p, size_t *bytes)
 /* Introspection for tests: copies the host-side plan arrays out.
  * which: 0 = virtual blocks (int32 x4 each), 1 = work units (int32 x12 each),
  *        2 = cta_unit_begin (int32), 3 = merge items (int32 x4 + int64 x2 each),
- *        4 = per-tile mask summaries (int32 x2 each).
+ *        4 = per-tile mask summaries (int32 x2 each), 5 / 6 = write-back plans: destination block-table index per
+ *        virtual block, q_row0 of the storing work item per context KV tile (int32 each).
  * Call with buf == NULL to get the byte size. */
 int msa_plan_export(msa_plan p, int which, void *buf, size_t *bytes)
 {
@@ -337,6 +382,8 @@ int msa_plan_export(msa_plan p, int which, void *buf, size_t *bytes)
     case 2: src = p->hp.cta_unit_begin.data(); n = p->hp.cta_unit_begin.size() * sizeof(int32_t); break;
     case 3: src = p->hp.merge_items.data(); n = p->hp.merge_items.size() * sizeof(MergeItem); break;
     case 4: src = p->hp.tile_info.data(); n = p->hp.tile_info.size() * sizeof(TileInfo); break;
+    case 5: src = p->hp.vb_dst.data(); n = p->hp.vb_dst.size() * sizeof(int32_t); break;
+    case 6: src = p->hp.tile_writer.data(); n = p->hp.tile_writer.size() * sizeof(int32_t); break;
     default: return MSA_ERR_INVALID_ARG;
     }
     if (buf) {
@@ -374,10 +421,12 @@ bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) ==
 constexpr size_t kMapCacheEntries = 64;
 
 // The 23 tensor maps of one (q, pool, arena) pointer set, encoded once and kept in the handle.
-int cached_tensor_maps(msa_handle h, const HostPlan &hp, const void *q, int64_t total_q, const void *pool_k, const void *pool_v,
-                       int64_t num_blocks, const void *contig_k, const void *contig_v, int64_t contig_rows, FwdParams *out)
+int cached_tensor_maps(msa_handle h, const HostPlan &hp_in, bool writeback, const void *q, int64_t total_q, const void *pool_k,
+                       const void *pool_v, int64_t num_blocks, const void *contig_k, const void *contig_v, int64_t contig_rows,
+                       FwdParams *out)
 {
     const int Hq = h->cfg.num_q_heads, Hkv = h->cfg.num_kv_heads, D = h->cfg.head_dim;
+    struct { bool uses_paged, uses_contig; } hp{hp_in.uses_paged || writeback, hp_in.uses_contig};   // write-back stores through the pool maps
     // a plan that uses no paged (or no contiguous) segment never dereferences those maps: they are encoded over q
     msa_handle_s::MapKey key{q, hp.uses_paged ? pool_k : nullptr, hp.uses_paged ? pool_v : nullptr,
                              hp.uses_contig ? contig_k : nullptr, hp.uses_contig ? contig_v : nullptr,
@@ -424,17 +473,22 @@ int cached_tensor_maps(msa_handle h, const HostPlan &hp, const void *q, int64_t 
 
 }  // namespace
 
-extern "C" {
+namespace {
 
-int msa_forward(msa_handle h, msa_plan p, const void *q, int64_t total_q, const void *pool_k, const void *pool_v,
-                int64_t num_blocks, const int32_t *block_table, int64_t block_table_len, const void *contig_k,
-                const void *contig_v, int64_t contig_rows, float softmax_scale, void *o, float *lse, void *workspace,
-                size_t workspace_bytes, void *cuda_stream)
+int forward_impl(msa_handle h, msa_plan p, const void *q, int64_t total_q, const void *pool_k, const void *pool_v,
+                 int64_t num_blocks, const int32_t *block_table, int64_t block_table_len, const void *contig_k,
+                 const void *contig_v, int64_t contig_rows, float softmax_scale, void *o, float *lse, void *workspace,
+                 size_t workspace_bytes, void *cuda_stream, bool writeback)
 {
     if (!h || !p || p->h != h) return MSA_ERR_INVALID_ARG;
     if (h->planning_only) return MSA_ERR_NO_DEVICE;
     h->last_launches = 0;
     const HostPlan &hp = p->hp;
+    if (writeback) {
+        if (!hp.has_writeback) return MSA_ERR_INVALID_ARG;          // the plan must come from msa_plan_create_writeback
+        if (!pool_k || !pool_v || !block_table || num_blocks < 1 || num_blocks * MSA_BLOCK_SIZE > 0x7fffffffLL) return MSA_ERR_INVALID_ARG;
+        if (hp.wb_max_bt >= block_table_len) return MSA_ERR_OUT_OF_RANGE;
+    }
     if (!(softmax_scale > 0.f) || !isfinite(softmax_scale)) return MSA_ERR_INVALID_ARG;
     if (total_q < 0 || num_blocks < 0 || block_table_len < 0 || contig_rows < 0) return MSA_ERR_INVALID_ARG;
     if (hp.info.num_units == 0) return MSA_OK;
@@ -458,13 +512,15 @@ int msa_forward(msa_handle h, msa_plan p, const void *q, int64_t total_q, const 
     DeviceGuard guard(h->cfg.device);      // the caller's current device may be another one
     if (guard.err != cudaSuccess) return cuda_fail(guard.err, "msa_forward: cudaSetDevice");
     FwdParams fp;
-    int rc = cached_tensor_maps(h, hp, q, total_q, pool_k, pool_v, num_blocks, contig_k, contig_v, contig_rows, &fp);
+    int rc = cached_tensor_maps(h, hp, writeback, q, total_q, pool_k, pool_v, num_blocks, contig_k, contig_v, contig_rows, &fp);
     if (rc != MSA_OK) return rc;
     fp.vblocks = p->d_vblocks;
     fp.units = p->d_units;
     fp.cta_unit_begin = p->d_cta_begin;
     fp.tile_info = p->d_tile_info;
     fp.block_table = block_table;
+    fp.vb_dst = writeback ? p->d_vb_dst : nullptr;
+    fp.tile_writer = writeback ? p->d_tile_writer : nullptr;
     fp.kv_to_q = h->d_kv_to_q;
     fp.o = o;
     fp.lse = lse;
@@ -501,6 +557,28 @@ int msa_forward(msa_handle h, msa_plan p, const void *q, int64_t total_q, const 
         ++h->ev_steps;
     }
     return MSA_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int msa_forward(msa_handle h, msa_plan p, const void *q, int64_t total_q, const void *pool_k, const void *pool_v,
+                int64_t num_blocks, const int32_t *block_table, int64_t block_table_len, const void *contig_k,
+                const void *contig_v, int64_t contig_rows, float softmax_scale, void *o, float *lse, void *workspace,
+                size_t workspace_bytes, void *cuda_stream)
+{
+    return forward_impl(h, p, q, total_q, pool_k, pool_v, num_blocks, block_table, block_table_len, contig_k, contig_v, contig_rows,
+                        softmax_scale, o, lse, workspace, workspace_bytes, cuda_stream, false);
+}
+
+int msa_forward_writeback(msa_handle h, msa_plan p, const void *q, int64_t total_q, void *pool_k, void *pool_v, int64_t num_blocks,
+                          const int32_t *block_table, int64_t block_table_len, const void *contig_k, const void *contig_v,
+                          int64_t contig_rows, float softmax_scale, void *o, float *lse, void *workspace, size_t workspace_bytes,
+                          void *cuda_stream)
+{
+    return forward_impl(h, p, q, total_q, pool_k, pool_v, num_blocks, block_table, block_table_len, contig_k, contig_v, contig_rows,
+                        softmax_scale, o, lse, workspace, workspace_bytes, cuda_stream, true);
 }
 
 int msa_forward_host(msa_handle h, msa_plan p, const void *q_host, int64_t total_q, const void *pool_k,

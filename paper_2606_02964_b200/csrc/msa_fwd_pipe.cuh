@@ -96,6 +96,11 @@ enum PipeBar : int {
     kBarCount = 28
 };
 
+#ifdef MSA_NO_WRITEBACK           /* A/B builds only: the ring without its second "empty" arrival */
+constexpr bool kWritebackRing = false;
+#else
+constexpr bool kWritebackRing = true;
+#endif
 constexpr uint32_t kNamedStFull = 1;   // named barriers 1, 2: (l, ref) of chain 0 / 1 are in shared memory (128 + 128 threads)
 
 struct RingPos {
@@ -138,7 +143,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
         mbar_init(bar(kBarQEmpty), 1);
         for (int i = 0; i < C::kStages; ++i) {
             mbar_init(bar(kBarKvFull + i), 1);
-            mbar_init(bar(kBarKvEmpty + i), 1);
+            mbar_init(bar(kBarKvEmpty + i), kWritebackRing ? 2 : 1);   // the MMA warp's commit + the loader (or the write-back warp)
         }
         for (int c = 0; c < 2; ++c) {
             mbar_init(bar(kBarSFull + c), 1);
@@ -490,6 +495,9 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     r.row = (e.z > 0 && e.w) ? __ldg(P.block_table + e.x) * kBlock : e.x;
                     return r;
                 };
+                // fused KV write-back: in a write-back launch warp 15 follows the ring, stores the arena blocks of
+                // flagged units into their cache blocks straight from the ring slot, and gives every slot's second arrival
+                const bool wb = P.vb_dst != nullptr;
                 ResolvedVb cur = resolve(fetch(wu.tile_begin));
                 ResolvedVb nxt = resolve(fetch(wu.tile_begin + 1));
                 int4 raw = fetch(wu.tile_begin + 2);
@@ -571,6 +579,9 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                         }
                     }
                     __syncwarp();
+                    // second arrival on the slot's empty barrier: here, at once, unless this is a write-back launch (then the
+                    // write-back warp gives it for every tile, after its stores -- if any -- have read the slot)
+                    if (kWritebackRing && !wb && elect_one()) mbar_arrive(bar(kBarKvEmpty + rp.slot));
                     rp.advance2(C::kStages);
                     cur = nxt;
                     nxt = resolve(raw);
@@ -750,6 +761,84 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             prof_acc[14] = static_cast<unsigned long long>(clock64() - prof_mma_start);
             PROF_FLUSH(8, 15);
 #endif
+        }
+        else if (warp == 15 && P.vb_dst != nullptr) {
+            // ======================================================= write-back warp (plans from msa_plan_create_writeback)
+            // Follows the ring like the MMA warp.  In a flagged unit, once a K or V tile has landed, lane b stores virtual
+            // block b -- if it is an arena block with a destination -- into the cache (one TMA store per 64-element half,
+            // same box and swizzle as the load, partly filled blocks through the 8/4/2/1-row boxes), and when the stores
+            // have read the slot the warp gives the slot's second "empty" arrival that the loader gives everywhere else.
+            uint32_t entry = 0;                              // ring entry of K of the CTA's next tile (V: entry + 1)
+            int held = -1;                                   // slot whose stores may still be reading it (released one entry later)
+            for (int u = u_begin; u < u_end; ++u) {
+                const WorkUnit wu = P.units[u];
+                const int n = wu.tile_end - wu.tile_begin;
+                if (n <= 0) continue;
+                const int c0 = wu.kvh * D;
+#pragma unroll 1
+                for (int j = 0; j < n; ++j) {
+                    const int tile = wu.tile_begin + j;
+                    int dsti = -1, nv = 0, drow = 0;
+                    // is this tile mine to store?  (the planner deals the tiles out among the units that load them)
+                    if (wu.writeback != 0 && __ldg(P.tile_writer + wu.tile_info_begin + tile) == wu.q_row0 && lane < kVbPerTile &&
+                        tile * kVbPerTile + lane < wu.vb_count) {
+                        const int idx = wu.vb_begin + tile * kVbPerTile + lane;
+                        const int4 e = __ldg(reinterpret_cast<const int4 *>(P.vblocks + idx));   // {src, abs_start, nvalid, paged}
+                        if (e.z > 0 && e.w == 0) {
+                            dsti = __ldg(P.vb_dst + idx);
+                            nv = e.z;
+                            if (dsti >= 0) drow = __ldg(P.block_table + dsti) * kBlock;
+                        }
+                    }
+                    const bool stores = __any_sync(0xffffffffu, dsti >= 0);
+#pragma unroll 1
+                    for (int which = 0; which < 2; ++which, ++entry) {
+                        const uint32_t slot = entry % C::kStages, parity = (entry / C::kStages) & 1u;
+                        const CUtensorMap *tm_pool = which ? P.tm_pool_v : P.tm_pool_k;
+                        // Every tile of every unit, in ring order: a waiter that skips ahead (or is lapped) by two uses of a slot
+                        // cannot tell the phases apart, and an arrival given before the loader has taken the slot for THIS tile
+                        // would count for the slot's previous use and hand it back while the MMAs still read it.
+                        mbar_wait(bar(kBarKvFull + slot), parity);
+                        if (stores) {
+                            if (dsti >= 0) {
+                                const uint32_t src = sRing + slot * C::kTileBytes + lane * (kBlock * 128);
+                                int off = 0;
+#pragma unroll 1
+                                for (int i = 0; i < 5; ++i) {
+                                    const int rows_i = kBlock >> i;
+                                    if (nv & rows_i) {
+#pragma unroll 1
+                                        for (int h = 0; h < C::kHalves; ++h)
+                                            tma_store_2d(tm_pool + i, src + h * C::kHalfBytes + off * 128, c0 + h * 64, drow + off);
+                                        off += rows_i;
+                                    }
+                                }
+                            }
+                            tma_store_commit();                      // (an empty group for lanes without a block)
+                            if (held >= 0) {                         // the group before this one has read its slot by now
+                                asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+                                __syncwarp();
+                                if (lane == 0) mbar_arrive(bar(kBarKvEmpty + held));
+                            }
+                            held = static_cast<int>(slot);
+                        } else {
+                            if (held >= 0) {
+                                tma_store_wait_read();
+                                __syncwarp();
+                                if (lane == 0) mbar_arrive(bar(kBarKvEmpty + held));
+                                held = -1;
+                            }
+                            if (lane == 0) mbar_arrive(bar(kBarKvEmpty + slot));
+                        }
+                    }
+                }
+            }
+            if (held >= 0) {
+                tma_store_wait_read();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(kBarKvEmpty + held));
+            }
+            tma_store_wait_all();                            // the data is in global memory before the CTA retires
         }
 #if defined(MSA_PROF) && MSA_PROF == 2
         else if (warp == 15 && lane == 0 && blockIdx.x == 0 && u_begin < u_end) {

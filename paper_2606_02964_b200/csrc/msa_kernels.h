@@ -22,6 +22,8 @@ struct FwdParams {
     const int32_t *cta_unit_begin;   // [num_ctas+1]
     const TileInfo *tile_info;
     const int32_t *block_table;
+    const int32_t *vb_dst;           // fused KV write-back (NULL: none): per virtual block, block-table index of its destination or -1
+    const int32_t *tile_writer;      // ... and per context KV tile, q_row0 of the work item that stores it (or -1)
     const int32_t *kv_to_q;          // [Hkv][G] q heads of each kv head
     void *o;                         // bf16 [total_q][Hq][D]
     float *lse;                      // [total_q][Hq]

@@ -43,7 +43,7 @@ struct alignas(16) WorkUnit {
                            // kModeSplit: one q tile, even/odd KV tiles go to the two softmax
                            // warpgroups and are merged in the epilogue (short queries)
     int32_t tile_info_begin;  // index of the context's first TileInfo
-    int32_t reserved;
+    int32_t writeback;        // 1: this unit stores some of the K/V tiles it loads into the paged cache (HostPlan::tile_writer, vb_dst)
 };
 
 constexpr int kModePair = 0;

@@ -39,9 +39,10 @@ int64_t clamp_sum(int64_t c0, int64_t T, int64_t n)
 }  // namespace
 
 int build_plan(const PlannerConfig &cfg, const msa_request *req, int32_t n_req, const msa_segment *seg, int32_t n_seg,
-               HostPlan *out)
+               HostPlan *out, const msa_append *jobs, int32_t n_jobs)
 {
     if (!out || n_req < 0 || n_seg < 0 || (n_req > 0 && !req) || (n_seg > 0 && !seg)) return MSA_ERR_INVALID_ARG;
+    if (n_jobs < 0 || (n_jobs > 0 && !jobs)) return MSA_ERR_INVALID_ARG;
     if (cfg.G < 1 || cfg.R < 8 || cfg.tiles_per_group < 1 || cfg.num_ctas < 1) return MSA_ERR_INVALID_ARG;
     HostPlan &hp = *out;
     hp = HostPlan();
@@ -127,6 +128,45 @@ int build_plan(const PlannerConfig &cfg, const msa_request *req, int32_t n_req, 
         ctxs[key] = c;
     }
 
+    // ---- fused KV write-back: which virtual block goes to which block-table entry ------------
+    // A job's 16-token copy units must coincide with virtual blocks of the arena (same first row, same number of
+    // valid slots): then the unit that loads a K/V tile for the attention can store it into the cache as it is.
+    struct WbUnit { int32_t bt_index, nvalid; bool used; };
+    std::map<int64_t, WbUnit> wb_units;          // first arena row -> destination
+    if (n_jobs > 0) {
+        std::vector<std::pair<int64_t, int64_t>> spans;
+        for (int32_t j = 0; j < n_jobs; ++j) {
+            const msa_append &a = jobs[j];
+            if (a.len < 1 || a.row_off < 0 || a.block_off < 0) return MSA_ERR_INVALID_ARG;
+            const int nblk = (a.len + kBlock - 1) / kBlock;
+            const int64_t last_bt = static_cast<int64_t>(a.block_off) + nblk - 1;
+            if (last_bt > INT32_MAX || a.row_off + a.len - 1 > INT32_MAX) return MSA_ERR_OUT_OF_RANGE;
+            spans.emplace_back(a.block_off, last_bt + 1);
+            hp.wb_max_bt = std::max(hp.wb_max_bt, last_bt);
+            for (int b = 0; b < nblk; ++b) {
+                const int64_t row = a.row_off + static_cast<int64_t>(b) * kBlock;
+                if (wb_units.count(row)) return MSA_ERR_OVERLAP;
+                wb_units[row] = WbUnit{a.block_off + b, std::min(kBlock, a.len - b * kBlock), false};
+            }
+        }
+        std::sort(spans.begin(), spans.end());
+        for (size_t i = 1; i < spans.size(); ++i)
+            if (spans[i].first < spans[i - 1].second) return MSA_ERR_OVERLAP;
+        hp.vb_dst.assign(hp.vblocks.size(), -1);
+        for (size_t v = 0; v < hp.vblocks.size(); ++v) {
+            const VBlock &vb = hp.vblocks[v];
+            if (vb.paged || vb.nvalid <= 0) continue;
+            auto it = wb_units.find(vb.src);
+            if (it == wb_units.end()) continue;
+            if (it->second.nvalid != vb.nvalid) return MSA_ERR_UNSUPPORTED;      // job and segment cut the rows differently
+            hp.vb_dst[v] = it->second.bt_index;
+            it->second.used = true;
+        }
+        for (const auto &kv : wb_units)
+            if (!kv.second.used) return MSA_ERR_UNSUPPORTED;                      // rows no segment of this batch holds
+        hp.has_writeback = true;
+    }
+
     // ---- work items: (run, kv head, q-tile group), horizon folded in ------------------
     // tiles_per_group == 2: groups of 2R tokens run as kModePair (two q tiles share each KV
     // tile); a remainder of <= R tokens (and every short run) runs as kModeSplit.
@@ -167,6 +207,43 @@ int build_plan(const PlannerConfig &cfg, const msa_request *req, int32_t n_req, 
                 t0 += it.n_tok;
             }
         }
+    }
+
+    // ---- write-back: which item stores which KV tile --------------------------------------------------------
+    // All q-tile groups (items) of the runs that share a context load the same K/V tiles; the tiles that hold blocks
+    // with a destination are dealt out round-robin among the items whose causal horizon reaches them, so the extra
+    // stores are spread evenly over the units (the same assignment for every kv head).
+    std::vector<uint8_t> item_writes(items.size(), 0);
+    if (hp.has_writeback) {
+        hp.tile_writer.assign(hp.tile_info.size(), -1);
+        std::map<int32_t, std::vector<size_t>> by_ctx;                            // vb_begin -> items of kv head 0, in q order
+        for (size_t i = 0; i < items.size(); ++i)
+            if (items[i].kvh == 0) by_ctx[items[i].vb_begin].push_back(i);
+        std::map<std::pair<int32_t, int32_t>, uint8_t> writes;                    // (vb_begin, q_row0) -> writes something
+        for (const auto &kv : ctxs) {
+            const Ctx &c = kv.second;
+            const std::vector<size_t> &its = by_ctx[c.vb_begin];
+            const int32_t n_tiles = (c.vb_count + kVbPerTile - 1) / kVbPerTile;
+            for (int32_t t = 0; t < n_tiles; ++t) {
+                bool any = false;
+                int32_t last_b = -1;
+                for (int b = 0; b < kVbPerTile && t * kVbPerTile + b < c.vb_count; ++b)
+                    if (hp.vb_dst[c.vb_begin + t * kVbPerTile + b] >= 0) {
+                        any = true;
+                        last_b = t * kVbPerTile + b;
+                    }
+                if (!any) continue;
+                std::vector<size_t> cand;
+                for (size_t i : its)
+                    if (items[i].vb_count > last_b) cand.push_back(i);           // loads every destination block of the tile
+                if (cand.empty()) return MSA_ERR_UNSUPPORTED;                    // a row no query of this batch attends to
+                const Item &w = items[cand[static_cast<size_t>(t) % cand.size()]];
+                hp.tile_writer[c.ti_begin + t] = w.q_row0;
+                writes[std::make_pair(c.vb_begin, w.q_row0)] = 1;
+            }
+        }
+        for (size_t i = 0; i < items.size(); ++i)
+            item_writes[i] = writes.count(std::make_pair(items[i].vb_begin, items[i].q_row0)) ? 1 : 0;
     }
 
     // ---- persistent schedule ------------------------------------------------------------
@@ -331,6 +408,7 @@ int build_plan(const PlannerConfig &cfg, const msa_request *req, int32_t n_req, 
             u.tile_info_begin = it.ti_begin;
             u.tile_begin = pc.tb;
             u.tile_end = pc.te;
+            u.writeback = item_writes[pc.item];
             if (pieces[pc.item] > 1) {
                 const int64_t rows = static_cast<int64_t>(it.n_tok) * cfg.G;
                 const int64_t stride = (rows * (cfg.D + 1) + 3) / 4 * 4;

@@ -25,13 +25,18 @@ struct HostPlan {
     std::vector<int32_t> cta_unit_begin;   // [num_ctas_used + 1]
     std::vector<MergeItem> merge_items;
     std::vector<TileInfo> tile_info;
+    std::vector<int32_t> vb_dst;           // write-back plans: per virtual block, block-table index of its destination or -1
+    std::vector<int32_t> tile_writer;      // write-back plans: per context KV tile, q_row0 of the item that stores it or -1
     msa_plan_info info{};
     int64_t workspace_floats = 0;
     bool uses_paged = false, uses_contig = false;
+    bool has_writeback = false;
+    int64_t wb_max_bt = -1;                // largest block-table index a write-back job touches
 };
 
 // Returns MSA_OK or a negative MSA_ERR_* code.
+// jobs / n_jobs: optional KV write-back fused into the forward launch (msa_plan_create_writeback).
 int build_plan(const PlannerConfig &cfg, const msa_request *req, int32_t n_req, const msa_segment *seg, int32_t n_seg,
-               HostPlan *out);
+               HostPlan *out, const msa_append *jobs = nullptr, int32_t n_jobs = 0);
 
 }  // namespace msa

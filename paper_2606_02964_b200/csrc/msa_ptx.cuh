@@ -59,14 +59,21 @@ __device__ __forceinline__ bool mbar_try_wait_sleep(uint32_t bar, uint32_t parit
 }
 // Waits for the phase with the given parity to complete.  The loop is kept to a handful of instructions: a
 // sleeping warp is woken by every mbarrier event of its CTA, not only by its own, and each spurious wake-up takes
-// issue slots from the warps of its SM sub-partition that have work.  A wait that goes through ~2^27 wake-ups
-// (seconds) traps instead of hanging the device (a lost arrive is a bug, not a state).
+// issue slots from the warps of its SM sub-partition that have work.  A wait that lasts seconds traps instead of
+// hanging the device (a lost arrive is a bug, not a state).
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     if (mbar_try_wait(bar, parity)) return;
     uint32_t spins = 0;
+    long long t0 = 0;
     while (!mbar_try_wait_sleep(bar, parity, 1000000u)) {
-        if (++spins == (1u << 27)) __trap();
+        // in a live kernel a wake-up comes every few dozen cycles, in a dead one every millisecond: look at the clock
+        // every 1024 wake-ups and give up after ~2 s of SM clocks either way
+        if ((++spins & 1023u) == 0) {
+            const long long t = clock64();
+            if (t0 == 0) t0 = t;
+            else if (t - t0 > 4000000000LL) __trap();
+        }
     }
 }
 // ------------------------------------------------------------------ proxies / fences
@@ -100,6 +107,27 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const void *tmap, uint
         "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
         ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(bar), "r"(c0), "r"(c1)
         : "memory");
+}
+// 2-D tiled store: the box at smem `src` goes to global memory (bulk async-group completion).
+__device__ __forceinline__ void tma_store_2d(const void *tmap, uint32_t src, int32_t c0, int32_t c1)
+{
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
+                 ::"l"(reinterpret_cast<uint64_t>(tmap)), "r"(src), "r"(c0), "r"(c1)
+                 : "memory");
+}
+__device__ __forceinline__ void tma_store_commit()
+{
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+// all bulk groups of this thread have finished READING shared memory (the source may be overwritten)
+__device__ __forceinline__ void tma_store_wait_read()
+{
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+// all bulk groups of this thread are complete (the data is in global memory)
+__device__ __forceinline__ void tma_store_wait_all()
+{
+    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 // ------------------------------------------------------------------ TMEM
 __device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols)
