@@ -167,7 +167,6 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
     const int u_begin = P.cta_unit_begin[blockIdx.x], u_end = P.cta_unit_begin[blockIdx.x + 1];
     const int G = P.G, R = P.R;
     const float sl = P.scale_log2;
-    const float inv_sl = 1.f / sl;
 
     if (warp < 8) {
         // =========================================================== softmax warpgroups
@@ -245,7 +244,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     // fast path: stale reference, tile max found alongside, P handed over in parts
                     move_reference(true);
                     float tile_sum, tile_max;
-                    done = softmax_fast_tile(tS, sl, inv_sl, ref, tile_sum, tile_max, [&](int part) {
+                    done = softmax_fast_tile(tS, sl, ref, tile_sum, tile_max, [&](int part) {
                         __syncwarp();
                         if (lane == 0) mbar_arrive(bar((part == 0 ? kBarPLo : kBarPQ2) + c));
                         if ((threadIdx.x & 127) == 0 && part == 0) PROF_TRACE(1 + c, s, 4);

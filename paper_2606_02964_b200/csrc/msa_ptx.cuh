@@ -232,47 +232,11 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16
           "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
         : "memory");
 }
-// 16x256b / 16x128b: the warp touches 16 TMEM lanes starting at the address's lane (a multiple of 16
-// inside the warp's 32-lane quarter).  Thread t holds, per repetition i (checked on B200 with a probe):
-//   ld 16x256b: r[4i], r[4i+1] = lane t/4,     columns 8i + 2(t%4), 8i + 2(t%4) + 1
-//               r[4i+2], r[4i+3] = lane t/4 + 8, same columns
-//   st 16x128b: r[2i] = lane t/4, column 4i + t%4;  r[2i+1] = lane t/4 + 8, same column
-// so a row's 32-bit pairs packed to bf16x2 land in exactly the thread that computed them.
-__device__ __forceinline__ void tmem_ld_16x256b_x4(uint32_t taddr, uint32_t (&r)[16])
-{
-    asm volatile("tcgen05.ld.sync.aligned.16x256b.x4.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-                   "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-                 : "r"(taddr)
-                 : "memory");
-}
-__device__ __forceinline__ void tmem_st_16x256b_x4(uint32_t taddr, const uint32_t (&r)[16])
-{
-    asm volatile("tcgen05.st.sync.aligned.16x256b.x4.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
-                 ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
-                   "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
-                 : "memory");
-}
-__device__ __forceinline__ void tmem_st_16x128b_x4(uint32_t taddr, const uint32_t (&r)[8])
-{
-    asm volatile("tcgen05.st.sync.aligned.16x128b.x4.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
-                 ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
-                 : "memory");
-}
 // wait::st that names registers computed by the work that is meant to hide the store latency: the compiler cannot
 // schedule the wait (and the publication that follows it) above that work
 __device__ __forceinline__ void tmem_wait_st_after(uint32_t &a, uint32_t &b, uint32_t &c, uint32_t &d)
 {
     asm volatile("tcgen05.wait::st.sync.aligned;" : "+r"(a), "+r"(b), "+r"(c), "+r"(d) : : "memory");
-}
-// wait::ld that also names 16 destination registers, so no consumer of them can be scheduled above the wait
-__device__ __forceinline__ void tmem_wait_ld_regs16(uint32_t *r)
-{
-    asm volatile("tcgen05.wait::ld.sync.aligned;"
-                 : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]),
-                   "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15])
-                 :
-                 : "memory");
 }
 __device__ __forceinline__ void tmem_wait_ld()
 {
@@ -313,15 +277,6 @@ __device__ __forceinline__ float2 fadd2(float2 a, float2 b)
     asm("add.rn.ftz.f32x2 %0, %1, %2;"
         : "=l"(d)
         : "l"(*reinterpret_cast<uint64_t *>(&a)), "l"(*reinterpret_cast<uint64_t *>(&b)));
-    return *reinterpret_cast<float2 *>(&d);
-}
-__device__ __forceinline__ float2 ffma2_rm(float2 a, float2 b, float2 c)   // round toward -inf
-{
-    uint64_t d;
-    asm("fma.rm.ftz.f32x2 %0, %1, %2, %3;"
-        : "=l"(d)
-        : "l"(*reinterpret_cast<uint64_t *>(&a)), "l"(*reinterpret_cast<uint64_t *>(&b)),
-          "l"(*reinterpret_cast<uint64_t *>(&c)));
     return *reinterpret_cast<float2 *>(&d);
 }
 // wait::ld that also names the 32 destination registers, so no consumer of them can be

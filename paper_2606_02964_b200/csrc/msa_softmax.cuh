@@ -13,13 +13,13 @@
 // headroom for the accumulation that follows: P <= 2^64, a tile adds at most 2^71 to l and
 // 2^71 |V| to O (fp32 holds 2^127).
 //
-// Pipes (B200, measured with working microbenchmarks, cycles per warp instruction on one SM
-// sub-partition): MUFU.EX2 8.0; FFMA2 / FADD2 2.1; every ALU-pipe instruction (F2FP pack, FMNMX,
-// LEA) 2.0; FFMA / FADD 1.0.  MUFU time overlaps with everything else, FFMA2 and ALU time add up.
-// An all-MUFU tile therefore costs 1024 cycles of MUFU per warp while the tensor core needs 1024
-// per tile and chain: with both chains on one sub-partition MUFU alone would bound the kernel.
-// kEmuMask moves part of the exponentials to the FMA/ALU pipes (ex2_emu_pair: exact range
-// reduction by two FMAs, degree-3 polynomial, exponent added as an integer).
+// Pipes (B200, measured with working microbenchmarks, profiles/r02_microbench.md; cycles per warp instruction on one
+// SM sub-partition): MUFU.EX2 8.0; FFMA2 / FADD2 2.1; every ALU-pipe instruction (F2FP pack, FMNMX, LEA) 2.0;
+// FFMA / FADD 1.0.  MUFU time overlaps with everything else, FFMA2 and ALU time add up.  An all-MUFU tile costs 1024
+// cycles of MUFU per warp, about what the tensor core needs per tile and chain -- but moving part of the exponentials
+// to a polynomial on the FMA / ALU pipes (measured at 4/16 ... 8/16 of the elements, with a range reduction of two
+// FMAs and a degree-3 polynomial) made the kernel slower, not faster: one in-order warp per row set is bound by its
+// own issue order and by the P -> PV -> QK -> S round trip, not by the MUFU pipe.
 //
 // Hand-off.  P is published in three steps (keys 0-63, 64-95, 96-127): `arrive(i)` is called once
 // the corresponding columns of P are visible to the tensor core, so O += P V trails the
@@ -32,48 +32,18 @@
 namespace msa {
 
 constexpr float kGuardLog2 = 64.f;    // largest s*scale_log2 - ref the fast path accepts
-// bit j: pair j of the 16 element pairs of every 32-column chunk takes 2^x from ex2_emu_pair
-// (FMA / ALU pipes) instead of MUFU.EX2
-#ifndef MSA_EMU_MASK
-#define MSA_EMU_MASK 0x0000u
-#endif
-constexpr uint32_t kEmuMask = MSA_EMU_MASK;
 
 struct SoftmaxRow {
     float2 sl2;       // scale_log2
     float2 nr2;       // -ref
-    float2 k2;        // 1.5*2^23 - ref (exact: both are integers below 2^24)
-    float s_floor;    // scores below (ref - 120)/scale_log2 are clamped: their p is < 2^-120 either way
 };
 
-__device__ __forceinline__ SoftmaxRow make_softmax_row(float sl, float inv_sl, float ref)
+__device__ __forceinline__ SoftmaxRow make_softmax_row(float sl, float ref)
 {
     SoftmaxRow r;
     r.sl2 = make_float2(sl, sl);
     r.nr2 = make_float2(-ref, -ref);
-    r.k2 = make_float2(12582912.f - ref, 12582912.f - ref);
-    r.s_floor = (ref - 120.f) * inv_sl;
     return r;
-}
-
-// 2^(s*sl - ref) for a pair on the FMA / ALU pipes, straight from the raw scores:
-//   r = fma.rm(s, sl, magic - ref) = magic + floor(x)      (x = s*sl - ref, |x| < 2^22)
-//   f = fma(s, sl, (magic - ref) - r) = x - floor(x)       one rounding, in [0, 1]
-//   2^f by a degree-3 polynomial with p(0) = 1 (minimax relative error 8.6e-5 on [0,1), far below
-//   the bf16 rounding of P), floor(x) added into the exponent field.
-__device__ __forceinline__ float2 ex2_emu_pair(float s0, float s1, const SoftmaxRow &t)
-{
-    const float2 sc = make_float2(fmaxf(s0, t.s_floor), fmaxf(s1, t.s_floor));
-    const float2 r = ffma2_rm(sc, t.sl2, t.k2);
-    const float2 c = ffma2(r, make_float2(-1.f, -1.f), t.k2);
-    const float2 f = ffma2(sc, t.sl2, c);
-    float2 p = ffma2(f, make_float2(0.07706724107265472f, 0.07706724107265472f),
-                     make_float2(0.22764497995376587f, 0.22764497995376587f));
-    p = ffma2(p, f, make_float2(0.6951166391372681f, 0.6951166391372681f));
-    p = ffma2(p, f, make_float2(1.f, 1.f));
-    p.x = __uint_as_float(__float_as_uint(p.x) + (__float_as_uint(r.x) << 23));
-    p.y = __uint_as_float(__float_as_uint(p.y) + (__float_as_uint(r.y) << 23));
-    return p;
 }
 
 __device__ __forceinline__ float chunk_max(const uint32_t (&sr)[32])
@@ -88,22 +58,18 @@ __device__ __forceinline__ float chunk_max(const uint32_t (&sr)[32])
 }
 
 // Pairs [J0, J1) of a 32-column chunk: scores -> packed bf16 pairs; two sum accumulators keep
-// the dependent FADD2 chain short.  MASK bit j: pair j takes 2^x from ex2_emu_pair.
-template <uint32_t MASK, int J0, int J1>
+// the dependent FADD2 chain short.
+template <int J0, int J1>
 __device__ __forceinline__ void softmax_pairs(const uint32_t (&sr)[32], const SoftmaxRow &t, float2 &sa, float2 &sb,
                                               uint32_t (&pk)[16])
 {
 #pragma unroll
     for (int j = J0; j < J1; ++j) {
         const float s0 = __uint_as_float(sr[2 * j]), s1 = __uint_as_float(sr[2 * j + 1]);
+        const float2 x = ffma2(make_float2(s0, s1), t.sl2, t.nr2);
         float2 pp;
-        if (MASK >> j & 1) {
-            pp = ex2_emu_pair(s0, s1, t);
-        } else {
-            const float2 x = ffma2(make_float2(s0, s1), t.sl2, t.nr2);
-            pp.x = ex2_approx(x.x);
-            pp.y = ex2_approx(x.y);
-        }
+        pp.x = ex2_approx(x.x);
+        pp.y = ex2_approx(x.y);
         if (j & 1) sb = fadd2(sb, pp); else sa = fadd2(sa, pp);
         pk[j] = pack_bf16x2(pp.x, pp.y);
     }
@@ -117,10 +83,10 @@ __device__ __forceinline__ void softmax_pairs(const uint32_t (&sr)[32], const So
 // The waits for the P stores name registers of the chunk computed in between (tmem_wait_st_after):
 // without that the compiler is free to schedule the wait -- and the stall -- right behind the store.
 template <class Arrive, class Mark>
-__device__ __forceinline__ bool softmax_fast_tile(uint32_t tS, float sl, float inv_sl, float ref, float &tile_sum,
+__device__ __forceinline__ bool softmax_fast_tile(uint32_t tS, float sl, float ref, float &tile_sum,
                                                   float &tile_max, Arrive &&arrive, Mark &&mark)
 {
-    const SoftmaxRow t = make_softmax_row(sl, inv_sl, ref);
+    const SoftmaxRow t = make_softmax_row(sl, ref);
     float2 sa = make_float2(0.f, 0.f), sb = make_float2(0.f, 0.f);
     uint32_t c0[32], c1[32], c2[32], c3[32];
     uint32_t pk0[16], pk1[16];
@@ -132,13 +98,13 @@ __device__ __forceinline__ bool softmax_fast_tile(uint32_t tS, float sl, float i
     tmem_ld32(tS + 96, c3);
     mark(1);
     float mx = fmaxf(chunk_max(c0), chunk_max(c1));
-    softmax_pairs<kEmuMask, 0, 16>(c0, t, sa, sb, pk0);
+    softmax_pairs<0, 16>(c0, t, sa, sb, pk0);
     // the second half has landed by now: its row max is found among the arithmetic of chunk 1,
     // so the guard is ready as soon as the first half of P is
     tmem_wait_ld_regs(c2);
     tmem_wait_ld_regs(c3);
     mx = fmaxf(mx, fmaxf(chunk_max(c2), chunk_max(c3)));
-    softmax_pairs<kEmuMask, 0, 16>(c1, t, sa, sb, pk1);
+    softmax_pairs<0, 16>(c1, t, sa, sb, pk1);
     mark(2);
     tile_max = mx;
     if (__any_sync(0xffffffffu, !(fmaf(mx, sl, -ref) <= kGuardLog2))) return false;
@@ -147,16 +113,16 @@ __device__ __forceinline__ bool softmax_fast_tile(uint32_t tS, float sl, float i
     tmem_st16(tS + 16, pk1);
     // each part is published while the next one is computed: its stores have completed by then
     // (no stall), and O += P V of the published keys finishes before the next part is ready
-    softmax_pairs<kEmuMask, 0, 16>(c2, t, sa, sb, pk0);
+    softmax_pairs<0, 16>(c2, t, sa, sb, pk0);
     tmem_wait_st_after(pk0[12], pk0[13], pk0[14], pk0[15]);
     tc_fence_before();
     arrive(0);
     tmem_st16(tS + 32, pk0);
-    softmax_pairs<kEmuMask, 0, 8>(c3, t, sa, sb, pk1);
+    softmax_pairs<0, 8>(c3, t, sa, sb, pk1);
     tmem_wait_st_after(pk1[4], pk1[5], pk1[6], pk1[7]);
     tc_fence_before();
     arrive(1);
-    softmax_pairs<kEmuMask, 8, 16>(c3, t, sa, sb, pk1);
+    softmax_pairs<8, 16>(c3, t, sa, sb, pk1);
     tmem_st16(tS + 48, pk1);
     tile_sum = (sa.x + sb.x) + (sa.y + sb.y);
     mark(5);
