@@ -290,8 +290,9 @@ def run_mine(args, rank: int, world: int, local_rank: int):
             # the other three performance configs of BASELINE.json, each with its own roofline block and clocks
             del p
             line["secondary"] = []
-            for wl, k in (("cfg3_70b_long", 30), ("cfg4_mixed", 20), ("cfg5_short_query", 50)):
+            for wl, k in (("cfg5_short_query", 50), ("cfg3_70b_long", 30), ("cfg4_mixed", 20)):
                 torch.cuda.empty_cache()
+                time.sleep(2.0)            # each workload starts from an idle chip, not from the last one's power state
                 sec, psec = bench_workload(wl, max(10, min(args.steps, k)), args.warmup, do_e2e=False)
                 line["secondary"].append(dict(workload=wl, metric=sec["metric"], value=sec["value"], unit=sec["unit"],
                                               ms_per_step=sec["ms_per_step"], gpu_launches=sec["gpu_launches"],
