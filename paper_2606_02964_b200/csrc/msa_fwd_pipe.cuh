@@ -286,10 +286,10 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     }
                     m_run = fmaxf(m_run, fmaxf(mx0, mx1));
                     move_reference(s > 0);
+                    // p chunk by chunk, handed over in the same three parts as on the fast path: O += P V of the keys
+                    // that are done runs while the rest is still being exponentiated
                     float sum0 = 0.f, sum1 = 0.f;
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        uint32_t pk[16];
+                    auto exact_chunk = [&](int q, uint32_t (&pk)[16]) {
 #pragma unroll
                         for (int j = 0; j < 16; ++j) {
                             const float p0 = ex2_approx(fmaf(__uint_as_float(sr[q * 32 + 2 * j]), sl, -ref));
@@ -298,17 +298,28 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                             sum1 += p1;
                             pk[j] = pack_bf16x2(p0, p1);
                         }
-                        tmem_st16(tS + q * 16, pk);
-                    }
+                    };
+                    auto publish = [&](int b) {
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(bar(b + c));
+                    };
+                    uint32_t pka[16], pkb[16];
+                    exact_chunk(0, pka);
+                    tmem_st16(tS, pka);
+                    exact_chunk(1, pkb);
+                    tmem_st16(tS + 16, pkb);
+                    exact_chunk(2, pka);
+                    tmem_wait_st_after(pka[12], pka[13], pka[14], pka[15]);
+                    publish(kBarPLo);
+                    tmem_st16(tS + 32, pka);
+                    exact_chunk(3, pkb);
+                    tmem_wait_st_after(pkb[12], pkb[13], pkb[14], pkb[15]);
+                    publish(kBarPQ2);
+                    tmem_st16(tS + 48, pkb);
                     l += sum0 + sum1;
                     tmem_wait_st();
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) {
-                        mbar_arrive(bar(kBarPLo + c));
-                        mbar_arrive(bar(kBarPQ2 + c));
-                        mbar_arrive(bar(kBarPQ3 + c));
-                    }
+                    publish(kBarPQ3);
                 }
                 PROF_ADD(2);
                 if ((threadIdx.x & 127) == 0) PROF_TRACE(1 + c, s, 6);
@@ -622,18 +633,20 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             // tile, and it never carries out of its field (shared memory ends below 256 KB), so a tile's descriptor
             // is formed once and every MMA adds a compile-time constant to it: the issuing thread shares its SM
             // sub-partition with two softmax warps, and every instruction it does not need shortens the P -> S round trip.
-            const uint64_t q_desc = make_smem_desc(sQ, 16, 1024);
-            const uint64_t k_desc = make_smem_desc(sRing, 16, 1024);
-            const uint64_t v_desc = make_smem_desc(sRing, C::kHalfBytes, 1024);
-            constexpr uint64_t kTileStep = C::kTileBytes >> 4;
+            // (the high word -- SBO 1024, version, 128-byte swizzle -- is the same constant for all three operands)
+            constexpr uint32_t kDescHi = make_smem_desc_hi(1024);
+            const uint32_t q_desc = make_smem_desc_lo(sQ, 16);
+            const uint32_t k_desc = make_smem_desc_lo(sRing, 16);
+            const uint32_t v_desc = make_smem_desc_lo(sRing, C::kHalfBytes);
+            constexpr uint32_t kTileStep = C::kTileBytes >> 4;
             auto qk = [&](int c, int qtile, uint32_t kslot) {
-                const uint64_t qd = q_desc + qtile * kTileStep, kd = k_desc + kslot * kTileStep;
+                const uint32_t qd = q_desc + qtile * kTileStep, kd = k_desc + kslot * kTileStep;
                 const uint32_t d_tmem = tmem + C::kColS + c * C::kChainCols;
 #pragma unroll
                 for (int k = 0; k < D / 16; ++k) {
                     constexpr uint32_t kHalfStep = C::kHalfBytes >> 4;
-                    const uint64_t off = (k >> 2) * kHalfStep + (k & 3) * 2;          // ((k>>2)*kHalfBytes + (k&3)*32) >> 4
-                    umma_ss(d_tmem, qd + off, kd + off, idesc_s, k > 0);
+                    const uint32_t off = (k >> 2) * kHalfStep + (k & 3) * 2;          // ((k>>2)*kHalfBytes + (k&3)*32) >> 4
+                    umma_ss_lo<kDescHi>(d_tmem, qd + off, kd + off, idesc_s, k > 0);
                 }
                 umma_commit(bar(kBarSFull + c));
             };
@@ -652,20 +665,20 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     ph_ofree[c] ^= 1;
                 }
                 tc_fence_after();
-                const uint64_t vd = v_desc + vslot * kTileStep;
+                const uint32_t vd = v_desc + vslot * kTileStep;
 #pragma unroll
                 for (int k = 0; k < kTileN / 32; ++k)
-                    umma_ts(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
+                    umma_ts_lo<kDescHi>(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
                             vd + k * ((kBlock * 128) >> 4), idesc_o, (!first || k > 0) ? 1u : 0u);
             };
             auto pv_hi = [&](int c, uint32_t vslot) {
-                const uint64_t vd = v_desc + vslot * kTileStep;
+                const uint32_t vd = v_desc + vslot * kTileStep;
                 mbar_wait(bar(kBarPQ2 + c), ph_p[c]);
                 PROF_TRACE(0, tr_step, 7 + 2 * c);
                 tc_fence_after();
 #pragma unroll
                 for (int k = kTileN / 32; k < 3 * kTileN / 64; ++k)
-                    umma_ts(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
+                    umma_ts_lo<kDescHi>(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
                             vd + k * ((kBlock * 128) >> 4), idesc_o, 1u);
                 mbar_wait(bar(kBarPQ3 + c), ph_p[c]);
                 PROF_TRACE(0, tr_step, 8 + 2 * c);
@@ -673,7 +686,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                 tc_fence_after();
 #pragma unroll
                 for (int k = 3 * kTileN / 64; k < kTileN / 16; ++k)
-                    umma_ts(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
+                    umma_ts_lo<kDescHi>(tmem + C::kColO + c * C::kChainCols, tmem + C::kColS + c * C::kChainCols + k * 8,
                             vd + k * ((kBlock * 128) >> 4), idesc_o, 1u);
             };
             auto pv = [&](int c, uint32_t vslot, bool first) {
