@@ -204,6 +204,7 @@ int msa_create(const msa_config *cfg, msa_handle *out)
     DeviceGuard guard(cfg->device);
     cudaError_t e = guard.err;
     if (e == cudaSuccess) e = configure_fwd(cfg->head_dim);     // per device: a second handle on another GPU sets its own
+    if (e == cudaSuccess) e = configure_append();
     if (e == cudaSuccess) e = cudaMalloc(&h->d_kv_to_q, h->kv_to_q.size() * sizeof(int32_t));
     if (e == cudaSuccess)
         e = cudaMemcpy(h->d_kv_to_q, h->kv_to_q.data(), h->kv_to_q.size() * sizeof(int32_t), cudaMemcpyHostToDevice);

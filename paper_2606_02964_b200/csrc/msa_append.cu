@@ -1,18 +1,69 @@
-// KV write-back (include/msa.h, msa_kv_append): arena rows -> paged cache blocks, 16 tokens per copy unit.
-// HBM-bound copy: every byte is read once and written once with 16-byte accesses.  One copy unit is 16 tokens x
-// (Hkv*D*2) bytes for each of K and V -- contiguous on both sides -- so a block walks its unit in chunks of
-// kInFlight x 16 bytes per thread and tensor: all loads of a chunk are issued before the first store (the copy is
-// latency-bound otherwise: a 64 KB unit is only a handful of trips per thread).
+// KV write-back as its own launch (include/msa.h, msa_kv_append): arena rows -> paged cache blocks, 16 tokens per copy
+// unit.  HBM-bound copy: every byte is read once and written once.  A copy unit is contiguous on both sides (up to
+// 16 rows x Hkv*D*2 bytes per tensor), so each persistent CTA moves whole units with the bulk-copy engine:
+// cp.async.bulk global -> shared (mbarrier completion), then shared -> global (bulk async-group), kStages units in flight.
+// One thread per CTA issues everything; the SM's other resources stay idle.
 #include "msa_kernels.h"
+#include "msa_ptx.cuh"
 
 namespace msa {
 
+constexpr int kAppendStages = 3;
+constexpr int kAppendMaxUnitBytes = 2 * 16 * 2048;     // K + V of one unit at Hkv*D*2 <= 2048 bytes per row (else the fallback kernel)
+
+__global__ void __launch_bounds__(32) msa_kv_append_bulk_kernel(const AppendParams P)
+{
+    extern __shared__ __align__(128) uint8_t smem[];
+    __shared__ uint64_t full[kAppendStages];
+    if (threadIdx.x != 0) return;
+    const uint32_t rb = static_cast<uint32_t>(P.row_bytes);
+    const uint32_t stage_bytes = 2u * 16u * rb;
+    for (int s = 0; s < kAppendStages; ++s) mbar_init(smem_u32(&full[s]), 1);
+    fence_mbar_init();
+    const int first = blockIdx.x, stride = gridDim.x;
+    const int n_mine = first < P.n_units ? (P.n_units - first + stride - 1) / stride : 0;
+    auto load = [&](int i) {          // i-th unit of this CTA -> stage i % kAppendStages
+        const int s = i % kAppendStages;
+        const AppendUnit un = P.units[first + i * stride];
+        const uint32_t bytes = static_cast<uint32_t>(un.nvalid) * rb;
+        const uint32_t dst = smem_u32(smem) + s * stage_bytes, bar = smem_u32(&full[s]);
+        const uint8_t *sk = static_cast<const uint8_t *>(P.contig_k) + un.src_row * P.row_bytes;
+        const uint8_t *sv = static_cast<const uint8_t *>(P.contig_v) + un.src_row * P.row_bytes;
+        mbar_arrive_expect_tx(bar, 2u * bytes);
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"(dst), "l"(sk), "r"(bytes), "r"(bar) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"(dst + 16u * rb), "l"(sv), "r"(bytes), "r"(bar) : "memory");
+    };
+    for (int i = 0; i < n_mine && i < kAppendStages - 1; ++i) load(i);
+    for (int i = 0; i < n_mine; ++i) {
+        const int s = i % kAppendStages;
+        // the stage that unit i + kStages - 1 will use was stored from by unit i - 1: its stores must have read it
+        if (i + kAppendStages - 1 < n_mine) {
+            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+            load(i + kAppendStages - 1);
+        }
+        mbar_wait(smem_u32(&full[s]), static_cast<uint32_t>(i / kAppendStages) & 1u);
+        const AppendUnit un = P.units[first + i * stride];
+        const uint32_t bytes = static_cast<uint32_t>(un.nvalid) * rb;
+        const int64_t dst_row = static_cast<int64_t>(__ldg(P.block_table + un.bt_index)) * kBlock;
+        uint8_t *dk = static_cast<uint8_t *>(P.pool_k) + dst_row * P.row_bytes;
+        uint8_t *dv = static_cast<uint8_t *>(P.pool_v) + dst_row * P.row_bytes;
+        const uint32_t src = smem_u32(smem) + s * stage_bytes;
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dk), "r"(src), "r"(bytes) : "memory");
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dv), "r"(src + 16u * rb), "r"(bytes) : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    }
+    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+}
+
+// Fallback for rows wider than 2 KB: 16-byte loads and stores, 8 loads in flight per thread before the first store.
 constexpr int kAppendThreads = 256;
-constexpr int kInFlight = 4;          // uint4 per thread, tensor and trip
+constexpr int kInFlight = 4;
 
 __global__ void __launch_bounds__(kAppendThreads) msa_kv_append_kernel(const AppendParams P)
 {
-    const int64_t row_vec = P.row_bytes / 16;                     // uint4 per token row (Hkv * D * 2 / 16)
+    const int64_t row_vec = P.row_bytes / 16;
     for (int u = blockIdx.x; u < P.n_units; u += gridDim.x) {
         const AppendUnit un = P.units[u];
         const int64_t dst_row = static_cast<int64_t>(__ldg(P.block_table + un.bt_index)) * kBlock;
@@ -27,7 +78,7 @@ __global__ void __launch_bounds__(kAppendThreads) msa_kv_append_kernel(const App
             for (int j = 0; j < kInFlight; ++j) {
                 const int64_t i = base + j * kAppendThreads + threadIdx.x;
                 if (i < n) {
-                    a[j] = __ldcs(sk + i);                         // streaming: read once
+                    a[j] = __ldcs(sk + i);
                     b[j] = __ldcs(sv + i);
                 }
             }
@@ -43,11 +94,22 @@ __global__ void __launch_bounds__(kAppendThreads) msa_kv_append_kernel(const App
     }
 }
 
+cudaError_t configure_append()
+{
+    return cudaFuncSetAttribute(msa_kv_append_bulk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                kAppendStages * kAppendMaxUnitBytes);
+}
+
 cudaError_t launch_append(const AppendParams &p, int num_sms, cudaStream_t stream)
 {
     if (p.n_units <= 0) return cudaSuccess;
-    const int grid = p.n_units < num_sms * 8 ? p.n_units : num_sms * 8;
-    msa_kv_append_kernel<<<grid, kAppendThreads, 0, stream>>>(p);
+    if (2 * 16 * p.row_bytes <= kAppendMaxUnitBytes) {
+        const int grid = p.n_units < num_sms ? p.n_units : num_sms;
+        msa_kv_append_bulk_kernel<<<grid, 32, kAppendStages * 2 * 16 * static_cast<size_t>(p.row_bytes), stream>>>(p);
+    } else {
+        const int grid = p.n_units < num_sms * 8 ? p.n_units : num_sms * 8;
+        msa_kv_append_kernel<<<grid, kAppendThreads, 0, stream>>>(p);
+    }
     return cudaGetLastError();
 }
 

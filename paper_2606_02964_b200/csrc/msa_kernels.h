@@ -57,6 +57,7 @@ struct AppendParams {
     int32_t n_units;
 };
 
+cudaError_t configure_append();   // per device, like configure_fwd
 cudaError_t launch_append(const AppendParams &p, int num_sms, cudaStream_t stream);
 
 // Forward kernel: persistent, warp-specialised (msa_fwd_pipe.cuh).  configure_fwd sets the kernel's dynamic
