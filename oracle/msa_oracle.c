@@ -36,6 +36,15 @@
  * copy; segment-cut / block-table-permutation invariance; LSE-merge identity; closed
  * forms (uniform scores -> mean of V and ln n; V==1; V[0]=position -> p/2; position 0);
  * future-independence; key-shift invariance; Eq. (4) pair counts.
+ *
+ * fp8 KV pool (motive: the KV footprint; reading c20):
+ * msa_oracle_forward_kv8 is the same definition with the PAGED pool stored as OCP FP8 E4M3 bytes
+ * (1 sign, 4 exponent bits with bias 7, 3 mantissa bits; no infinities; S.1111.111 = NaN) and one
+ * fp32 scale per KV head for K and for V:  K_j[kvh][d] = e4m3(byte) * k_scale[kvh], likewise V.  The
+ * arena (CONTIG / SELF) stays bf16.  Dequantisation happens here, in fp64, from the same bytes the
+ * CUDA path reads.  Pins: all 256 codes against torch's float8_e4m3fn -> float conversion and the
+ * format's closed forms (448, 2^-9, 1.0); the whole function against msa_oracle_forward on a pool
+ * that holds the dequantised values as bf16 (exact for power-of-two scales).
  */
 #include <math.h>
 #include <stdint.h>
@@ -55,6 +64,18 @@ static double bf16_to_double(uint16_t h)
     return (double)f;
 }
 
+/* OCP FP8 E4M3 ("e4m3fn"): value = (-1)^s * 2^(e-7) * (1 + m/8) for e in 1..15, (-1)^s * 2^-6 * (m/8) for e = 0;
+ * the code with e = 15, m = 7 is NaN; there is no infinity (the largest finite value is 448). */
+double msa_oracle_e4m3_to_double(uint8_t b)
+{
+    const int s = b >> 7, e = (b >> 3) & 15, m = b & 7;
+    double v;
+    if (e == 15 && m == 7) return NAN;
+    if (e == 0) v = ldexp((double)m / 8.0, -6);
+    else v = ldexp(1.0 + (double)m / 8.0, e - 7);
+    return s ? -v : v;
+}
+
 int msa_oracle_num_threads(void)
 {
 #ifdef _OPENMP
@@ -69,10 +90,11 @@ int msa_oracle_num_threads(void)
  * run), grouped by request in any order.  O is [n_rows][Hq][D] doubles, LSE [n_rows][Hq].
  * Returns 0, or -1 on allocation failure, -2 on a malformed descriptor.
  */
-int msa_oracle_forward(
+static int forward_impl(
     int Hq, int Hkv, int D, const int32_t *q_to_kv,
     const uint16_t *q,                                   /* bf16 [total_q][Hq][D]          */
-    const uint16_t *pool_k, const uint16_t *pool_v,      /* bf16 [num_blocks][16][Hkv][D]  */
+    const void *pool_k_any, const void *pool_v_any,      /* [num_blocks][16][Hkv][D]: bf16, or e4m3 bytes when kv8 */
+    int kv8, const float *k_scale, const float *v_scale, /* kv8: fp32 scale per KV head    */
     const int32_t *block_table,
     const uint16_t *contig_k, const uint16_t *contig_v,  /* bf16 [rows][Hkv][D]            */
     int n_req, const int32_t *req_q_row_start, const int32_t *req_q_len,
@@ -84,6 +106,8 @@ int msa_oracle_forward(
     double *O, double *LSE)
 {
     const double scale_d = (double)scale;
+    const uint16_t *pool_k = (const uint16_t *)pool_k_any, *pool_v = (const uint16_t *)pool_v_any;
+    const uint8_t *pool_k8 = (const uint8_t *)pool_k_any, *pool_v8 = (const uint8_t *)pool_v_any;
     for (int r = 0; r < n_req; ++r) {
         /* any row of this request asked for? */
         int64_t wanted = 0;
@@ -111,6 +135,17 @@ int msa_oracle_forward(
             for (int idx = 0; idx < seg_len[s]; ++idx) {
                 const int64_t j = base + idx;
                 const uint16_t *ksrc, *vsrc;
+                pos[j] = (int64_t)seg_abs_start[s] + idx;
+                if (seg_kind[s] == 0 && kv8) {   /* paged, fp8 pool: e4m3 byte times the KV head's scale */
+                    int64_t blk = block_table[seg_block_off[s] + idx / ORACLE_BLOCK];
+                    size_t off = ((size_t)blk * ORACLE_BLOCK + (size_t)(idx % ORACLE_BLOCK)) * per_tok;
+                    for (size_t e = 0; e < per_tok; ++e) {
+                        const size_t kvh = e / (size_t)D;
+                        Kc[(size_t)j * per_tok + e] = msa_oracle_e4m3_to_double(pool_k8[off + e]) * (double)k_scale[kvh];
+                        Vc[(size_t)j * per_tok + e] = msa_oracle_e4m3_to_double(pool_v8[off + e]) * (double)v_scale[kvh];
+                    }
+                    continue;
+                }
                 if (seg_kind[s] == 0) {          /* paged: through the block table */
                     int64_t blk = block_table[seg_block_off[s] + idx / ORACLE_BLOCK];
                     size_t off = ((size_t)blk * ORACLE_BLOCK + (size_t)(idx % ORACLE_BLOCK)) * per_tok;
@@ -121,7 +156,6 @@ int msa_oracle_forward(
                     ksrc = contig_k + off;
                     vsrc = contig_v + off;
                 }
-                pos[j] = (int64_t)seg_abs_start[s] + idx;
                 for (size_t e = 0; e < per_tok; ++e) {
                     Kc[(size_t)j * per_tok + e] = bf16_to_double(ksrc[e]);
                     Vc[(size_t)j * per_tok + e] = bf16_to_double(vsrc[e]);
@@ -180,4 +214,45 @@ int msa_oracle_forward(
         if (fail) return -1;
     }
     return 0;
+}
+
+int msa_oracle_forward(
+    int Hq, int Hkv, int D, const int32_t *q_to_kv,
+    const uint16_t *q,                                   /* bf16 [total_q][Hq][D]          */
+    const uint16_t *pool_k, const uint16_t *pool_v,      /* bf16 [num_blocks][16][Hkv][D]  */
+    const int32_t *block_table,
+    const uint16_t *contig_k, const uint16_t *contig_v,  /* bf16 [rows][Hkv][D]            */
+    int n_req, const int32_t *req_q_row_start, const int32_t *req_q_len,
+    const int32_t *req_q_abs_start, const int32_t *req_seg_begin, const int32_t *req_seg_count,
+    const int32_t *seg_kind, const int32_t *seg_abs_start, const int32_t *seg_len,
+    const int32_t *seg_block_off, const int64_t *seg_row_off,
+    float scale,
+    int64_t n_rows, const int32_t *row_req, const int32_t *row_idx,
+    double *O, double *LSE)
+{
+    return forward_impl(Hq, Hkv, D, q_to_kv, q, pool_k, pool_v, 0, NULL, NULL, block_table, contig_k, contig_v, n_req,
+                        req_q_row_start, req_q_len, req_q_abs_start, req_seg_begin, req_seg_count, seg_kind, seg_abs_start,
+                        seg_len, seg_block_off, seg_row_off, scale, n_rows, row_req, row_idx, O, LSE);
+}
+
+/* The same with an fp8 (E4M3) paged pool: pool_k / pool_v are bytes [num_blocks][16][Hkv][D], k_scale / v_scale
+ * fp32 [Hkv]; everything else as above. */
+int msa_oracle_forward_kv8(
+    int Hq, int Hkv, int D, const int32_t *q_to_kv,
+    const uint16_t *q,
+    const uint8_t *pool_k, const uint8_t *pool_v, const float *k_scale, const float *v_scale,
+    const int32_t *block_table,
+    const uint16_t *contig_k, const uint16_t *contig_v,
+    int n_req, const int32_t *req_q_row_start, const int32_t *req_q_len,
+    const int32_t *req_q_abs_start, const int32_t *req_seg_begin, const int32_t *req_seg_count,
+    const int32_t *seg_kind, const int32_t *seg_abs_start, const int32_t *seg_len,
+    const int32_t *seg_block_off, const int64_t *seg_row_off,
+    float scale,
+    int64_t n_rows, const int32_t *row_req, const int32_t *row_idx,
+    double *O, double *LSE)
+{
+    if (!k_scale || !v_scale) return -2;
+    return forward_impl(Hq, Hkv, D, q_to_kv, q, pool_k, pool_v, 1, k_scale, v_scale, block_table, contig_k, contig_v, n_req,
+                        req_q_row_start, req_q_len, req_q_abs_start, req_seg_begin, req_seg_count, seg_kind, seg_abs_start,
+                        seg_len, seg_block_off, seg_row_off, scale, n_rows, row_req, row_idx, O, LSE);
 }

@@ -39,12 +39,20 @@ def _load() -> ctypes.CDLL:
     if _lib is None:
         _lib = ctypes.CDLL(build())
         _lib.msa_oracle_forward.restype = ctypes.c_int
+        _lib.msa_oracle_forward_kv8.restype = ctypes.c_int
+        _lib.msa_oracle_e4m3_to_double.restype = ctypes.c_double
+        _lib.msa_oracle_e4m3_to_double.argtypes = [ctypes.c_uint8]
         _lib.msa_oracle_num_threads.restype = ctypes.c_int
     return _lib
 
 
 def num_threads() -> int:
     return int(_load().msa_oracle_num_threads())
+
+
+def e4m3_to_double(code: int) -> float:
+    """Value of one OCP FP8 E4M3 code (the oracle's own decoder, written from the format's definition)."""
+    return float(_load().msa_oracle_e4m3_to_double(ctypes.c_uint8(int(code) & 0xff)))
 
 
 def _ptr(a: Optional[np.ndarray]):
@@ -61,18 +69,30 @@ def forward(a: Dict[str, np.ndarray], Hq: int, Hkv: int, D: int, scale: float,
     n = int(row_req.shape[0])
     O = np.zeros((n, Hq, D), np.float64)
     LSE = np.zeros((n, Hq), np.float64)
+    kv8 = a.get("k_scale") is not None      # fp8 (E4M3) paged pool: bytes + one fp32 scale per KV head
+    pool_dt = np.uint8 if kv8 else np.uint16
+    if kv8:
+        assert a["pool_k"].dtype == np.uint8 and a["pool_v"].dtype == np.uint8
     keep = dict(
         q=np.ascontiguousarray(a["q"], np.uint16),
-        pool_k=np.ascontiguousarray(a["pool_k"], np.uint16), pool_v=np.ascontiguousarray(a["pool_v"], np.uint16),
+        pool_k=np.ascontiguousarray(a["pool_k"], pool_dt), pool_v=np.ascontiguousarray(a["pool_v"], pool_dt),
         bt=np.ascontiguousarray(a["block_table"], np.int32),
         ck=np.ascontiguousarray(a["contig_k"], np.uint16), cv=np.ascontiguousarray(a["contig_v"], np.uint16),
         sk=np.ascontiguousarray(a["seg_kind"], np.int32), sa=np.ascontiguousarray(a["seg_abs_start"], np.int32),
         sl=np.ascontiguousarray(a["seg_len"], np.int32), sb=np.ascontiguousarray(a["seg_block_off"], np.int32),
         sr=np.ascontiguousarray(a["seg_row_off"], np.int64),
         hm=None if a.get("q_to_kv") is None else np.ascontiguousarray(a["q_to_kv"], np.int32))
-    rc = lib.msa_oracle_forward(
+    scales = ()
+    fn = lib.msa_oracle_forward
+    if kv8:
+        keep["ks"] = np.ascontiguousarray(a["k_scale"], np.float32)
+        keep["vs"] = np.ascontiguousarray(a["v_scale"], np.float32)
+        assert keep["ks"].shape == (Hkv,) and keep["vs"].shape == (Hkv,)
+        scales = (_ptr(keep["ks"]), _ptr(keep["vs"]))
+        fn = lib.msa_oracle_forward_kv8
+    rc = fn(
         ctypes.c_int(Hq), ctypes.c_int(Hkv), ctypes.c_int(D), _ptr(keep["hm"]),
-        _ptr(keep["q"]), _ptr(keep["pool_k"]), _ptr(keep["pool_v"]), _ptr(keep["bt"]),
+        _ptr(keep["q"]), _ptr(keep["pool_k"]), _ptr(keep["pool_v"]), *scales, _ptr(keep["bt"]),
         _ptr(keep["ck"]), _ptr(keep["cv"]),
         ctypes.c_int(req.shape[0]), _ptr(cols[0]), _ptr(cols[1]), _ptr(cols[2]), _ptr(cols[3]), _ptr(cols[4]),
         _ptr(keep["sk"]), _ptr(keep["sa"]), _ptr(keep["sl"]), _ptr(keep["sb"]), _ptr(keep["sr"]),

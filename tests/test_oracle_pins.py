@@ -360,3 +360,72 @@ def test_generator_recipes_are_deterministic_and_well_formed():
     assert 0.55 <= cached <= 0.65 and c3.n_seg == 9
     c5 = W.cfg5_short_query(layout_only=True)
     assert c5.n_req == 256 and c5.req[:, 1].min() >= 1 and c5.req[:, 1].max() <= 8
+
+
+# ---------------------------------------------------------------- P10: fp8 (E4M3) paged pool (reading c20)
+def test_p10_e4m3_decoder_against_torch_and_the_formats_closed_forms():
+    """The oracle's own E4M3 decoder: every one of the 256 codes against torch's float8_e4m3fn -> float32 conversion
+    (a library routine that shares nothing with the oracle) and against what the OCP format fixes."""
+    codes = torch.arange(256, dtype=torch.int32).to(torch.uint8)
+    ref = codes.view(torch.float8_e4m3fn).float().numpy().astype(np.float64)
+    mine = np.array([oracle.e4m3_to_double(c) for c in range(256)])
+    nan = np.isnan(ref)
+    assert nan.sum() == 2 and np.isnan(mine[0x7f]) and np.isnan(mine[0xff])        # S.1111.111, no infinities
+    assert np.array_equal(np.isnan(mine), nan)
+    assert np.array_equal(mine[~nan], ref[~nan])
+    assert np.array_equal(np.signbit(mine[~nan]), np.signbit(ref[~nan]))            # -0 keeps its sign
+    # closed forms: largest finite 448 = 2^8 * 1.75, smallest subnormal 2^-9, smallest normal 2^-6, one
+    assert mine[0x7e] == 448.0 and mine[0xfe] == -448.0
+    assert mine[0x01] == 2.0 ** -9 and mine[0x07] == 7 * 2.0 ** -9 and mine[0x08] == 2.0 ** -6
+    assert mine[0x38] == 1.0 and mine[0x3c] == 1.5 and mine[0x40] == 2.0
+    # monotone over the positive codes
+    assert np.all(np.diff(mine[:0x7f]) > 0)
+
+
+def _dequantised_twin(p8):
+    """bf16 problem whose pool holds code * scale (exact in bf16 for power-of-two scales), made with torch's decoder."""
+    import copy
+    p = copy.copy(p8)
+    for name, sc in (("pool_k", p8.k_scale), ("pool_v", p8.v_scale)):
+        codes = getattr(p8, name)
+        val = codes.view(torch.float8_e4m3fn).float() * torch.from_numpy(np.asarray(sc, np.float32))[None, None, :, None]
+        assert torch.equal(val.to(torch.bfloat16).float()[torch.isfinite(val)], val[torch.isfinite(val)])
+        setattr(p, name, val.to(torch.bfloat16))
+    p.k_scale = p.v_scale = None
+    return p
+
+
+@pytest.mark.parametrize("seed", [5, 6, 7])
+def test_p10_kv8_forward_equals_the_bf16_oracle_on_the_dequantised_pool(seed):
+    """msa_oracle_forward_kv8 = msa_oracle_forward (pinned by P1-P9) on a pool that holds the dequantised values:
+    a wrong scale index, K / V scale swapped, a wrong byte offset or a decoder slip changes the result."""
+    p = W.random_problem(seed, n_req=3, Hq=8, Hkv=4, D=64, max_ctx=300, max_q=40, keep_dense=False)
+    p8 = W.to_fp8_pool(p, k_exp=[-6, -5, -7, -4], v_exp=[-5, -6, -3, -7])          # different scale per head, K != V
+    O8, L8 = oracle.forward_problem(p8)
+    O, L = oracle.forward_problem(_dequantised_twin(p8))
+    assert np.array_equal(O8, O) and np.array_equal(L8, L)
+    # and it is not the bf16 problem's result (quantisation moved the values) nor scale-blind
+    O0, _ = oracle.forward_problem(p)
+    assert np.abs(O8 - O0).max() > 1e-3
+    p8b = W.to_fp8_pool(p, k_exp=[-6, -5, -7, -4], v_exp=[-5, -6, -3, -7])
+    p8b.v_scale = p8b.v_scale * 2
+    Ob, Lb = oracle.forward_problem(p8b)
+    assert np.abs(Ob - O8).max() > 1e-3 and np.array_equal(Lb, L8)                  # V's scale moves O, never LSE
+
+
+def test_p10_kv8_scale_closed_form():
+    """Only paged segments: doubling v_scale doubles O exactly; multiplying k_scale by 2 equals doubling the softmax scale."""
+    ctx = ContextSpec([(SEG_PAGED, 0, 75)])
+    p = build_problem("kv8_only_paged", 4, 2, 64, [ctx], [RunSpec(0, 70, 5)], seed=77)
+    p8 = W.to_fp8_pool(p, k_exp=[-6, -6], v_exp=[-6, -6])
+    O, L = oracle.forward_problem(p8)
+    p8.v_scale = p8.v_scale * 2
+    O2, L2 = oracle.forward_problem(p8)
+    assert np.array_equal(O2, 2 * O) and np.array_equal(L2, L)
+    p8.v_scale = p8.v_scale / 2
+    p8.k_scale = p8.k_scale * 2
+    O3, L3 = oracle.forward_problem(p8)
+    p8.k_scale = p8.k_scale / 2
+    p8.scale = float(np.float32(p8.scale * 2))
+    O4, L4 = oracle.forward_problem(p8)
+    assert np.allclose(O3, O4, atol=1e-13) and np.allclose(L3, L4, atol=1e-12)

@@ -11,5 +11,5 @@ from .msa_inputs import (  # noqa: F401
     ContextSpec, RunSpec, MsaProblem,
     build_problem, random_problem,
     cfg1_tiny, cfg2_llama8b, cfg3_70b_long, cfg4_mixed, cfg5_short_query, f1_hybrid_pod, f2_fig13,
-    CONFIGS, EXTRA_CONFIGS, pick_rows, visible_pairs,
+    CONFIGS, EXTRA_CONFIGS, pick_rows, visible_pairs, to_fp8_pool,
 )

@@ -79,6 +79,10 @@ class MsaProblem:
     # list of dict(pos=int64[n], k=bf16[n,Hkv,D], v=bf16[n,Hkv,D]) in ascending position
     dense: Optional[List[Dict[str, torch.Tensor]]] = None
     run_ctx: Optional[np.ndarray] = None       # int32 [n_req] context index of each run
+    # fp8 paged pool: pool_k / pool_v are uint8 [num_blocks,16,Hkv,D] holding OCP E4M3 codes and
+    # k_scale / v_scale float32 [Hkv] (powers of two) -- see to_fp8_pool(); None for a bf16 pool
+    k_scale: Optional[np.ndarray] = None
+    v_scale: Optional[np.ndarray] = None
     notes: Dict[str, object] = field(default_factory=dict)
 
     # ---- convenience -----------------------------------------------------
@@ -99,13 +103,15 @@ class MsaProblem:
             return self.q_to_kv.astype(np.int32)
         return (np.arange(self.Hq, dtype=np.int32) // self.G).astype(np.int32)
 
-    def kv_tokens(self) -> int:
-        """Tokens of K/V a launch must read at least once per KV head (sum over runs)."""
+    def kv_tokens(self, kind: Optional[int] = None) -> int:
+        """Tokens of K/V a launch must read at least once per KV head (sum over runs); `kind`: only segments of that kind."""
         tot = 0
         for r in range(self.n_req):
             _, q_len, q_abs, sb, sc = (int(x) for x in self.req[r])
             p_last = q_abs + q_len - 1
             for s in range(sb, sb + sc):
+                if kind is not None and int(self.seg_kind[s]) != kind:
+                    continue
                 a, n = int(self.seg_abs_start[s]), int(self.seg_len[s])
                 tot += max(0, min(n, p_last - a + 1))
         return tot
@@ -116,6 +122,8 @@ class MsaProblem:
         pairs = visible_pairs(self)
         kv_tok = self.kv_tokens()
         kv_bytes = kv_tok * self.Hkv * self.D * 2 * 2
+        if self.k_scale is not None:       # fp8 pool: one byte per cached element
+            kv_bytes -= self.kv_tokens(SEG_PAGED) * self.Hkv * self.D * 2
         qo_bytes = self.total_q * self.Hq * self.D * 2 * 2 + self.total_q * self.Hq * 4
         id_bytes = int(self.block_table_np.size) * 4
         return dict(pairs_per_head=pairs, flops=4.0 * self.D * self.Hq * pairs,
@@ -130,8 +138,11 @@ class MsaProblem:
         read by a correct gather)."""
         assert self.q is not None, "layout_only problem has no values"
         big = (self.pool_k.numel() + self.contig_k.numel()) * 2 > (1 << 30)
+        kv8 = self.k_scale is not None
 
         def u16(t: torch.Tensor) -> np.ndarray:
+            if t.dtype == torch.uint8:      # fp8 pool: the E4M3 codes as they are
+                return t.detach().cpu().contiguous().numpy()
             return t.detach().cpu().contiguous().view(torch.int16).numpy().view(np.uint16)
 
         out: Dict[str, np.ndarray] = dict(
@@ -139,12 +150,14 @@ class MsaProblem:
             req=self.req, seg_kind=self.seg_kind, seg_abs_start=self.seg_abs_start,
             seg_len=self.seg_len, seg_block_off=self.seg_block_off, seg_row_off=self.seg_row_off,
             q_to_kv=self.head_map())
+        if kv8:
+            out.update(k_scale=np.asarray(self.k_scale, np.float32), v_scale=np.asarray(self.v_scale, np.float32))
         if not big or reqs is None:
             out.update(pool_k=u16(self.pool_k), pool_v=u16(self.pool_v),
                        contig_k=u16(self.contig_k), contig_v=u16(self.contig_v))
             return out
-        pk = np.empty(tuple(self.pool_k.shape), np.uint16)
-        pv = np.empty(tuple(self.pool_v.shape), np.uint16)
+        pk = np.empty(tuple(self.pool_k.shape), np.uint8 if kv8 else np.uint16)
+        pv = np.empty(tuple(self.pool_v.shape), np.uint8 if kv8 else np.uint16)
         ck = np.empty(tuple(self.contig_k.shape), np.uint16)
         cv = np.empty(tuple(self.contig_v.shape), np.uint16)
         blk_ids: List[np.ndarray] = []
@@ -359,6 +372,41 @@ def build_problem(name: str, Hq: int, Hkv: int, D: int,
     p.pool_k, p.pool_v = pool_k.to(device), pool_v.to(device)
     p.contig_k, p.contig_v = ck.to(device), cv.to(device)
     return p
+
+
+# --------------------------------------------------------------------------- fp8 paged pool
+def to_fp8_pool(p: MsaProblem, k_exp: Optional[Sequence[int]] = None, v_exp: Optional[Sequence[int]] = None) -> MsaProblem:
+    """The same problem with its paged pool stored as OCP FP8 E4M3 codes (KV footprint).
+
+    k_exp / v_exp: per KV head, the power of two of the scale (k_scale[h] = 2**k_exp[h]); default: the smallest power of two
+    that brings the head's largest |value| within E4M3's 448, so every head uses the format's full range.  The codes are
+    produced with torch's float8_e4m3fn conversion (round to nearest even) of value / scale: this is input generation --
+    both the oracle and the CUDA path start from the bytes.  Descriptors, q and the arena are shared with ``p``."""
+    import copy
+    assert p.pool_k is not None and p.pool_k.dtype == torch.bfloat16
+    out = copy.copy(p)
+    out.name = p.name + "_kv8"
+    out.dense = None                         # the un-segmented bf16 copy no longer describes the pool
+
+    def quant(pool: torch.Tensor, exps: Optional[Sequence[int]]):
+        codes = torch.empty(pool.shape, dtype=torch.uint8, device=pool.device)
+        scales = np.zeros(p.Hkv, np.float32)
+        for h in range(p.Hkv):
+            x = pool[:, :, h, :].float()
+            fin = torch.where(torch.isfinite(x), x.abs(), torch.zeros_like(x))
+            if exps is None:
+                amax = float(fin.max()) if fin.numel() else 1.0
+                e = int(math.ceil(math.log2(max(amax, 2.0 ** -20) / 448.0)))
+            else:
+                e = int(exps[h])
+            scales[h] = np.float32(2.0 ** e)
+            y = (x * (2.0 ** -e)).clamp(-448.0, 448.0)          # NaN stays NaN (poisoned slack in the tests)
+            codes[:, :, h, :] = y.to(torch.float8_e4m3fn).view(torch.uint8)
+        return codes, scales
+
+    out.pool_k, out.k_scale = quant(p.pool_k, k_exp)
+    out.pool_v, out.v_scale = quant(p.pool_v, v_exp)
+    return out
 
 
 # --------------------------------------------------------------------------- random problems
