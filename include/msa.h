@@ -43,7 +43,9 @@ enum {
     MSA_OK = 0,
     MSA_ERR_INVALID_ARG = -1,      /* NULL pointer, negative size, non-positive / non-finite scale */
     MSA_ERR_UNSUPPORTED = -2,      /* head_dim not in {64,128}, block_size != 16, Hq % Hkv != 0, G > 16,
-                                      head map that does not give every KV head exactly G q heads */
+                                      head map that does not give every KV head exactly G q heads, an fp8 pool
+                                      scale that is not a power of two in [2^-14, 2^14], KV write-back into an
+                                      fp8 pool through the forward launch */
     MSA_ERR_OVERLAP = -3,          /* segments of one request overlap in absolute position, or two
                                       requests write the same q rows */
     MSA_ERR_UNSORTED = -4,         /* segments of one request not in ascending abs_start */
@@ -60,6 +62,18 @@ enum {
  *   SELF   -- the current chunk's own K/V, also rows of the contiguous arena           */
 enum { MSA_SEG_PAGED = 0, MSA_SEG_CONTIG = 1, MSA_SEG_SELF = 2 };
 
+/* Storage format of the paged pool (the KV cache; its footprint is what limits how much context stays resident,
+ * PAPER.md:22).  The arena (recomputed runs, own chunk) and q / o are always bf16.
+ *   MSA_POOL_BF16      bf16 elements
+ *   MSA_POOL_FP8_E4M3  one byte per element, OCP FP8 E4M3 (1 sign, 4 exponent bits with bias 7, 3 mantissa bits, no
+ *                      infinity, S.1111.111 = NaN), and one scale per KV head for K and one for V:
+ *                          K_j[kvh][d] = e4m3(pool_k byte) * k_scale[kvh],   V_j[kvh][d] = e4m3(pool_v byte) * v_scale[kvh]
+ *                      The scales must be powers of two in [2^-14, 2^14] (as in the OCP MX formats): the dequantised
+ *                      value is then exactly a bf16, the kernel converts the codes on chip and the result is the bf16
+ *                      path's result on the dequantised pool -- same tolerances.  A NaN code dequantises to an
+ *                      unspecified finite value (non-finite K/V are outside the definition, DESIGN.md c19). */
+enum { MSA_POOL_BF16 = 0, MSA_POOL_FP8_E4M3 = 1 };
+
 typedef struct {
     int32_t num_q_heads;           /* Hq                                                     */
     int32_t num_kv_heads;          /* Hkv, divides Hq; G = Hq/Hkv <= 16                      */
@@ -67,6 +81,9 @@ typedef struct {
     int32_t block_size;            /* must be 16                                             */
     const int32_t *q_to_kv_head;   /* host int32[Hq] GQA head map, or NULL => h / G (Llama)  */
     int32_t device;                /* CUDA device ordinal                                    */
+    int32_t pool_format;           /* MSA_POOL_BF16 (0) or MSA_POOL_FP8_E4M3                 */
+    const float *k_scale;          /* fp8 pool: host fp32[Hkv] (copied); NULL => all 1.0     */
+    const float *v_scale;          /* fp8 pool: host fp32[Hkv] (copied); NULL => all 1.0     */
 } msa_config;
 
 typedef struct {
@@ -145,7 +162,8 @@ int msa_workspace_bytes(msa_plan p, size_t *bytes);
  * stream).  Never allocates, never synchronises, never reads device memory on the host.
  *
  *   q            device bf16 [total_q][Hq][D]
- *   pool_k/v     device bf16 [num_blocks][16][Hkv][D]      (paged KV cache)
+ *   pool_k/v     device bf16 [num_blocks][16][Hkv][D]      (paged KV cache; E4M3 bytes of the same shape when the
+ *                                                          handle was created with MSA_POOL_FP8_E4M3)
  *   block_table  device int32 [block_table_len], physical block ids in logical order
  *   contig_k/v   device bf16 [contig_rows][Hkv][D]         (recomputed runs + own chunk)
  *   o            device bf16 [total_q][Hq][D]   (written for every row of every run)
@@ -204,6 +222,9 @@ void msa_append_plan_destroy(msa_append_plan ap);
  * in msa_forward, except that the pool is written.  The destination blocks must not be read by a kernel running
  * concurrently on another stream.  MSA_ERR_OUT_OF_RANGE if a job exceeds contig_rows or block_table_len (block ids
  * themselves are trusted, they live on the device); MSA_ERR_MISALIGNED for pointers not 16-byte aligned. */
+/* fp8 pool: the rows are quantised on the way, code = E4M3 code nearest to arena value / scale (ties to the even code,
+ * |value / scale| > 448 saturates to +-448, NaN gives the NaN code), so that e4m3(code) * scale is what a later PAGED
+ * segment reads. */
 int msa_kv_append(msa_handle h, msa_append_plan ap,
                   const void *contig_k, const void *contig_v, int64_t contig_rows,
                   void *pool_k, void *pool_v, int64_t num_blocks,

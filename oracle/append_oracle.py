@@ -21,3 +21,29 @@ def kv_append(pool: np.ndarray, arena: np.ndarray, block_table: np.ndarray,
         for i in range(n):
             out[int(block_table[block_off + i // 16]), i % 16] = arena[row_off + i]
     return out
+
+
+def quantize_e4m3(values: np.ndarray, scale: float, decode) -> np.ndarray:
+    """fp8 pool (include/msa.h, msa_kv_append on an MSA_POOL_FP8_E4M3 handle): the E4M3 code nearest to value / scale,
+    ties to the even code, |value / scale| beyond 448 saturates to +-448, NaN gives the NaN code 0x7f.  Written as the
+    definition: a search over the 127 non-negative finite codes, whose values come from `decode` (the oracle's own E4M3
+    decoder, oracle.e4m3_to_double).  Pin (tests/test_kv8.py): torch's float8_e4m3fn conversion inside +-448, closed forms
+    outside it and at the ties."""
+    grid = np.array([decode(c) for c in range(0x7f)], np.float64)          # ascending: code order is value order
+    v = np.asarray(values, np.float64) / float(scale)
+    out = np.zeros(v.shape, np.uint8)
+    flat_v, flat_o = v.reshape(-1), out.reshape(-1)
+    for i, x in enumerate(flat_v):
+        if np.isnan(x):
+            flat_o[i] = 0x7f
+            continue
+        a = abs(x)
+        if a >= grid[-1]:
+            c = 0x7e
+        else:
+            hi = int(np.searchsorted(grid, a, side="left"))                 # grid[hi-1] < a <= grid[hi]
+            lo = max(hi - 1, 0)
+            d_lo, d_hi = a - grid[lo], grid[hi] - a
+            c = lo if d_lo < d_hi else hi if d_hi < d_lo else (lo if lo % 2 == 0 else hi)
+        flat_o[i] = c | (0x80 if np.signbit(x) else 0)
+    return out

@@ -18,12 +18,14 @@ MSA_OK = 0
 MSA_ERR_INVALID_ARG, MSA_ERR_UNSUPPORTED, MSA_ERR_OVERLAP, MSA_ERR_UNSORTED = -1, -2, -3, -4
 MSA_ERR_OUT_OF_RANGE, MSA_ERR_MISALIGNED, MSA_ERR_WORKSPACE, MSA_ERR_CUDA, MSA_ERR_NO_DEVICE = -5, -6, -7, -8, -9
 MSA_SEG_PAGED, MSA_SEG_CONTIG, MSA_SEG_SELF = 0, 1, 2
+MSA_POOL_BF16, MSA_POOL_FP8_E4M3 = 0, 1
 
 
 class MsaConfig(ctypes.Structure):
     _fields_ = [("num_q_heads", ctypes.c_int32), ("num_kv_heads", ctypes.c_int32), ("head_dim", ctypes.c_int32),
                 ("block_size", ctypes.c_int32), ("q_to_kv_head", ctypes.POINTER(ctypes.c_int32)),
-                ("device", ctypes.c_int32)]
+                ("device", ctypes.c_int32), ("pool_format", ctypes.c_int32),
+                ("k_scale", ctypes.POINTER(ctypes.c_float)), ("v_scale", ctypes.POINTER(ctypes.c_float))]
 
 
 class MsaSegment(ctypes.Structure):
@@ -143,12 +145,19 @@ def msa_version() -> str:
 
 
 def msa_create(num_q_heads: int, num_kv_heads: int, head_dim: int, q_to_kv_head=None, device: int = 0,
-               block_size: int = 16) -> ctypes.c_void_p:
-    cfg = MsaConfig(num_q_heads, num_kv_heads, head_dim, block_size, None, device)
+               block_size: int = 16, pool_format: int = MSA_POOL_BF16, k_scale=None, v_scale=None) -> ctypes.c_void_p:
+    """pool_format = MSA_POOL_FP8_E4M3: the paged pool holds E4M3 codes; k_scale / v_scale float32 [Hkv] (powers of two)."""
+    cfg = MsaConfig(num_q_heads, num_kv_heads, head_dim, block_size, None, device, pool_format, None, None)
     keep = None
     if q_to_kv_head is not None:
         keep = np.ascontiguousarray(q_to_kv_head, np.int32)
         cfg.q_to_kv_head = keep.ctypes.data_as(ctypes.POINTER(ctypes.c_int32))
+    keep_s = []
+    for name, sc in (("k_scale", k_scale), ("v_scale", v_scale)):
+        if sc is not None:
+            arr = np.ascontiguousarray(sc, np.float32)
+            keep_s.append(arr)
+            setattr(cfg, name, arr.ctypes.data_as(ctypes.POINTER(ctypes.c_float)))
     h = ctypes.c_void_p()
     _check(_lib().msa_create(ctypes.byref(cfg), ctypes.byref(h)), "msa_create")
     return h
@@ -266,7 +275,10 @@ class MsaSession:
     def __init__(self, problem, device: int = 0):
         import torch
         self.problem = p = problem
-        self.h = msa_create(p.Hq, p.Hkv, p.D, p.q_to_kv, device=device)
+        kv8 = getattr(p, "k_scale", None) is not None       # fp8 (E4M3) paged pool
+        self.h = msa_create(p.Hq, p.Hkv, p.D, p.q_to_kv, device=device,
+                            pool_format=MSA_POOL_FP8_E4M3 if kv8 else MSA_POOL_BF16,
+                            k_scale=p.k_scale if kv8 else None, v_scale=p.v_scale if kv8 else None)
         R, n_req, S, n_seg = make_descriptors(p.req, p.seg_kind, p.seg_abs_start, p.seg_len, p.seg_block_off,
                                               p.seg_row_off)
         self.plan = msa_plan_create(self.h, R, n_req, S, n_seg)

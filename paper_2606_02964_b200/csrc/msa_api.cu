@@ -84,6 +84,10 @@ struct msa_handle_s {
     bool planning_only = false;
     std::vector<int32_t> kv_to_q;      // [Hkv][G]
     int32_t *d_kv_to_q = nullptr;
+    bool kv8 = false;                  // fp8 (E4M3) paged pool
+    std::vector<float> kv_scale;       // kv8: [2][Hkv] K scales then V scales (powers of two)
+    uint32_t *d_kv8_mul = nullptr;     // kv8: [2][Hkv] bf16x2 {2^(112+k), 2^(112+k)} (forward kernel)
+    float *d_kv8_inv = nullptr;        // kv8: [2][Hkv] 1 / scale (quantising msa_kv_append)
     EncodeTiledFn encode = nullptr;
     // Tensor maps depend only on (base pointer, extent) of q / pool / arena: a model calls msa_forward once per
     // layer with the same few pointer sets step after step, so the 23 encoded maps are kept per pointer set.
@@ -162,11 +166,34 @@ int msa_create(const msa_config *cfg, msa_handle *out)
     if (cfg->num_q_heads % cfg->num_kv_heads != 0) return MSA_ERR_UNSUPPORTED;
     const int G = cfg->num_q_heads / cfg->num_kv_heads;
     if (G > MSA_MAX_GROUP) return MSA_ERR_UNSUPPORTED;
+    if (cfg->pool_format != MSA_POOL_BF16 && cfg->pool_format != MSA_POOL_FP8_E4M3) return MSA_ERR_INVALID_ARG;
+    const bool kv8 = cfg->pool_format == MSA_POOL_FP8_E4M3;
+    std::vector<float> kv_scale;
+    std::vector<uint32_t> kv8_mul;
+    std::vector<float> kv8_inv;
+    if (kv8) {
+        // power-of-two scales only: code * 2^k is exactly a bf16, so the on-chip conversion loses nothing
+        for (int which = 0; which < 2; ++which)
+            for (int kv = 0; kv < cfg->num_kv_heads; ++kv) {
+                const float *src = which ? cfg->v_scale : cfg->k_scale;
+                const float sc = src ? src[kv] : 1.f;
+                int e = 0;
+                if (!(sc > 0.f) || !isfinite(sc)) return MSA_ERR_INVALID_ARG;
+                if (frexpf(sc, &e) != 0.5f || e - 1 < -14 || e - 1 > 14) return MSA_ERR_UNSUPPORTED;
+                const uint32_t b = static_cast<uint32_t>(127 + 112 + (e - 1)) << 7;      // bf16 bits of 2^(112 + k)
+                kv_scale.push_back(sc);
+                kv8_mul.push_back(b | (b << 16));
+                kv8_inv.push_back(1.f / sc);
+            }
+    }
 
     msa_handle h = new (std::nothrow) msa_handle_s();
     if (!h) return MSA_ERR_INVALID_ARG;
     h->cfg = *cfg;
     h->cfg.q_to_kv_head = nullptr;
+    h->cfg.k_scale = h->cfg.v_scale = nullptr;
+    h->kv8 = kv8;
+    h->kv_scale = kv_scale;
     h->G = G;
     h->R = (kTileM / G) & ~7;
     // head map -> q heads of each kv head, in ascending q-head order
@@ -203,16 +230,24 @@ int msa_create(const msa_config *cfg, msa_handle *out)
     h->num_sms = prop.multiProcessorCount;
     DeviceGuard guard(cfg->device);
     cudaError_t e = guard.err;
-    if (e == cudaSuccess) e = configure_fwd(cfg->head_dim);     // per device: a second handle on another GPU sets its own
+    if (e == cudaSuccess) e = configure_fwd(cfg->head_dim, kv8);     // per device: a second handle on another GPU sets its own
     if (e == cudaSuccess) e = configure_append();
     if (e == cudaSuccess) e = cudaMalloc(&h->d_kv_to_q, h->kv_to_q.size() * sizeof(int32_t));
     if (e == cudaSuccess)
         e = cudaMemcpy(h->d_kv_to_q, h->kv_to_q.data(), h->kv_to_q.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (kv8) {
+        if (e == cudaSuccess) e = cudaMalloc(&h->d_kv8_mul, kv8_mul.size() * sizeof(uint32_t));
+        if (e == cudaSuccess) e = cudaMemcpy(h->d_kv8_mul, kv8_mul.data(), kv8_mul.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMalloc(&h->d_kv8_inv, kv8_inv.size() * sizeof(float));
+        if (e == cudaSuccess) e = cudaMemcpy(h->d_kv8_inv, kv8_inv.data(), kv8_inv.size() * sizeof(float), cudaMemcpyHostToDevice);
+    }
     void *fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (e == cudaSuccess) e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
     if (e != cudaSuccess || !fn) {
         if (h->d_kv_to_q) cudaFree(h->d_kv_to_q);
+        if (h->d_kv8_mul) cudaFree(h->d_kv8_mul);
+        if (h->d_kv8_inv) cudaFree(h->d_kv8_inv);
         delete h;
         return e != cudaSuccess ? cuda_fail(e, "msa_create") : MSA_ERR_NO_DEVICE;
     }
@@ -227,6 +262,8 @@ void msa_destroy(msa_handle h)
     if (!h->planning_only) {
         DeviceGuard guard(h->cfg.device);
         if (h->d_kv_to_q) cudaFree(h->d_kv_to_q);
+        if (h->d_kv8_mul) cudaFree(h->d_kv8_mul);
+        if (h->d_kv8_inv) cudaFree(h->d_kv8_inv);
         for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
         h->s_q.release(); h->s_o.release(); h->s_lse.release(); h->s_ck.release();
         h->s_cv.release(); h->s_bt.release(); h->s_ws.release();
@@ -253,6 +290,7 @@ int msa_plan_create_writeback(msa_handle h, const msa_request *requests, int32_t
                               int32_t n_seg, const msa_append *jobs, int32_t n_jobs, msa_plan *out)
 {
     if (n_jobs < 0 || (n_jobs > 0 && !jobs)) return MSA_ERR_INVALID_ARG;
+    if (h && h->kv8 && n_jobs > 0) return MSA_ERR_UNSUPPORTED;   // the fused write-back stores bf16 tiles as they are: use msa_kv_append
     return plan_create(h, requests, n_req, segments, n_seg, jobs, n_jobs, out);
 }
 
@@ -417,6 +455,27 @@ int encode_2d(msa_handle h, CUtensorMap *tm, const void *base, uint64_t inner_el
     return MSA_OK;
 }
 
+// fp8 pool: bytes [rows][inner], box = head_dim bytes x box_rows, no swizzle (the converter warps read the staging slot
+// with plain 16-byte shared loads)
+int encode_2d_u8(msa_handle h, CUtensorMap *tm, const void *base, uint64_t inner_bytes, uint64_t rows, uint32_t box_inner,
+                 uint32_t box_rows)
+{
+    cuuint64_t gdim[2] = {inner_bytes, rows > 0 ? rows : 1};
+    cuuint64_t gstride[1] = {inner_bytes};
+    cuuint32_t box[2] = {box_inner, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = h->encode(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(base), gdim, gstride, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        char msg[96];
+        snprintf(msg, sizeof msg, "cuTensorMapEncodeTiled (u8) failed: CUresult %d", static_cast<int>(r));
+        g_cuda_err = msg;
+        return MSA_ERR_CUDA;
+    }
+    return MSA_OK;
+}
+
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 constexpr size_t kMapCacheEntries = 64;
@@ -448,6 +507,11 @@ int cached_tensor_maps(msa_handle h, const HostPlan &hp_in, bool writeback, cons
     const uint64_t prow = hp.uses_paged ? static_cast<uint64_t>(num_blocks) * MSA_BLOCK_SIZE : static_cast<uint64_t>(total_q);
     const uint64_t pin = hp.uses_paged ? static_cast<uint64_t>(Hkv) * D : static_cast<uint64_t>(Hq) * D;
     for (int i = 0; i < 5; ++i) {
+        if (h->kv8 && hp.uses_paged) {
+            if ((rc = encode_2d_u8(h, &fp.tm_pool_k[i], pk, pin, prow, D, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
+            if ((rc = encode_2d_u8(h, &fp.tm_pool_v[i], pv, pin, prow, D, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
+            continue;
+        }
         if ((rc = encode_2d(h, &fp.tm_pool_k[i], pk, pin, prow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
         if ((rc = encode_2d(h, &fp.tm_pool_v[i], pv, pin, prow, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
     }
@@ -486,6 +550,7 @@ int forward_impl(msa_handle h, msa_plan p, const void *q, int64_t total_q, const
     h->last_launches = 0;
     const HostPlan &hp = p->hp;
     if (writeback) {
+        if (h->kv8) return MSA_ERR_UNSUPPORTED;
         if (!hp.has_writeback) return MSA_ERR_INVALID_ARG;          // the plan must come from msa_plan_create_writeback
         if (!pool_k || !pool_v || !block_table || num_blocks < 1 || num_blocks * MSA_BLOCK_SIZE > 0x7fffffffLL) return MSA_ERR_INVALID_ARG;
         if (hp.wb_max_bt >= block_table_len) return MSA_ERR_OUT_OF_RANGE;
@@ -523,6 +588,7 @@ int forward_impl(msa_handle h, msa_plan p, const void *q, int64_t total_q, const
     fp.vb_dst = writeback ? p->d_vb_dst : nullptr;
     fp.tile_writer = writeback ? p->d_tile_writer : nullptr;
     fp.kv_to_q = h->d_kv_to_q;
+    fp.kv8_mul = h->d_kv8_mul;
     fp.o = o;
     fp.lse = lse;
     fp.workspace = static_cast<float *>(workspace);
@@ -535,7 +601,7 @@ int forward_impl(msa_handle h, msa_plan p, const void *q, int64_t total_q, const
     const bool rec = h->timing && static_cast<size_t>(h->ev_steps) * 3 + 3 <= h->ev.size();
     cudaEvent_t *ev = rec ? &h->ev[static_cast<size_t>(h->ev_steps) * 3] : nullptr;
     if (rec) MSA_CUDA(cudaEventRecord(ev[0], stream));
-    MSA_CUDA(launch_fwd(fp, D, hp.info.num_ctas, stream));
+    MSA_CUDA(launch_fwd(fp, D, h->kv8, hp.info.num_ctas, stream));
     if (rec) MSA_CUDA(cudaEventRecord(ev[1], stream));
     h->last_launches = 1;
     if (!hp.merge_items.empty()) {
@@ -714,6 +780,9 @@ int msa_kv_append(msa_handle h, msa_append_plan ap, const void *contig_k, const 
     ap_params.pool_v = pool_v;
     ap_params.row_bytes = static_cast<int64_t>(h->cfg.num_kv_heads) * h->cfg.head_dim * 2;
     ap_params.n_units = static_cast<int32_t>(ap->units.size());
+    ap_params.inv_scale = h->kv8 ? h->d_kv8_inv : nullptr;
+    ap_params.Hkv = h->cfg.num_kv_heads;
+    ap_params.D = h->cfg.head_dim;
     MSA_CUDA(launch_append(ap_params, h->num_sms, static_cast<cudaStream_t>(cuda_stream)));
     h->last_launches = 1;
     return MSA_OK;

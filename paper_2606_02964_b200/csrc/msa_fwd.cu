@@ -3,29 +3,37 @@
 
 namespace msa {
 
-int fwd_smem_bytes(int head_dim)
+template <int D, bool KV8>
+static cudaError_t configure_one()
 {
-    return head_dim == 128 ? PipeCfg<128>::kSmemBytes : PipeCfg<64>::kSmemBytes;
+    return cudaFuncSetAttribute(msa_fwd_pipe_kernel<D, KV8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                PipeCfg<D, KV8>::kSmemBytes);
+}
+
+template <int D, bool KV8>
+static void launch_one(const FwdParams &p, int num_ctas, cudaStream_t stream)
+{
+    msa_fwd_pipe_kernel<D, KV8><<<num_ctas, 512, PipeCfg<D, KV8>::kSmemBytes, stream>>>(p);
 }
 
 // The kernel needs more dynamic shared memory than the default limit; the attribute is per device and
-// per function, so the handle sets it once for its own device (msa_create).
-cudaError_t configure_fwd(int head_dim)
+// per function, so the handle sets it once for its own device (msa_create).  kv8: the fp8-pool variant.
+cudaError_t configure_fwd(int head_dim, bool kv8)
 {
-    if (head_dim == 128)
-        return cudaFuncSetAttribute(msa_fwd_pipe_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    PipeCfg<128>::kSmemBytes);
-    return cudaFuncSetAttribute(msa_fwd_pipe_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                PipeCfg<64>::kSmemBytes);
+    if (head_dim == 128) return kv8 ? configure_one<128, true>() : configure_one<128, false>();
+    return kv8 ? configure_one<64, true>() : configure_one<64, false>();
 }
 
-cudaError_t launch_fwd(const FwdParams &p, int head_dim, int num_ctas, cudaStream_t stream)
+cudaError_t launch_fwd(const FwdParams &p, int head_dim, bool kv8, int num_ctas, cudaStream_t stream)
 {
     if (num_ctas <= 0) return cudaSuccess;
-    if (head_dim == 128)
-        msa_fwd_pipe_kernel<128><<<num_ctas, 512, PipeCfg<128>::kSmemBytes, stream>>>(p);
-    else
-        msa_fwd_pipe_kernel<64><<<num_ctas, 512, PipeCfg<64>::kSmemBytes, stream>>>(p);
+    if (head_dim == 128) {
+        if (kv8) launch_one<128, true>(p, num_ctas, stream);
+        else launch_one<128, false>(p, num_ctas, stream);
+    } else {
+        if (kv8) launch_one<64, true>(p, num_ctas, stream);
+        else launch_one<64, false>(p, num_ctas, stream);
+    }
     return cudaGetLastError();
 }
 

@@ -7,7 +7,12 @@
 //   warp  12    loader of Q and K tiles: virtual blocks -> TMA boxes (paged and contiguous alike)
 //   warp  13    MMA issuer: tcgen05.mma for S = Q K^T and O += P V, accumulators in TMEM
 //   warp  14    loader of V tiles (same code path as warp 12)
-//   warp  15    idle (it only completes the 4-warp group setmaxnreg needs)
+//   warp  15    write-back warp in a write-back launch (msa_forward_writeback), else idle
+//
+// KV8 variant (fp8 E4M3 paged pool): cached blocks arrive as bytes in a staging ring (warp 15 issues
+// their TMA boxes), warps 8-11 turn them into the bf16 rows of the tile's ring slot (exact: code * 2^k) before they
+// do the unit's epilogue, and warps 12 / 14 load only the arena blocks of a tile directly; a ring slot is "full" once
+// the loader and the four converter warps have arrived.  The MMA and softmax roles are the same code in both variants.
 //
 // Two independent "chains" keep the tensor core busy while the other chain's softmax runs:
 //   kModePair   chain c owns q tile c of the unit; both chains consume every KV tile
@@ -66,17 +71,22 @@ __device__ long long g_trace[4][64][12];
 #define PROF_FLUSH(lo, hi)
 #endif
 
-template <int D>
+template <int D, bool KV8 = false>
 struct PipeCfg {
     static constexpr int kHalves = D / 64;
     static constexpr int kHalfBytes = kTileM * 128;                  // 128 rows x 128 B
     static constexpr int kTileBytes = kHalves * kHalfBytes;
-    static constexpr int kStages = 5;
+    static constexpr int kStages = KV8 ? 3 : 5;
     static constexpr int kQBytes = 2 * kTileBytes;
     static constexpr int kRingBytes = kStages * kTileBytes;
+    // KV8: staging ring for the fp8 blocks of a tile (128 rows x D bytes, row-major, no swizzle), deep enough to keep
+    // an SM's share of the HBM stream in flight; the bf16 ring behind it only decouples converters and tensor core
+    static constexpr int kStgStages = KV8 ? 4 : 0;
+    static constexpr int kStgTileBytes = kTileN * D;
+    static constexpr int kStgBytes = kStgStages * kStgTileBytes;
     static constexpr int kStatsBytes = 2 * kTileM * 2 * 4;           // [chain][row]{l, m}
-    static constexpr int kBarBytes = 256;
-    static constexpr int kSmemBytes = kQBytes + kRingBytes + kStatsBytes + kBarBytes;
+    static constexpr int kBarBytes = 512;
+    static constexpr int kSmemBytes = kQBytes + kRingBytes + kStgBytes + kStatsBytes + kBarBytes;
     static constexpr uint32_t kColS = 0, kColO = 256, kChainCols = 128;
     static constexpr float kRescaleThreshold = 8.0f;                 // log2 units (lazy rescale)
 };
@@ -93,8 +103,11 @@ enum PipeBar : int {
     kBarStFree = 22,     // [2]
     kBarPQ2 = 24,        // [2] P of keys 64-95 in TMEM
     kBarPQ3 = 26,        // [2] P of keys 96-127 in TMEM
-    kBarCount = 28
+    kBarStgFull = 28,    // [4] KV8: fp8 blocks of a K (or V) tile have landed in a staging slot
+    kBarStgEmpty = 32,   // [4] KV8: the four converter warps are done with a staging slot
+    kBarCount = 36
 };
+constexpr int kConvWarps = 4;          // KV8: warps 8-11 convert (and, per unit, do the epilogue)
 
 #ifdef MSA_NO_WRITEBACK           /* A/B builds only: the ring without its second "empty" arrival */
 constexpr bool kWritebackRing = false;
@@ -120,15 +133,74 @@ struct ResolvedVb {
     int32_t nvp;      // valid slots (0: nothing to load) | paged << 8
 };
 
+// ---------------------------------------------------------------- KV8: E4M3 codes -> bf16, exactly
+// Two codes -> two bf16 = code * 2^k.  cvt gives the exact f16; an f16 that came from an E4M3 code is a normal number (or
+// zero) with 3 mantissa bits, so shifting its exponent and mantissa into the bf16 fields leaves a bf16 whose exponent is
+// the f16's (biased by 15 instead of 127): multiplying by 2^(112 + k) in bf16 arithmetic (exact, zero stays zero) rebiases
+// it and applies the KV head's scale; the sign is put back with one LOP3.  `mul` = bf16x2 {2^(112+k), 2^(112+k)}.
+__device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t two_codes, uint32_t mul)
+{
+    uint32_t h, r;
+    asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(h) : "h"(static_cast<uint16_t>(two_codes)));
+    const uint32_t t = (h >> 3) & 0x0fff0fffu;
+    asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(t), "r"(mul));
+    return r | (h & 0x80008000u);
+}
+
+// The fp8 blocks of one K (or V) tile: staging slot (row-major, D bytes per row, block b at b*16*D) -> the bf16 tile in
+// its ring slot (128-byte swizzle, one 16 KB half per 64 elements, as TMA would have written it).  Called by the four
+// converter warps (cw = 0..3); a warp iteration covers 512 staged bytes, a lane 16 codes = two 16-byte bf16 chunks.
+// Only rows < nvalid of a block are written (the V loader has zeroed the others, K's are masked).
 template <int D>
+__device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uint32_t m_paged, int nvp, uint32_t mul, int cw,
+                                                 int lane)
+{
+    constexpr int kLanesPerRow = D / 16, kRowsPerIt = 32 / kLanesPerRow, kItPerBlock = kBlock / kRowsPerIt;
+    constexpr int kHalfBytes = kTileM * 128;
+    const int chunk = lane % kLanesPerRow, rsub = lane / kLanesPerRow;
+#pragma unroll
+    for (int it0 = 0; it0 < kVbPerTile * kItPerBlock; it0 += kConvWarps) {
+        const int it = it0 + cw;
+        const int b = it / kItPerBlock;
+        const int nv = __shfl_sync(0xffffffffu, nvp, b) & 0xff;
+        const int row = (it % kItPerBlock) * kRowsPerIt + rsub;
+        if (((m_paged >> b) & 1u) && row < nv) {
+            uint32_t w0, w1, w2, w3;
+            asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
+                         : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3)
+                         : "r"(stg + static_cast<uint32_t>((b * kBlock + row) * D + chunk * 16)));
+            const int r = b * kBlock + row;
+            const uint32_t base = dst + static_cast<uint32_t>((chunk >> 2) * kHalfBytes + r * 128);
+            const uint32_t c0 = static_cast<uint32_t>(2 * (chunk & 3)), x = static_cast<uint32_t>(r & 7);
+            const uint32_t a_lo = base + (((c0) ^ x) << 4), a_hi = base + (((c0 + 1) ^ x) << 4);
+            const uint32_t o0 = e4m3x2_to_bf16x2(w0, mul), o1 = e4m3x2_to_bf16x2(w0 >> 16, mul);
+            const uint32_t o2 = e4m3x2_to_bf16x2(w1, mul), o3 = e4m3x2_to_bf16x2(w1 >> 16, mul);
+            const uint32_t o4 = e4m3x2_to_bf16x2(w2, mul), o5 = e4m3x2_to_bf16x2(w2 >> 16, mul);
+            const uint32_t o6 = e4m3x2_to_bf16x2(w3, mul), o7 = e4m3x2_to_bf16x2(w3 >> 16, mul);
+            // lanes of the upper half (D = 128) store their two chunks in the other order: the eight lanes of a
+            // quarter-warp then hit eight different 16-byte bank groups
+            if (chunk & 4) {
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a_hi), "r"(o4), "r"(o5), "r"(o6), "r"(o7) : "memory");
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a_lo), "r"(o0), "r"(o1), "r"(o2), "r"(o3) : "memory");
+            } else {
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a_lo), "r"(o0), "r"(o1), "r"(o2), "r"(o3) : "memory");
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a_hi), "r"(o4), "r"(o5), "r"(o6), "r"(o7) : "memory");
+            }
+        }
+    }
+}
+
+template <int D, bool KV8>
 __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_constant__ FwdParams P)
 {
-    using C = PipeCfg<D>;
+    using C = PipeCfg<D, KV8>;
     extern __shared__ __align__(1024) uint8_t smem[];
     const uint32_t sbase = smem_u32(smem);
     const uint32_t sQ = sbase, sRing = sbase + C::kQBytes;
-    float2 *stats = reinterpret_cast<float2 *>(smem + C::kQBytes + C::kRingBytes);
-    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + C::kQBytes + C::kRingBytes + C::kStatsBytes);
+    const uint32_t sStg = sRing + C::kRingBytes;
+    (void)sStg;
+    float2 *stats = reinterpret_cast<float2 *>(smem + C::kQBytes + C::kRingBytes + C::kStgBytes);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + C::kQBytes + C::kRingBytes + C::kStgBytes + C::kStatsBytes);
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(bars + kBarCount);
     const uint32_t bar0 = smem_u32(bars);
     auto bar = [bar0](int i) { return bar0 + static_cast<uint32_t>(i) * 8u; };
@@ -142,8 +214,12 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
         mbar_init(bar(kBarQFull), 1);
         mbar_init(bar(kBarQEmpty), 1);
         for (int i = 0; i < C::kStages; ++i) {
-            mbar_init(bar(kBarKvFull + i), 1);
+            mbar_init(bar(kBarKvFull + i), KV8 ? 1 + kConvWarps : 1);  // the loader (+ KV8: every converter warp)
             mbar_init(bar(kBarKvEmpty + i), kWritebackRing ? 2 : 1);   // the MMA warp's commit + the loader (or the write-back warp)
+        }
+        for (int i = 0; i < C::kStgStages; ++i) {
+            mbar_init(bar(kBarStgFull + i), 1);
+            mbar_init(bar(kBarStgEmpty + i), kConvWarps);
         }
         for (int c = 0; c < 2; ++c) {
             mbar_init(bar(kBarSFull + c), 1);
@@ -344,11 +420,57 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
         const int g = row / R, t = row - g * R;
         const uint32_t trow = tmem + (static_cast<uint32_t>((warp & 3) * 32) << 16);
         uint32_t ph_o[2] = {0, 0};
+        uint32_t cv_slot = 0, cv_ph = 1, cv_st = 0, cv_stph = 0;     // KV8: ring entry / staging entry the converters are at
+        (void)cv_slot; (void)cv_ph; (void)cv_st; (void)cv_stph;
         for (int u = u_begin; u < u_end; ++u) {
             const WorkUnit wu = P.units[u];
             const int n = wu.tile_end - wu.tile_begin;
             const bool pair = wu.mode == kModePair;
             const int rows_total = wu.n_tok * G;
+            if constexpr (KV8) {
+                // ---- converters: every ring entry of the unit in order (K, V of tile 0, K, V of tile 1, ...).  An entry
+                // is waited for even when its tile holds no cached block: a waiter that skips a use of a slot cannot
+                // tell the phases of its barrier apart.
+                const int cw = warp - 8;
+                const uint32_t mul_k = __ldg(P.kv8_mul + wu.kvh), mul_v = __ldg(P.kv8_mul + P.Hkv + wu.kvh);
+                auto fetch_nvp = [&](int tile) -> int {          // lane b < 8: nvalid | paged << 8 of virtual block b
+                    int r = 0;
+                    if (lane < kVbPerTile && tile < wu.tile_end && tile * kVbPerTile + lane < wu.vb_count) {
+                        const int4 e = __ldg(reinterpret_cast<const int4 *>(P.vblocks + wu.vb_begin + tile * kVbPerTile + lane));
+                        r = e.z | ((e.z > 0 && e.w != 0) ? 256 : 0);
+                    }
+                    return r;
+                };
+                int cur = n > 0 ? fetch_nvp(wu.tile_begin) : 0;
+#pragma unroll 1
+                for (int j = 0; j < n; ++j) {
+                    const int nxt = fetch_nvp(wu.tile_begin + j + 1);
+                    const uint32_t m_paged = __ballot_sync(0xffffffffu, (cur >> 8) != 0) & 0xffu;
+#pragma unroll 1
+                    for (int which = 0; which < 2; ++which) {
+                        mbar_wait(bar(kBarKvEmpty + cv_slot), cv_ph);
+                        if (m_paged != 0) {
+                            mbar_wait(bar(kBarStgFull + cv_st), cv_stph);
+                            kv8_convert_tile<D>(sStg + cv_st * C::kStgTileBytes, sRing + cv_slot * C::kTileBytes, m_paged, cur,
+                                                which ? mul_v : mul_k, cw, lane);
+                            fence_proxy_async_smem();
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(bar(kBarStgEmpty + cv_st));
+                            if (++cv_st == C::kStgStages) {
+                                cv_st = 0;
+                                cv_stph ^= 1;
+                            }
+                        }
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(bar(kBarKvFull + cv_slot));
+                        if (++cv_slot == C::kStages) {
+                            cv_slot = 0;
+                            cv_ph ^= 1;
+                        }
+                    }
+                    cur = nxt;
+                }
+            }
             const int n_out = pair ? 2 : 1;                       // q tiles written by this unit
             for (int qt = 0; qt < n_out; ++qt) {
                 const int tok = qt * R + t;
@@ -468,6 +590,12 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             const CUtensorMap *tm_ctg = which ? P.tm_ctg_v : P.tm_ctg_k;
             const CUtensorMap *tm_ctg128 = which ? &P.tm_ctg_v128 : &P.tm_ctg_k128;
             RingPos rp{static_cast<uint32_t>(which), 1};
+            // KV8 (three ring slots): this loader also waits, in ring order, for the slots of the OTHER loader's entries.
+            // A waiter that does not see every use of a slot cannot tell its barrier's phases apart: with three slots the
+            // V loader could otherwise run from V(i) to V(i+3) -- the same slot two uses later -- while V(i) is still
+            // being multiplied, find the parity it expects and overwrite the tile.
+            RingPos ro{static_cast<uint32_t>(which ^ 1), 1};
+            (void)ro;
             uint32_t ph_qempty = 1;
             PROF_DECL();
             for (int u = u_begin; u < u_end; ++u) {
@@ -502,7 +630,8 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                 auto resolve = [&](const int4 &e) -> ResolvedVb {
                     ResolvedVb r;
                     r.nvp = e.z | (e.w << 8);
-                    r.row = (e.z > 0 && e.w) ? __ldg(P.block_table + e.x) * kBlock : e.x;
+                    if (KV8) r.row = e.x;                           // cached blocks come through the staging ring (warp 15)
+                    else r.row = (e.z > 0 && e.w) ? __ldg(P.block_table + e.x) * kBlock : e.x;
                     return r;
                 };
                 // fused KV write-back: in a write-back launch warp 15 follows the ring, stores the arena blocks of
@@ -521,11 +650,17 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     const uint32_t m_any = __ballot_sync(0xffffffffu, nv > 0) & 0xffu;
                     const uint32_t m_full = __ballot_sync(0xffffffffu, nv == kBlock) & 0xffu;
                     const uint32_t m_paged = __ballot_sync(0xffffffffu, (cur.nvp >> 8) != 0) & 0xffu;
+                    const bool direct = !KV8 || (cur.nvp >> 8) == 0;          // this lane's block is loaded here, as bf16
+                    const uint32_t m_dir = KV8 ? (m_any & ~m_paged) : m_any;
                     int rows_b[kVbPerTile];
 #pragma unroll
                     for (int b = 0; b < kVbPerTile; ++b) rows_b[b] = __shfl_sync(0xffffffffu, cur.row, b);
                     const bool run = m_full == 0xffu && m_paged == 0 &&
                                      __all_sync(0xffffffffu, lane >= kVbPerTile || cur.row == rows_b[0] + lane * kBlock);
+                    if (KV8 && which == 1) {                       // K(j) comes before V(j) in the ring
+                        mbar_wait(bar(kBarKvEmpty + ro.slot), ro.phase);
+                        ro.advance2(C::kStages);
+                    }
                     {
                         PROF_T0();
                         mbar_wait(bar(kBarKvEmpty + rp.slot), rp.phase);
@@ -557,10 +692,10 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                         }
                     } else if (m_any == m_full) {
                         if (elect_one()) {
-                            mbar_arrive_expect_tx(full, static_cast<uint32_t>(__popc(m_any) * kBlock * D * 2));
+                            mbar_arrive_expect_tx(full, static_cast<uint32_t>(__popc(m_dir) * kBlock * D * 2));
 #pragma unroll
                             for (int b = 0; b < kVbPerTile; ++b) {
-                                if (m_any >> b & 1) {
+                                if (m_dir >> b & 1) {
                                     const CUtensorMap *tm = (m_paged >> b & 1) ? tm_pool : tm_ctg;
 #pragma unroll
                                     for (int h = 0; h < C::kHalves; ++h)
@@ -569,10 +704,10 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                             }
                         }
                     } else {
-                        const uint32_t rows = __reduce_add_sync(0xffffffffu, static_cast<uint32_t>(nv));
+                        const uint32_t rows = __reduce_add_sync(0xffffffffu, static_cast<uint32_t>(direct ? nv : 0));
                         if (elect_one()) mbar_arrive_expect_tx(full, rows * D * 2);
                         __syncwarp();
-                        if (nv > 0) {     // rare path: each lane issues the boxes of its own block
+                        if (nv > 0 && direct) {     // rare path: each lane issues the boxes of its own block
                             const CUtensorMap *tm = (cur.nvp >> 8) ? tm_pool : tm_ctg;
                             int off = 0;
 #pragma unroll 1
@@ -593,6 +728,10 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     // write-back warp gives it for every tile, after its stores -- if any -- have read the slot)
                     if (kWritebackRing && !wb && elect_one()) mbar_arrive(bar(kBarKvEmpty + rp.slot));
                     rp.advance2(C::kStages);
+                    if (KV8 && which == 0) {                       // V(j) follows K(j)
+                        mbar_wait(bar(kBarKvEmpty + ro.slot), ro.phase);
+                        ro.advance2(C::kStages);
+                    }
                     cur = nxt;
                     nxt = resolve(raw);
                     raw = fetch(wu.tile_begin + j + 3);
@@ -773,6 +912,84 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             prof_acc[14] = static_cast<unsigned long long>(clock64() - prof_mma_start);
             PROF_FLUSH(8, 15);
 #endif
+        }
+        else if (KV8 && warp == 15) {
+            // ======================================================= KV8: loader of the fp8 blocks (staging ring)
+            // For every tile that holds cached blocks: their K codes into one staging slot, their V codes into the next
+            // (block b at b * 16 * D, rows of D bytes, no swizzle).  Independent of the bf16 ring, so the fp8 stream runs
+            // kStgStages tiles ahead of the converters whatever the tensor core is doing.
+            uint32_t st = 0, st_ph = 1;
+            for (int u = u_begin; u < u_end; ++u) {
+                const WorkUnit wu = P.units[u];
+                const int n = wu.tile_end - wu.tile_begin;
+                if (n <= 0) continue;
+                const int c0 = wu.kvh * D;
+                auto fetch = [&](int tile) -> int4 {
+                    int4 e = make_int4(0, 0, 0, 0);
+                    if (lane < kVbPerTile && tile < wu.tile_end && tile * kVbPerTile + lane < wu.vb_count)
+                        e = __ldg(reinterpret_cast<const int4 *>(P.vblocks + wu.vb_begin + tile * kVbPerTile + lane));
+                    return e;
+                };
+                auto resolve = [&](const int4 &e) -> ResolvedVb {     // nvp = valid slots of a CACHED block (0 otherwise)
+                    ResolvedVb r;
+                    const bool pg = e.z > 0 && e.w != 0;
+                    r.nvp = pg ? e.z : 0;
+                    r.row = pg ? __ldg(P.block_table + e.x) * kBlock : 0;
+                    return r;
+                };
+                ResolvedVb cur = resolve(fetch(wu.tile_begin));
+                ResolvedVb nxt = resolve(fetch(wu.tile_begin + 1));
+                int4 raw = fetch(wu.tile_begin + 2);
+#pragma unroll 1
+                for (int j = 0; j < n; ++j) {
+                    const int nv = cur.nvp;
+                    const uint32_t m_paged = __ballot_sync(0xffffffffu, nv > 0) & 0xffu;
+                    const uint32_t m_full = __ballot_sync(0xffffffffu, nv == kBlock) & 0xffu;
+                    if (m_paged != 0) {
+                        int rows_b[kVbPerTile];
+#pragma unroll
+                        for (int b = 0; b < kVbPerTile; ++b) rows_b[b] = __shfl_sync(0xffffffffu, cur.row, b);
+                        const uint32_t rows = __reduce_add_sync(0xffffffffu, static_cast<uint32_t>(nv));
+#pragma unroll 1
+                        for (int which = 0; which < 2; ++which) {
+                            const CUtensorMap *tm = which ? P.tm_pool_v : P.tm_pool_k;
+                            mbar_wait(bar(kBarStgEmpty + st), st_ph);
+                            const uint32_t full = bar(kBarStgFull + st);
+                            const uint32_t dst = sStg + st * C::kStgTileBytes;
+                            if (m_paged == m_full) {
+                                if (elect_one()) {
+                                    mbar_arrive_expect_tx(full, rows * D);
+#pragma unroll
+                                    for (int b = 0; b < kVbPerTile; ++b)
+                                        if (m_paged >> b & 1) tma_load_2d(dst + b * (kBlock * D), tm, full, c0, rows_b[b]);
+                                }
+                            } else {
+                                if (elect_one()) mbar_arrive_expect_tx(full, rows * D);
+                                __syncwarp();
+                                if (nv > 0) {     // a partly filled block loads only its valid rows (8/4/2/1-row boxes)
+                                    int off = 0;
+#pragma unroll 1
+                                    for (int i = 0; i < 5; ++i) {
+                                        const int rows_i = kBlock >> i;
+                                        if (nv & rows_i) {
+                                            tma_load_2d(dst + lane * (kBlock * D) + off * D, tm + i, full, c0, cur.row + off);
+                                            off += rows_i;
+                                        }
+                                    }
+                                }
+                            }
+                            __syncwarp();
+                            if (++st == C::kStgStages) {
+                                st = 0;
+                                st_ph ^= 1;
+                            }
+                        }
+                    }
+                    cur = nxt;
+                    nxt = resolve(raw);
+                    raw = fetch(wu.tile_begin + j + 3);
+                }
+            }
         }
         else if (warp == 15 && P.vb_dst != nullptr) {
             // ======================================================= write-back warp (plans from msa_plan_create_writeback)

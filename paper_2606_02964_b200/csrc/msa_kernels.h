@@ -12,6 +12,7 @@ struct FwdParams {
     CUtensorMap tm_q;        // bf16 [total_q][Hq*D], box 64 x R
     // K/V tensors: pool bf16 [num_blocks*16][Hkv*D], arena bf16 [contig_rows][Hkv*D]; boxes of
     // 64 elements x {16, 8, 4, 2, 1} rows: a partly filled block loads only its valid rows.
+    // fp8 pool: tm_pool_* are over bytes [num_blocks*16][Hkv*D] with boxes of D bytes x {16, 8, 4, 2, 1} rows, no swizzle.
     CUtensorMap tm_pool_k[5];
     CUtensorMap tm_ctg_k[5];
     CUtensorMap tm_pool_v[5];
@@ -25,6 +26,7 @@ struct FwdParams {
     const int32_t *vb_dst;           // fused KV write-back (NULL: none): per virtual block, block-table index of its destination or -1
     const int32_t *tile_writer;      // ... and per context KV tile, q_row0 of the work item that stores it (or -1)
     const int32_t *kv_to_q;          // [Hkv][G] q heads of each kv head
+    const uint32_t *kv8_mul;         // fp8 pool only: [2][Hkv] bf16x2 {2^(112+k), 2^(112+k)} for K then V, scale = 2^k (see e4m3x2_to_bf16x2)
     void *o;                         // bf16 [total_q][Hq][D]
     float *lse;                      // [total_q][Hq]
     float *workspace;
@@ -53,8 +55,10 @@ struct AppendParams {
     const int32_t *block_table;
     const void *contig_k, *contig_v;
     void *pool_k, *pool_v;
-    int64_t row_bytes;     // Hkv * D * 2
+    int64_t row_bytes;     // Hkv * D * 2 (arena row)
     int32_t n_units;
+    const float *inv_scale; // fp8 pool: [2][Hkv] 1 / scale for K then V (the rows are quantised to E4M3); NULL for a bf16 pool
+    int32_t Hkv, D;
 };
 
 cudaError_t configure_append();   // per device, like configure_fwd
@@ -63,8 +67,8 @@ cudaError_t launch_append(const AppendParams &p, int num_sms, cudaStream_t strea
 // Forward kernel: persistent, warp-specialised (msa_fwd_pipe.cuh).  configure_fwd sets the kernel's dynamic
 // shared-memory limit on the CURRENT device (once per device and head dim); launch_fwd assumes it was done.
 constexpr int kTilesPerGroup = 2;    // q tiles (of 128 packed rows) one work item covers in pair mode
-cudaError_t configure_fwd(int head_dim);
-cudaError_t launch_fwd(const FwdParams &p, int head_dim, int num_ctas, cudaStream_t stream);
+cudaError_t configure_fwd(int head_dim, bool kv8);
+cudaError_t launch_fwd(const FwdParams &p, int head_dim, bool kv8, int num_ctas, cudaStream_t stream);
 cudaError_t launch_merge(const MergeParams &p, int n_items, int max_rows, cudaStream_t stream);
 
 }  // namespace msa

@@ -1,0 +1,241 @@
+"""fp8 (E4M3) paged pool (include/msa.h MSA_POOL_FP8_E4M3; reading c20).
+
+CPU part: host validation of the scales, the quantiser oracle's pins.  GPU part (-m gpu): the CUDA path against the fp64
+oracle, which dequantises the same bytes itself -- same tolerances as the bf16 path (BASELINE.json north_star), because
+code * 2^k is exactly a bf16 -- plus bit-identity with the bf16 kernel on the dequantised pool, and the quantising
+msa_kv_append byte for byte.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import workloads as W
+from oracle.append_oracle import kv_append, quantize_e4m3
+from paper_2606_02964_b200 import (MSA_ERR_INVALID_ARG, MSA_ERR_UNSUPPORTED, MSA_POOL_FP8_E4M3, MsaError, MsaSession,
+                                   make_descriptors, msa_append_plan_create, msa_append_plan_destroy, msa_create, msa_destroy,
+                                   msa_kv_append, msa_plan_create_writeback, msa_plan_export)
+from workloads import SEG_CONTIG, SEG_PAGED, SEG_SELF, ContextSpec, RunSpec, build_problem
+
+DEV = "cuda:0"
+TOL_O_MAX, TOL_O_MEAN, TOL_LSE = 2e-2, 2e-3, 1e-3
+
+
+# ------------------------------------------------------------------ CPU: host logic and the quantiser oracle
+def test_scales_must_be_powers_of_two_within_range():
+    ok = msa_create(8, 2, 128, device=-1, pool_format=MSA_POOL_FP8_E4M3, k_scale=[0.25, 2.0 ** -14], v_scale=[2.0 ** 14, 1.0])
+    msa_destroy(ok)
+    msa_destroy(msa_create(8, 2, 128, device=-1, pool_format=MSA_POOL_FP8_E4M3))            # NULL scales: all 1.0
+    for bad in ([0.3, 1.0], [2.0 ** -15, 1.0], [2.0 ** 15, 1.0]):
+        with pytest.raises(MsaError) as e:
+            msa_create(8, 2, 128, device=-1, pool_format=MSA_POOL_FP8_E4M3, k_scale=bad)
+        assert e.value.status == MSA_ERR_UNSUPPORTED
+    for bad in ([0.0, 1.0], [-1.0, 1.0], [float("nan"), 1.0], [float("inf"), 1.0]):
+        with pytest.raises(MsaError) as e:
+            msa_create(8, 2, 128, device=-1, pool_format=MSA_POOL_FP8_E4M3, v_scale=bad)
+        assert e.value.status == MSA_ERR_INVALID_ARG
+    with pytest.raises(MsaError) as e:
+        msa_create(8, 2, 128, device=-1, pool_format=7)
+    assert e.value.status == MSA_ERR_INVALID_ARG
+
+
+def test_fused_writeback_is_refused_on_an_fp8_pool():
+    h = msa_create(4, 2, 64, device=-1, pool_format=MSA_POOL_FP8_E4M3)
+    R, n_req, S, n_seg = make_descriptors(np.array([[0, 16, 16, 0, 2]], np.int32), [SEG_PAGED, SEG_SELF], [0, 16], [16, 16],
+                                          [0, 0], [0, 0])
+    with pytest.raises(MsaError) as e:
+        msa_plan_create_writeback(h, R, n_req, S, n_seg, [(0, 16, 1)])
+    assert e.value.status == MSA_ERR_UNSUPPORTED
+    msa_destroy(h)
+
+
+def test_quantiser_oracle_against_torch_and_closed_forms():
+    rng = np.random.default_rng(11)
+    x = np.concatenate([rng.standard_normal(4000) * 3, rng.uniform(-448, 448, 2000), rng.standard_normal(500) * 1e-3,
+                        [0.0, -0.0, 448.0, -448.0, 2.0 ** -9, 2.0 ** -10, 3 * 2.0 ** -10]])
+    x = torch.from_numpy(x).to(torch.bfloat16).double().numpy()              # what the arena can hold
+    for scale in (1.0, 2.0 ** -6, 4.0):
+        mine = quantize_e4m3(x * scale, scale, oracle.e4m3_to_double)
+        ref = torch.from_numpy(x).float().to(torch.float8_e4m3fn).view(torch.uint8).numpy()   # library routine, |x| <= 448
+        assert np.array_equal(mine, ref)
+    # saturation and NaN (torch's conversion does not saturate, so these are closed forms)
+    q = lambda v: int(quantize_e4m3(np.array([v]), 1.0, oracle.e4m3_to_double)[0])
+    assert q(449.0) == 0x7e and q(1e30) == 0x7e and q(-1e30) == 0xfe and q(float("inf")) == 0x7e and q(float("nan")) == 0x7f
+    # ties go to the even code: halfway between 1.0 (0x38) and 1.125 (0x39) -> 0x38; between 1.125 and 1.25 (0x3a) -> 0x3a
+    assert q(1.0625) == 0x38 and q(1.1875) == 0x3a and q(2.0 ** -10) == 0x00 and q(3 * 2.0 ** -10) == 0x02
+    # decode(quantise(v)) is the nearest representable value
+    v = rng.uniform(-400, 400, 300)
+    codes = quantize_e4m3(v, 1.0, oracle.e4m3_to_double)
+    back = np.array([oracle.e4m3_to_double(int(c)) for c in codes])
+    grid = np.array([oracle.e4m3_to_double(c) for c in range(256) if c not in (0x7f, 0xff)])
+    assert np.allclose(np.abs(back - v), np.abs(grid[None, :] - v[:, None]).min(axis=1), atol=0)
+
+
+# ------------------------------------------------------------------ GPU parity
+def gpu_forward(p):
+    with MsaSession(p) as s:
+        o, lse = s.forward()
+        torch.cuda.synchronize()
+        return o.float().cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64), s.info
+
+
+def compare(p, o, lse, row_req=None, row_idx=None, strict=True):
+    O, LSE = oracle.forward_problem(p, row_req, row_idx)
+    if row_req is not None:
+        g = p.req[row_req, 0] + row_idx
+        o, lse = o[g], lse[g]
+    fin = np.isfinite(LSE)
+    assert np.array_equal(np.isneginf(lse), ~fin), "rows without a visible key must give LSE=-inf"
+    assert np.all(np.isfinite(o)), "non-finite O"
+    assert np.all(o[~fin] == 0.0)
+    d_o = np.abs(o - O)
+    d_l = np.abs(lse[fin] - LSE[fin]) if fin.any() else np.zeros(1)
+    if strict:
+        assert d_o.max() <= TOL_O_MAX, f"max|dO|={d_o.max()}"
+    else:
+        assert np.all(d_o <= TOL_O_MAX * np.maximum(1.0, np.abs(O) / 2.0)), f"max|dO|={d_o.max()}"
+    assert d_o.mean() <= TOL_O_MEAN, f"mean|dO|={d_o.mean()}"
+    assert d_l.max() <= TOL_LSE, f"max|dLSE|={d_l.max()}"
+    return d_o.max(), d_o.mean(), d_l.max()
+
+
+def _dequantised_twin(p8):
+    """bf16 problem whose pool holds code * scale (exact in bf16 for power-of-two scales)."""
+    import copy
+    p = copy.copy(p8)
+    for name, sc in (("pool_k", p8.k_scale), ("pool_v", p8.v_scale)):
+        codes = getattr(p8, name)
+        s = torch.from_numpy(np.asarray(sc, np.float32)).to(codes.device)[None, None, :, None]
+        setattr(p, name, (codes.view(torch.float8_e4m3fn).float() * s).to(torch.bfloat16))
+    p.k_scale = p.v_scale = None
+    return p
+
+
+CASES = [
+    dict(seed=101, Hq=4, Hkv=2, D=64, max_ctx=700, max_q=96),
+    dict(seed=102, Hq=8, Hkv=2, D=128, max_ctx=900, max_q=70),
+    dict(seed=103, Hq=4, Hkv=4, D=128, max_ctx=600, max_q=140, n_req=4),          # G=1
+    dict(seed=104, Hq=16, Hkv=2, D=64, max_ctx=500, max_q=40),                    # G=8
+    dict(seed=106, Hq=6, Hkv=2, D=128, max_ctx=500, max_q=90),                    # G=3 (R=40)
+    dict(seed=108, Hq=8, Hkv=2, D=128, max_ctx=600, max_q=100, hybrid=True, gaps=True),
+    dict(seed=109, Hq=4, Hkv=2, D=128, max_ctx=300, max_q=8, n_req=12, max_segs=8),   # short queries
+    dict(seed=110, Hq=4, Hkv=2, D=64, max_ctx=40, max_q=3, n_req=10, max_segs=4),     # tiny everything
+    dict(seed=111, Hq=4, Hkv=2, D=128, max_ctx=500, max_q=64, q_to_kv=[1, 0, 0, 1]),   # custom GQA map
+    dict(seed=112, Hq=8, Hkv=2, D=128, max_ctx=800, max_q=200, ragged=False),
+]
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("kw", CASES, ids=lambda k: f"seed{k['seed']}")
+def test_kv8_random_small_problems_against_the_oracle_and_the_bf16_kernel(kw):
+    p = W.random_problem(device=DEV, keep_dense=False, **kw)
+    exps = [(-6, -4), (-5, -7), (-7, -5), (-4, -6)]
+    p8 = W.to_fp8_pool(p, k_exp=[exps[h % 4][0] for h in range(p.Hkv)], v_exp=[exps[h % 4][1] for h in range(p.Hkv)])
+    o, lse, _ = gpu_forward(p8)
+    compare(p8, o, lse, strict=False)
+    # code * 2^k is exactly a bf16 and the conversion happens before the same MMAs: bit-identical to the bf16 kernel
+    o2, lse2, _ = gpu_forward(_dequantised_twin(p8))
+    assert np.array_equal(o, o2) and np.array_equal(lse, lse2)
+
+
+@pytest.mark.gpu
+def test_kv8_cfg1_tiny_and_default_scales():
+    p8 = W.to_fp8_pool(W.cfg1_tiny(device=DEV, keep_dense=False))
+    o, lse, info = gpu_forward(p8)
+    compare(p8, o, lse)
+    assert info["visible_pairs"] == 14368
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("seed", [201, 202])
+def test_kv8_nan_codes_in_the_slack_never_reach_the_output(seed):
+    """Block tails and unused blocks hold the NaN code 0x7f, arena gaps bf16 NaN."""
+    p = W.random_problem(seed, Hq=8, Hkv=2, D=128, max_ctx=600, max_q=70, fill="nan", arena_gap=3, device=DEV)
+    p8 = W.to_fp8_pool(p, k_exp=[-6, -5], v_exp=[-5, -6])
+    assert (p8.pool_k == 0x7f).any()
+    o, lse, _ = gpu_forward(p8)
+    compare(p8, o, lse, strict=False)
+
+
+@pytest.mark.gpu
+def test_kv8_split_kv_and_one_token_segments():
+    ctx = ContextSpec([(SEG_PAGED, 0, 3000), (SEG_CONTIG, 3000, 1777), (SEG_PAGED, 4777, 1500), (SEG_SELF, 6277, 40)])
+    p = build_problem("split", 8, 2, 128, [ctx], [RunSpec(0, 6277, 40)], seed=8, device=DEV)
+    p8 = W.to_fp8_pool(p)
+    with MsaSession(p8) as s:
+        assert s.info["num_split_items"] > 0
+    o, lse, _ = gpu_forward(p8)
+    compare(p8, o, lse)
+    c0 = ContextSpec([(SEG_PAGED, 3, 1), (SEG_CONTIG, 4, 1), (SEG_PAGED, 9, 1)])
+    c1 = ContextSpec([(SEG_PAGED, 0, 131), (SEG_CONTIG, 131, 1), (SEG_SELF, 132, 1)])
+    p = build_problem("edge", 4, 2, 128, [c0, c1], [RunSpec(0, 0, 5), RunSpec(1, 132, 1)], seed=7, device=DEV, keep_dense=True,
+                      fill="nan")
+    p8 = W.to_fp8_pool(p, k_exp=[-6, -6], v_exp=[-6, -6])
+    o, lse, _ = gpu_forward(p8)
+    compare(p8, o, lse, strict=False)
+    assert np.all(np.isneginf(lse[:3]))
+
+
+@pytest.mark.gpu
+def test_kv8_cfg5_short_query_every_row():
+    """BASELINE.json configs[4] with the cached blocks in fp8 (the launch bench.py --workload cfg5_kv8 times)."""
+    p8 = W.to_fp8_pool(W.cfg5_short_query(device=DEV))
+    o, lse, info = gpu_forward(p8)
+    mx, mean, dl = compare(p8, o, lse)
+    print(f"cfg5_kv8: {p8.total_q} rows x {p8.Hq} heads compared, max|dO|={mx:.3e} mean|dO|={mean:.3e} max|dLSE|={dl:.3e}")
+
+
+@pytest.mark.gpu
+def test_kv8_cfg2_prefill_sampled_rows():
+    p8 = W.to_fp8_pool(W.cfg2_llama8b(device=DEV))
+    o, lse, info = gpu_forward(p8)
+    rr, ii = W.pick_rows(p8, n_random=24, seed=3)
+    mx, mean, dl = compare(p8, o, lse, rr, ii)
+    print(f"cfg2_kv8: {len(rr)} rows x {p8.Hq} heads compared, max|dO|={mx:.3e} mean|dO|={mean:.3e} max|dLSE|={dl:.3e}")
+
+
+@pytest.mark.gpu
+def test_kv8_append_quantises_like_the_oracle_and_feeds_the_forward():
+    """msa_kv_append on an fp8 handle: every destination byte equals the oracle quantiser's code (untouched blocks and block
+    tails keep their canary), and a forward that reads the written blocks as PAGED segments matches the fp64 oracle."""
+    p = W.random_problem(305, n_req=3, Hq=8, Hkv=2, D=128, max_ctx=400, max_q=50, hybrid=True, device=DEV, keep_dense=False)
+    p8 = W.to_fp8_pool(p, k_exp=[-6, -5], v_exp=[-5, -7])
+    # a few extreme arena values: saturation, ties, tiny
+    p8.contig_k = p8.contig_k.clone()
+    p8.contig_k.view(-1)[:6] = torch.tensor([1000.0, -1000.0, 1.0625 * 2 ** -6, 2.0 ** -17, 0.0, -0.0], dtype=torch.bfloat16)
+    bt = p8.block_table_np
+    n_pool = int(p8.pool_k.shape[0])
+    jobs, kind2, boff2, cursor = [], p8.seg_kind.copy(), p8.seg_block_off.copy(), len(bt)
+    for s in range(len(p8.seg_kind)):
+        if int(p8.seg_kind[s]) != SEG_PAGED:
+            n = int(p8.seg_len[s])
+            jobs.append((int(p8.seg_row_off[s]), n, cursor))
+            kind2[s], boff2[s] = SEG_PAGED, cursor
+            cursor += (n + 15) // 16
+    extra = cursor - len(bt)
+    bt2 = np.concatenate([bt, (n_pool + np.random.default_rng(5).permutation(extra)).astype(np.int32)])
+    canary = 0x5a
+    pool_k = torch.cat([p8.pool_k, torch.full((extra,) + tuple(p8.pool_k.shape[1:]), canary, dtype=torch.uint8, device=DEV)])
+    pool_v = torch.cat([p8.pool_v, torch.full((extra,) + tuple(p8.pool_v.shape[1:]), canary, dtype=torch.uint8, device=DEV)])
+    bt2_d = torch.from_numpy(bt2).to(DEV)
+    h = msa_create(p8.Hq, p8.Hkv, p8.D, device=0, pool_format=MSA_POOL_FP8_E4M3, k_scale=p8.k_scale, v_scale=p8.v_scale)
+    ap = msa_append_plan_create(h, jobs)
+    msa_kv_append(h, ap, p8.contig_k, p8.contig_v, pool_k, pool_v, bt2_d, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    msa_append_plan_destroy(ap)
+    msa_destroy(h)
+    # expected bytes: the oracle's quantiser per KV head, placed by the oracle's write-back
+    for pool, arena, scales in ((pool_k, p8.contig_k, p8.k_scale), (pool_v, p8.contig_v, p8.v_scale)):
+        a = arena.float().cpu().double().numpy()
+        codes = np.stack([quantize_e4m3(a[:, hh, :], float(scales[hh]), oracle.e4m3_to_double) for hh in range(p8.Hkv)], axis=1)
+        start = np.concatenate([p8_pool.cpu().numpy() for p8_pool in (p8.pool_k if pool is pool_k else p8.pool_v,)] +
+                               [np.full((extra,) + tuple(pool.shape[1:]), canary, np.uint8)])
+        want = kv_append(start, codes, bt2, jobs)
+        assert np.array_equal(pool.cpu().numpy(), want)
+    # the forward reads what was written
+    import copy
+    p2 = copy.copy(p8)
+    p2.pool_k, p2.pool_v, p2.block_table, p2.block_table_np = pool_k, pool_v, bt2_d, bt2
+    p2.seg_kind, p2.seg_block_off, p2.num_blocks = kind2, boff2, n_pool + extra
+    o, lse, _ = gpu_forward(p2)
+    compare(p2, o, lse, strict=False)
