@@ -164,11 +164,15 @@ def all_workloads():
     """BASELINE.json's configs, the extra rows of SURVEY.md 8(f), and the batch whose residency the evictor decides."""
     import workloads as W
     from workloads.policy_trace import f3_policy_trace
-    return {**W.CONFIGS, **W.EXTRA_CONFIGS, "f3_policy_trace": f3_policy_trace}
+    out = {**W.CONFIGS, **W.EXTRA_CONFIGS, "f3_policy_trace": f3_policy_trace}
+    # the same batches with the paged pool stored as fp8 E4M3 codes (SURVEY.md 8 f4): `<name>_kv8`
+    for base in ("cfg2_llama8b", "cfg3_70b_long", "cfg4_mixed", "cfg5_short_query", "f1_hybrid_pod"):
+        out[base + "_kv8"] = (lambda b: (lambda device="cpu", **kw: W.to_fp8_pool(out[b](device=device, **kw))))(base)
+    return out
 
 
 def metric_of(workload: str):
-    if workload == "cfg5_short_query":
+    if workload in ("cfg5_short_query", "cfg5_short_query_kv8"):
         return "msa_short_query_hbm_gbs", "GB/s", "hbm"
     return "msa_attention_tflops", "TFLOP/s", "tensor"
 
@@ -267,6 +271,7 @@ def run_mine(args, rank: int, world: int, local_rank: int):
                 vs_baseline=None, dtype="bf16", data="synthetic",
                 config=dict(workload=args.workload, Hq=p.Hq, Hkv=p.Hkv, head_dim=p.D, requests=p.n_req,
                             total_q=p.total_q, kv_tokens=p.kv_tokens(), block_size=16,
+                            pool_format="fp8_e4m3 (power-of-two scale per KV head)" if p.k_scale is not None else "bf16",
                             l2_policy="inputs larger than L2 (%.0f MB per step), no flush" % (res["algorithmic"]["bytes"] / 1e6),
                             parallelism=f"replicas x{world}" if world > 1 else "single GPU"),
                 clocks=res["clocks"], e2e=res.get("e2e"), gpu_launches=res["gpu_launches"],
@@ -650,7 +655,10 @@ def run_reference(args, rank: int, world: int):
                      f1_hybrid_pod=dict(n_prefill=1, n_decode=2))
         if args.workload == "f3_policy_trace":
             raise SystemExit("the oracle arm covers BASELINE.json's configs and f1 (f3's residency is decided by the product's evictor)")
-        p = {**W.CONFIGS, **W.EXTRA_CONFIGS}[args.workload](device="cpu", **small.get(args.workload, {}))
+        base = args.workload[:-4] if args.workload.endswith("_kv8") else args.workload
+        p = {**W.CONFIGS, **W.EXTRA_CONFIGS}[base](device="cpu", **small.get(base, {}))
+        if base != args.workload:
+            p = W.to_fp8_pool(p)
     reqs = list(range(min(2, p.n_req)))
     dt, fl, pairs, n = oracle_sample(p, 8, 1, reqs)
     total = max(1, args.steps + args.warmup)
@@ -683,6 +691,7 @@ def main():
     ap.add_argument("--impl", default="mine", choices=["mine", "reference"])
     ap.add_argument("--workload", default="cfg2_llama8b",
                     choices=["cfg2_llama8b", "cfg3_70b_long", "cfg4_mixed", "cfg5_short_query", "f1_hybrid_pod", "f3_policy_trace",
+                             "cfg2_llama8b_kv8", "cfg3_70b_long_kv8", "cfg4_mixed_kv8", "cfg5_short_query_kv8", "f1_hybrid_pod_kv8",
                              "fig13", "evictor", "costmodel", "kv_append"])
     ap.add_argument("--no-secondary", action="store_true")
     args = ap.parse_args()

@@ -44,7 +44,7 @@ enum {
     MSA_ERR_INVALID_ARG = -1,      /* NULL pointer, negative size, non-positive / non-finite scale */
     MSA_ERR_UNSUPPORTED = -2,      /* head_dim not in {64,128}, block_size != 16, Hq % Hkv != 0, G > 16,
                                       head map that does not give every KV head exactly G q heads, an fp8 pool
-                                      scale that is not a power of two in [2^-14, 2^14], KV write-back into an
+                                      scale that is not a power of two in [2^-14, 2^7], KV write-back into an
                                       fp8 pool through the forward launch */
     MSA_ERR_OVERLAP = -3,          /* segments of one request overlap in absolute position, or two
                                       requests write the same q rows */
@@ -68,7 +68,7 @@ enum { MSA_SEG_PAGED = 0, MSA_SEG_CONTIG = 1, MSA_SEG_SELF = 2 };
  *   MSA_POOL_FP8_E4M3  one byte per element, OCP FP8 E4M3 (1 sign, 4 exponent bits with bias 7, 3 mantissa bits, no
  *                      infinity, S.1111.111 = NaN), and one scale per KV head for K and one for V:
  *                          K_j[kvh][d] = e4m3(pool_k byte) * k_scale[kvh],   V_j[kvh][d] = e4m3(pool_v byte) * v_scale[kvh]
- *                      The scales must be powers of two in [2^-14, 2^14] (as in the OCP MX formats): the dequantised
+ *                      The scales must be powers of two in [2^-14, 2^7] (as in the OCP MX formats): the dequantised
  *                      value is then exactly a bf16, the kernel converts the codes on chip and the result is the bf16
  *                      path's result on the dequantised pool -- same tolerances.  A NaN code dequantises to an
  *                      unspecified finite value (non-finite K/V are outside the definition, DESIGN.md c19). */

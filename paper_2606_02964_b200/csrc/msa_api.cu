@@ -84,9 +84,10 @@ struct msa_handle_s {
     bool planning_only = false;
     std::vector<int32_t> kv_to_q;      // [Hkv][G]
     int32_t *d_kv_to_q = nullptr;
+    bool token_major = false;          // q heads of every KV head are consecutive: q tiles are packed token-major (FwdParams::token_major)
     bool kv8 = false;                  // fp8 (E4M3) paged pool
     std::vector<float> kv_scale;       // kv8: [2][Hkv] K scales then V scales (powers of two)
-    uint32_t *d_kv8_mul = nullptr;     // kv8: [2][Hkv] bf16x2 {2^(112+k), 2^(112+k)} (forward kernel)
+    uint32_t *d_kv8_mul = nullptr;     // kv8: [2][Hkv] f16 bits of 2^k (forward kernel)
     float *d_kv8_inv = nullptr;        // kv8: [2][Hkv] 1 / scale (quantising msa_kv_append)
     EncodeTiledFn encode = nullptr;
     // Tensor maps depend only on (base pointer, extent) of q / pool / arena: a model calls msa_forward once per
@@ -179,10 +180,10 @@ int msa_create(const msa_config *cfg, msa_handle *out)
                 const float sc = src ? src[kv] : 1.f;
                 int e = 0;
                 if (!(sc > 0.f) || !isfinite(sc)) return MSA_ERR_INVALID_ARG;
-                if (frexpf(sc, &e) != 0.5f || e - 1 < -14 || e - 1 > 14) return MSA_ERR_UNSUPPORTED;
-                const uint32_t b = static_cast<uint32_t>(127 + 112 + (e - 1)) << 7;      // bf16 bits of 2^(112 + k)
+                if (frexpf(sc, &e) != 0.5f || e - 1 < -14 || e - 1 > 7) return MSA_ERR_UNSUPPORTED;
+                const uint32_t b = static_cast<uint32_t>(15 + (e - 1)) << 10;            // f16 bits of 2^k (normal for k >= -14)
                 kv_scale.push_back(sc);
-                kv8_mul.push_back(b | (b << 16));
+                kv8_mul.push_back(b);
                 kv8_inv.push_back(1.f / sc);
             }
     }
@@ -207,6 +208,10 @@ int msa_create(const msa_config *cfg, msa_handle *out)
         }
         h->kv_to_q[static_cast<size_t>(kv) * G + fill[kv]++] = q;
     }
+    h->token_major = true;
+    for (int kv = 0; kv < cfg->num_kv_heads; ++kv)
+        for (int g = 1; g < G; ++g)
+            if (h->kv_to_q[static_cast<size_t>(kv) * G + g] != h->kv_to_q[static_cast<size_t>(kv) * G] + g) h->token_major = false;
     if (cfg->device < 0) {
         // planning-only handle: descriptor validation and scheduling on the host; every
         // call that would touch the GPU reports MSA_ERR_NO_DEVICE.
@@ -502,6 +507,21 @@ int cached_tensor_maps(msa_handle h, const HostPlan &hp_in, bool writeback, cons
     memset(&fp, 0, sizeof fp);
     int rc = encode_2d(h, &fp.tm_q, q, static_cast<uint64_t>(Hq) * D, static_cast<uint64_t>(total_q), h->R);
     if (rc != MSA_OK) return rc;
+    {   // q as [total_q][Hq][D]: box = 64 elements x G heads x R tokens, rows land token-major
+        cuuint64_t gdim[3] = {static_cast<cuuint64_t>(D), static_cast<cuuint64_t>(Hq), static_cast<cuuint64_t>(total_q > 0 ? total_q : 1)};
+        cuuint64_t gstride[2] = {static_cast<cuuint64_t>(D) * 2, static_cast<cuuint64_t>(Hq) * D * 2};
+        cuuint32_t box[3] = {64, static_cast<cuuint32_t>(h->G), static_cast<cuuint32_t>(h->R)};
+        cuuint32_t estr[3] = {1, 1, 1};
+        CUresult r = h->encode(&fp.tm_q3, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void *>(q), gdim, gstride, box, estr,
+                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) {
+            char msg[96];
+            snprintf(msg, sizeof msg, "cuTensorMapEncodeTiled (q, 3-D) failed: CUresult %d", static_cast<int>(r));
+            g_cuda_err = msg;
+            return MSA_ERR_CUDA;
+        }
+    }
     const void *pk = hp.uses_paged ? pool_k : q;
     const void *pv = hp.uses_paged ? pool_v : q;
     const uint64_t prow = hp.uses_paged ? static_cast<uint64_t>(num_blocks) * MSA_BLOCK_SIZE : static_cast<uint64_t>(total_q);
@@ -597,11 +617,14 @@ int forward_impl(msa_handle h, msa_plan p, const void *q, int64_t total_q, const
     fp.Hkv = Hkv;
     fp.G = h->G;
     fp.R = h->R;
+    fp.token_major = h->token_major ? 1 : 0;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     const bool rec = h->timing && static_cast<size_t>(h->ev_steps) * 3 + 3 <= h->ev.size();
     cudaEvent_t *ev = rec ? &h->ev[static_cast<size_t>(h->ev_steps) * 3] : nullptr;
     if (rec) MSA_CUDA(cudaEventRecord(ev[0], stream));
-    MSA_CUDA(launch_fwd(fp, D, h->kv8, hp.info.num_ctas, stream));
+    bool any_pair = false;
+    for (const WorkUnit &wu : hp.units) any_pair = any_pair || (wu.mode == kModePair && wu.tile_end > wu.tile_begin);
+    MSA_CUDA(launch_fwd(fp, D, h->kv8, !any_pair, hp.info.num_ctas, stream));
     if (rec) MSA_CUDA(cudaEventRecord(ev[1], stream));
     h->last_launches = 1;
     if (!hp.merge_items.empty()) {

@@ -3,36 +3,42 @@
 
 namespace msa {
 
-template <int D, bool KV8>
+template <int D, bool KV8, int QT>
 static cudaError_t configure_one()
 {
-    return cudaFuncSetAttribute(msa_fwd_pipe_kernel<D, KV8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                PipeCfg<D, KV8>::kSmemBytes);
+    return cudaFuncSetAttribute(msa_fwd_pipe_kernel<D, KV8, QT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                PipeCfg<D, KV8, QT>::kSmemBytes);
 }
 
-template <int D, bool KV8>
+template <int D, bool KV8, int QT>
 static void launch_one(const FwdParams &p, int num_ctas, cudaStream_t stream)
 {
-    msa_fwd_pipe_kernel<D, KV8><<<num_ctas, 512, PipeCfg<D, KV8>::kSmemBytes, stream>>>(p);
+    msa_fwd_pipe_kernel<D, KV8, QT><<<num_ctas, 512, PipeCfg<D, KV8, QT>::kSmemBytes, stream>>>(p);
 }
 
 // The kernel needs more dynamic shared memory than the default limit; the attribute is per device and
-// per function, so the handle sets it once for its own device (msa_create).  kv8: the fp8-pool variant.
+// per function, so the handle sets it once for its own device (msa_create).  kv8: the fp8-pool variants
+// (two shared-memory layouts: with room for the two Q tiles of pair-mode units, or -- short queries only --
+// for one Q tile and a deeper staging ring).
 cudaError_t configure_fwd(int head_dim, bool kv8)
 {
-    if (head_dim == 128) return kv8 ? configure_one<128, true>() : configure_one<128, false>();
-    return kv8 ? configure_one<64, true>() : configure_one<64, false>();
+    if (!kv8) return head_dim == 128 ? configure_one<128, false, 2>() : configure_one<64, false, 2>();
+    cudaError_t e = head_dim == 128 ? configure_one<128, true, 2>() : configure_one<64, true, 2>();
+    if (e != cudaSuccess) return e;
+    return head_dim == 128 ? configure_one<128, true, 1>() : configure_one<64, true, 1>();
 }
 
-cudaError_t launch_fwd(const FwdParams &p, int head_dim, bool kv8, int num_ctas, cudaStream_t stream)
+cudaError_t launch_fwd(const FwdParams &p, int head_dim, bool kv8, bool one_q_tile, int num_ctas, cudaStream_t stream)
 {
     if (num_ctas <= 0) return cudaSuccess;
     if (head_dim == 128) {
-        if (kv8) launch_one<128, true>(p, num_ctas, stream);
-        else launch_one<128, false>(p, num_ctas, stream);
+        if (!kv8) launch_one<128, false, 2>(p, num_ctas, stream);
+        else if (one_q_tile) launch_one<128, true, 1>(p, num_ctas, stream);
+        else launch_one<128, true, 2>(p, num_ctas, stream);
     } else {
-        if (kv8) launch_one<64, true>(p, num_ctas, stream);
-        else launch_one<64, false>(p, num_ctas, stream);
+        if (!kv8) launch_one<64, false, 2>(p, num_ctas, stream);
+        else if (one_q_tile) launch_one<64, true, 1>(p, num_ctas, stream);
+        else launch_one<64, true, 2>(p, num_ctas, stream);
     }
     return cudaGetLastError();
 }

@@ -71,17 +71,20 @@ __device__ long long g_trace[4][64][12];
 #define PROF_FLUSH(lo, hi)
 #endif
 
-template <int D, bool KV8 = false>
+template <int D, bool KV8 = false, int QT = 2>
 struct PipeCfg {
     static constexpr int kHalves = D / 64;
     static constexpr int kHalfBytes = kTileM * 128;                  // 128 rows x 128 B
     static constexpr int kTileBytes = kHalves * kHalfBytes;
-    static constexpr int kStages = KV8 ? 3 : 5;
-    static constexpr int kQBytes = 2 * kTileBytes;
+    static constexpr int kStages = KV8 ? 4 : 5;
+    static constexpr int kQBytes = QT * kTileBytes;                  // QT = 1: a launch without pair-mode units (short queries only)
     static constexpr int kRingBytes = kStages * kTileBytes;
-    // KV8: staging ring for the fp8 blocks of a tile (128 rows x D bytes, row-major, no swizzle), deep enough to keep
-    // an SM's share of the HBM stream in flight; the bf16 ring behind it only decouples converters and tensor core
-    static constexpr int kStgStages = KV8 ? 4 : 0;
+    // KV8: staging ring for the fp8 blocks of a tile (128 rows x D bytes, row-major, no swizzle).  It holds the fp8
+    // bytes that are in flight from HBM; the bf16 ring behind it only decouples converters and tensor core.  A
+    // short-query launch needs one Q tile and spends the other's room on two more staging slots (an SM's share of the
+    // HBM stream in flight); a launch with prefill units reuses every K/V tile 256 rows long and needs little in flight.
+    static constexpr int kStgStages = KV8 ? (QT == 1 ? 4 : 2) : 0;
+    static constexpr int kStgDiv = kStgStages ? kStgStages : 1;      // (keeps the dead staging code of the bf16 variant well formed)
     static constexpr int kStgTileBytes = kTileN * D;
     static constexpr int kStgBytes = kStgStages * kStgTileBytes;
     static constexpr int kStatsBytes = 2 * kTileM * 2 * 4;           // [chain][row]{l, m}
@@ -128,72 +131,186 @@ struct RingPos {
     }
 };
 
+// KV8: the ring holds the tiles of a unit in the order the MMA warp takes them, so that an entry's slot is free again
+// a fixed number of entries later whatever the mode:
+//   pair mode   K0 V0 K1 V1 ...                          (K(j+1) is taken while V(j) is being multiplied)
+//   split mode  K0 K1 V0 K2 V1 ... K(n-1) V(n-2) V(n-1)  (QK of tile j+2 follows PV of tile j)
+// Index of K(i) / V(j) in that order, and its inverse.
+__device__ __forceinline__ int kv8_entry_of_k(int i, bool pair)
+{
+    return pair ? 2 * i : (i < 2 ? i : 2 * i - 1);
+}
+__device__ __forceinline__ int kv8_entry_of_v(int j, int n, bool pair)
+{
+    return pair ? 2 * j + 1 : (j == n - 1 ? 2 * n - 1 : 2 * j + 2);
+}
+__device__ __forceinline__ void kv8_entry(int e, int n, bool pair, bool &is_v, int &tile)
+{
+    if (pair) {
+        is_v = (e & 1) != 0;
+        tile = e >> 1;
+    } else if (e == 0) {
+        is_v = false;
+        tile = 0;
+    } else if (e == 2 * n - 1) {
+        is_v = true;
+        tile = n - 1;
+    } else if (e & 1) {
+        is_v = false;
+        tile = (e + 1) >> 1;
+    } else {
+        is_v = true;
+        tile = (e - 2) >> 1;
+    }
+}
+
 struct ResolvedVb {
     int32_t row;      // first row in the pool / arena row space
     int32_t nvp;      // valid slots (0: nothing to load) | paged << 8
 };
 
 // ---------------------------------------------------------------- KV8: E4M3 codes -> bf16, exactly
-// Two codes -> two bf16 = code * 2^k.  cvt gives the exact f16; an f16 that came from an E4M3 code is a normal number (or
-// zero) with 3 mantissa bits, so shifting its exponent and mantissa into the bf16 fields leaves a bf16 whose exponent is
-// the f16's (biased by 15 instead of 127): multiplying by 2^(112 + k) in bf16 arithmetic (exact, zero stays zero) rebiases
-// it and applies the KV head's scale; the sign is put back with one LOP3.  `mul` = bf16x2 {2^(112+k), 2^(112+k)}.
+// Two codes -> two bf16 = code * 2^k.  cvt gives the exact f16 pair (one ALU-pipe instruction); each half is widened
+// to f32 and multiplied by the KV head's scale in one mixed-precision FMA (fma.rn.f32.f16: f16 inputs, f32 result,
+// exact -- the product has four significant bits); the bf16 pair is the two high halves of those f32 (PRMT: nothing
+// is rounded).  Two ALU-pipe and two FMA-pipe instructions per pair; shifting the f16 fields into place and rebiasing
+// with a bf16 multiply instead costs four ALU-pipe instructions and measured 1.5x slower (profiles/r02_microbench.md).
+// `mul` = f16 bits of 2^k in the low half.
 __device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t two_codes, uint32_t mul)
 {
     uint32_t h, r;
+    float lo, hi;
     asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(h) : "h"(static_cast<uint16_t>(two_codes)));
-    const uint32_t t = (h >> 3) & 0x0fff0fffu;
-    asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(t), "r"(mul));
-    return r | (h & 0x80008000u);
+    asm("{\n\t.reg .b16 a, b;\n\tmov.b32 {a, b}, %2;\n\tfma.rn.f32.f16 %0, a, %3, 0f00000000;\n\tfma.rn.f32.f16 %1, b, %3, 0f00000000;\n\t}"
+        : "=f"(lo), "=f"(hi) : "r"(h), "h"(static_cast<uint16_t>(mul)));
+    asm("prmt.b32 %0, %1, %2, 0x7632;" : "=r"(r) : "r"(__float_as_uint(lo)), "r"(__float_as_uint(hi)));
+    return r;
 }
 
 // The fp8 blocks of one K (or V) tile: staging slot (row-major, D bytes per row, block b at b*16*D) -> the bf16 tile in
-// its ring slot (128-byte swizzle, one 16 KB half per 64 elements, as TMA would have written it).  Called by the four
-// converter warps (cw = 0..3); a warp iteration covers 512 staged bytes, a lane 16 codes = two 16-byte bf16 chunks.
-// Only rows < nvalid of a block are written (the V loader has zeroed the others, K's are masked).
+// its ring slot (128-byte swizzle, one 16 KB half per 64 elements, as TMA would have written it).  A warp iteration
+// covers 512 staged bytes (a lane: 16 codes = two 16-byte bf16 chunks); the calling warp takes iterations first,
+// first + stride, ...  Only rows < nvalid of a block are written (the V loader has zeroed the others, K's are masked).
+// The two stores of the lanes j and j + 4 of a row go to the same bank group (different 64-element halves): a two-way
+// conflict on the store pipe, which has room; ordering the stores per lane to avoid it costs ten selects per iteration
+// on the ALU pipe, which is what bounds the conversion (measured).
 template <int D>
-__device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uint32_t m_paged, int nvp, uint32_t mul, int cw,
-                                                 int lane)
+__device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uint32_t m_paged, int nvp, uint32_t mul, int first,
+                                                 int stride, int lane)
 {
     constexpr int kLanesPerRow = D / 16, kRowsPerIt = 32 / kLanesPerRow, kItPerBlock = kBlock / kRowsPerIt;
     constexpr int kHalfBytes = kTileM * 128;
     const int chunk = lane % kLanesPerRow, rsub = lane / kLanesPerRow;
+    const uint32_t c0 = static_cast<uint32_t>(2 * (chunk & 3));
+    const uint32_t src0 = stg + static_cast<uint32_t>(rsub * D + chunk * 16);
+    const uint32_t dst0 = dst + static_cast<uint32_t>((chunk >> 2) * kHalfBytes + rsub * 128);
+    constexpr int kIters = kVbPerTile * kItPerBlock;
+    auto convert_store = [&](int it, uint32_t w0, uint32_t w1, uint32_t w2, uint32_t w3) {
+        const int row0 = (it / kItPerBlock) * kBlock + (it % kItPerBlock) * kRowsPerIt;      // tile row of the iteration's first row
+        const uint32_t base = dst0 + static_cast<uint32_t>(row0 * 128);
+        const uint32_t x = static_cast<uint32_t>((row0 + rsub) & 7);
+        const uint32_t o0 = e4m3x2_to_bf16x2(w0, mul), o1 = e4m3x2_to_bf16x2(w0 >> 16, mul);
+        const uint32_t o2 = e4m3x2_to_bf16x2(w1, mul), o3 = e4m3x2_to_bf16x2(w1 >> 16, mul);
+        const uint32_t o4 = e4m3x2_to_bf16x2(w2, mul), o5 = e4m3x2_to_bf16x2(w2 >> 16, mul);
+        const uint32_t o6 = e4m3x2_to_bf16x2(w3, mul), o7 = e4m3x2_to_bf16x2(w3 >> 16, mul);
+        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(base + ((c0 ^ x) << 4)), "r"(o0), "r"(o1), "r"(o2), "r"(o3) : "memory");
+        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(base + (((c0 + 1) ^ x) << 4)), "r"(o4), "r"(o5), "r"(o6), "r"(o7) : "memory");
+    };
+    auto load = [&](int it, uint32_t &w0, uint32_t &w1, uint32_t &w2, uint32_t &w3) {
+        const int row0 = (it / kItPerBlock) * kBlock + (it % kItPerBlock) * kRowsPerIt;
+        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
+                     : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3)
+                     : "r"(src0 + static_cast<uint32_t>(row0 * D)));
+    };
+    const bool all_full = m_paged == 0xffu && __all_sync(0xffffffffu, lane >= kVbPerTile || (nvp & 0xff) == kBlock);
+    if (all_full) {
+        // the common tile (eight full cached blocks): four loads in flight before the first conversion -- one warp per
+        // SM sub-partition converts, and a shared-memory load takes a few hundred cycles next to the tensor core's reads
+        constexpr int kBatch = 4;
+#pragma unroll 1
+        for (int it0 = first; it0 < kIters; it0 += kBatch * stride) {
+            uint32_t w[kBatch][4];
 #pragma unroll
-    for (int it0 = 0; it0 < kVbPerTile * kItPerBlock; it0 += kConvWarps) {
-        const int it = it0 + cw;
+            for (int k = 0; k < kBatch; ++k)
+                if (it0 + k * stride < kIters) load(it0 + k * stride, w[k][0], w[k][1], w[k][2], w[k][3]);
+#pragma unroll
+            for (int k = 0; k < kBatch; ++k)
+                if (it0 + k * stride < kIters) convert_store(it0 + k * stride, w[k][0], w[k][1], w[k][2], w[k][3]);
+        }
+        return;
+    }
+#pragma unroll 1
+    for (int it = first; it < kIters; it += stride) {
         const int b = it / kItPerBlock;
         const int nv = __shfl_sync(0xffffffffu, nvp, b) & 0xff;
-        const int row = (it % kItPerBlock) * kRowsPerIt + rsub;
-        if (((m_paged >> b) & 1u) && row < nv) {
+        if (((m_paged >> b) & 1u) && (it % kItPerBlock) * kRowsPerIt + rsub < nv) {
             uint32_t w0, w1, w2, w3;
-            asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
-                         : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3)
-                         : "r"(stg + static_cast<uint32_t>((b * kBlock + row) * D + chunk * 16)));
-            const int r = b * kBlock + row;
-            const uint32_t base = dst + static_cast<uint32_t>((chunk >> 2) * kHalfBytes + r * 128);
-            const uint32_t c0 = static_cast<uint32_t>(2 * (chunk & 3)), x = static_cast<uint32_t>(r & 7);
-            const uint32_t a_lo = base + (((c0) ^ x) << 4), a_hi = base + (((c0 + 1) ^ x) << 4);
-            const uint32_t o0 = e4m3x2_to_bf16x2(w0, mul), o1 = e4m3x2_to_bf16x2(w0 >> 16, mul);
-            const uint32_t o2 = e4m3x2_to_bf16x2(w1, mul), o3 = e4m3x2_to_bf16x2(w1 >> 16, mul);
-            const uint32_t o4 = e4m3x2_to_bf16x2(w2, mul), o5 = e4m3x2_to_bf16x2(w2 >> 16, mul);
-            const uint32_t o6 = e4m3x2_to_bf16x2(w3, mul), o7 = e4m3x2_to_bf16x2(w3 >> 16, mul);
-            // lanes of the upper half (D = 128) store their two chunks in the other order: the eight lanes of a
-            // quarter-warp then hit eight different 16-byte bank groups
-            if (chunk & 4) {
-                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a_hi), "r"(o4), "r"(o5), "r"(o6), "r"(o7) : "memory");
-                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a_lo), "r"(o0), "r"(o1), "r"(o2), "r"(o3) : "memory");
-            } else {
-                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a_lo), "r"(o0), "r"(o1), "r"(o2), "r"(o3) : "memory");
-                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a_hi), "r"(o4), "r"(o5), "r"(o6), "r"(o7) : "memory");
-            }
+            load(it, w0, w1, w2, w3);
+            convert_store(it, w0, w1, w2, w3);
         }
     }
 }
 
-template <int D, bool KV8>
+// KV8 converters (warps 8-11): every ring entry of the unit in ring order; for an entry whose tile holds cached blocks,
+// the calling warp converts iterations first, first + stride, ... of the staged codes into the tile's ring slot
+// (first < 0: nothing) and arrives on the staging slot's "empty" barrier; every warp arrives on the ring slot's "full"
+// barrier for every entry.  An entry is waited for even when there is nothing to convert: a waiter that skips a use
+// of a slot cannot tell the phases of its barrier apart.
+template <class C, int D>
+__device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkUnit &wu, uint32_t bar0, uint32_t sStg, uint32_t sRing,
+                                                 int lane, int first, int stride, uint32_t &cv_ent, uint32_t &cv_stg)
+{
+    auto bar = [bar0](int i) { return bar0 + static_cast<uint32_t>(i) * 8u; };
+    const int n = wu.tile_end - wu.tile_begin;
+    const bool pair = wu.mode == kModePair;
+    const uint32_t mul_k = __ldg(P.kv8_mul + wu.kvh), mul_v = __ldg(P.kv8_mul + P.Hkv + wu.kvh);
+    auto fetch_nvp = [&](int e) -> int {             // lane b < 8: nvalid | paged << 8 of virtual block b of entry e's tile
+        int r = 0;
+        if (e < 2 * n) {
+            bool is_v;
+            int t;
+            kv8_entry(e, n, pair, is_v, t);
+            const int tile = wu.tile_begin + t;
+            if (lane < kVbPerTile && tile * kVbPerTile + lane < wu.vb_count) {
+                const int4 v = __ldg(reinterpret_cast<const int4 *>(P.vblocks + wu.vb_begin + tile * kVbPerTile + lane));
+                r = v.z | ((v.z > 0 && v.w != 0) ? 256 : 0);
+            }
+        }
+        return r;
+    };
+    int cur = fetch_nvp(0);
+#pragma unroll 1
+    for (int e = 0; e < 2 * n; ++e) {
+        const int nxt = fetch_nvp(e + 1);
+        const uint32_t m_paged = __ballot_sync(0xffffffffu, (cur >> 8) != 0) & 0xffu;
+        bool is_v;
+        int t;
+        kv8_entry(e, n, pair, is_v, t);
+        const uint32_t slot = cv_ent & (C::kStages - 1);
+        mbar_wait(bar(kBarKvEmpty + slot), ((cv_ent / C::kStages) & 1u) ^ 1u);
+        if (m_paged != 0) {
+            const uint32_t st = cv_stg & static_cast<uint32_t>(C::kStgDiv - 1);
+            mbar_wait(bar(kBarStgFull + st), (cv_stg / C::kStgDiv) & 1u);
+            if (first >= 0)
+                kv8_convert_tile<D>(sStg + st * C::kStgTileBytes, sRing + slot * C::kTileBytes, m_paged, cur, is_v ? mul_v : mul_k,
+                                    first, stride, lane);
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(kBarStgEmpty + st));
+            ++cv_stg;
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(kBarKvFull + slot));
+        ++cv_ent;
+        cur = nxt;
+    }
+}
+
+template <int D, bool KV8, int QT>
 __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_constant__ FwdParams P)
 {
-    using C = PipeCfg<D, KV8>;
+    using C = PipeCfg<D, KV8, QT>;
+    static_assert(!KV8 || (C::kStages & (C::kStages - 1)) == 0, "KV8 ring positions are taken from an entry counter with a mask");
     extern __shared__ __align__(1024) uint8_t smem[];
     const uint32_t sbase = smem_u32(smem);
     const uint32_t sQ = sbase, sRing = sbase + C::kQBytes;
@@ -249,7 +366,8 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
         asm volatile("setmaxnreg.inc.sync.aligned.u32 184;");
         const int c = warp >> 2;                       // chain
         const int row = threadIdx.x & 127;
-        const int g = row / R, t = row - g * R;
+        // row of a q tile -> token: token-major (row = t * G + g) or head-major (row = g * R + t), FwdParams::token_major
+        const int t = P.token_major ? row / G : row % R;
         const uint32_t trow = tmem + (static_cast<uint32_t>((warp & 3) * 32) << 16);
         const uint32_t tS = trow + C::kColS + c * C::kChainCols;
         const uint32_t tO = trow + C::kColO + c * C::kChainCols;
@@ -264,6 +382,26 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             if (steps <= 0) continue;
             const int p_row = wu.q_abs0 + (pair ? c * R : 0) + t;
             const int p_min = wu.q_abs0 + (pair ? c * R : 0);
+            // Token-major packing: the valid rows of the tile are its first tok * G rows.  A warp whose 32 rows lie beyond
+            // them skips the unit's tiles altogether (its rows of S, P and O hold garbage nobody reads); the first warp of
+            // the chain gives the idle warps' arrivals on the P barriers along with its own.
+            uint32_t p_arrivals = 1;
+            if (P.token_major) {
+                const int tok = pair ? min(max(wu.n_tok - c * R, 0), R) : wu.n_tok;
+                const int active = max(1, min(4, (tok * G + 31) >> 5));
+                if ((warp & 3) >= active) {
+                    ph_s ^= static_cast<uint32_t>(steps & 1);
+                    mbar_wait(bar(kBarStFree + c), ph_stfree);
+                    ph_stfree ^= 1;
+                    stats[c * kTileM + row] = make_float2(0.f, 0.f);
+                    // sync, not arrive: the warp stays here (in hardware, no issue slots) until the chain's working warps
+                    // have finished the unit -- were it to go on and wait for S of the next unit, a barrier that is still
+                    // several phases behind would show it the parity it expects
+                    named_bar_sync(kNamedStFull + c, 256);
+                    continue;
+                }
+                if ((warp & 3) == 0) p_arrivals += static_cast<uint32_t>(4 - active);
+            }
             // Row state: integer reference `ref` (log2 units), l = sum of 2^(s*sl - ref) so far,
             // m_run = running max of the raw scores.  See msa_softmax.cuh.
             float ref = 0.f, l = 0.f, m_run = -INFINITY;
@@ -322,7 +460,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     float tile_sum, tile_max;
                     done = softmax_fast_tile(tS, sl, ref, tile_sum, tile_max, [&](int part) {
                         __syncwarp();
-                        if (lane == 0) mbar_arrive(bar((part == 0 ? kBarPLo : kBarPQ2) + c));
+                        if (lane == 0) mbar_arrive_n(bar((part == 0 ? kBarPLo : kBarPQ2) + c), p_arrivals);
                         if ((threadIdx.x & 127) == 0 && part == 0) PROF_TRACE(1 + c, s, 4);
                     }, [&](int ev) {
                         if ((threadIdx.x & 127) == 0) PROF_TRACE(1 + c, s, ev);
@@ -331,7 +469,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                         l += tile_sum;
                         m_run = fmaxf(m_run, tile_max);
                         __syncwarp();
-                        if (lane == 0) mbar_arrive(bar(kBarPQ3 + c));
+                        if (lane == 0) mbar_arrive_n(bar(kBarPQ3 + c), p_arrivals);
                     }
                     PROF_ADD(20);
                 }
@@ -378,7 +516,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     auto publish = [&](int b) {
                         tc_fence_before();
                         __syncwarp();
-                        if (lane == 0) mbar_arrive(bar(b + c));
+                        if (lane == 0) mbar_arrive_n(bar(b + c), p_arrivals);
                     };
                     uint32_t pka[16], pkb[16];
                     exact_chunk(0, pka);
@@ -417,64 +555,30 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
         // =========================================================== epilogue warpgroup
         asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
         const int row = threadIdx.x & 127;
-        const int g = row / R, t = row - g * R;
+        const int t = P.token_major ? row / G : row % R;
+        const int g = P.token_major ? row % G : row / R;
         const uint32_t trow = tmem + (static_cast<uint32_t>((warp & 3) * 32) << 16);
         uint32_t ph_o[2] = {0, 0};
-        uint32_t cv_slot = 0, cv_ph = 1, cv_st = 0, cv_stph = 0;     // KV8: ring entry / staging entry the converters are at
-        (void)cv_slot; (void)cv_ph; (void)cv_st; (void)cv_stph;
+        uint32_t cv_ent = 0, cv_stg = 0;       // KV8: ring entry / staging entry the converters are at (CTA-wide counters)
+        (void)cv_ent; (void)cv_stg;
+        PROF_DECL();
         for (int u = u_begin; u < u_end; ++u) {
             const WorkUnit wu = P.units[u];
             const int n = wu.tile_end - wu.tile_begin;
             const bool pair = wu.mode == kModePair;
             const int rows_total = wu.n_tok * G;
             if constexpr (KV8) {
-                // ---- converters: every ring entry of the unit in order (K, V of tile 0, K, V of tile 1, ...).  An entry
-                // is waited for even when its tile holds no cached block: a waiter that skips a use of a slot cannot
-                // tell the phases of its barrier apart.
-                const int cw = warp - 8;
-                const uint32_t mul_k = __ldg(P.kv8_mul + wu.kvh), mul_v = __ldg(P.kv8_mul + P.Hkv + wu.kvh);
-                auto fetch_nvp = [&](int tile) -> int {          // lane b < 8: nvalid | paged << 8 of virtual block b
-                    int r = 0;
-                    if (lane < kVbPerTile && tile < wu.tile_end && tile * kVbPerTile + lane < wu.vb_count) {
-                        const int4 e = __ldg(reinterpret_cast<const int4 *>(P.vblocks + wu.vb_begin + tile * kVbPerTile + lane));
-                        r = e.z | ((e.z > 0 && e.w != 0) ? 256 : 0);
-                    }
-                    return r;
-                };
-                int cur = n > 0 ? fetch_nvp(wu.tile_begin) : 0;
-#pragma unroll 1
-                for (int j = 0; j < n; ++j) {
-                    const int nxt = fetch_nvp(wu.tile_begin + j + 1);
-                    const uint32_t m_paged = __ballot_sync(0xffffffffu, (cur >> 8) != 0) & 0xffu;
-#pragma unroll 1
-                    for (int which = 0; which < 2; ++which) {
-                        mbar_wait(bar(kBarKvEmpty + cv_slot), cv_ph);
-                        if (m_paged != 0) {
-                            mbar_wait(bar(kBarStgFull + cv_st), cv_stph);
-                            kv8_convert_tile<D>(sStg + cv_st * C::kStgTileBytes, sRing + cv_slot * C::kTileBytes, m_paged, cur,
-                                                which ? mul_v : mul_k, cw, lane);
-                            fence_proxy_async_smem();
-                            __syncwarp();
-                            if (lane == 0) mbar_arrive(bar(kBarStgEmpty + cv_st));
-                            if (++cv_st == C::kStgStages) {
-                                cv_st = 0;
-                                cv_stph ^= 1;
-                            }
-                        }
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(bar(kBarKvFull + cv_slot));
-                        if (++cv_slot == C::kStages) {
-                            cv_slot = 0;
-                            cv_ph ^= 1;
-                        }
-                    }
-                    cur = nxt;
-                }
+                // ---- converters (kv8_convert_unit): all four warps, unless the unit's valid q rows fit one softmax warp per
+                // chain (token-major packing, short queries) -- those two warps exponentiate on SM sub-partition 0, which warp 8
+                // shares with them, so warps 9-11 take the whole tile and warp 8 only gives its arrivals.
+                const bool one_row_warp = P.token_major && !pair && wu.n_tok * G <= 32;
+                kv8_convert_unit<C, D>(P, wu, bar0, sStg, sRing, lane, one_row_warp ? warp - 9 : warp - 8, one_row_warp ? 3 : 4, cv_ent,
+                                       cv_stg);
             }
             const int n_out = pair ? 2 : 1;                       // q tiles written by this unit
             for (int qt = 0; qt < n_out; ++qt) {
                 const int tok = qt * R + t;
-                const bool row_valid = (g < G) && (tok < wu.n_tok);
+                const bool row_valid = (g < G) && (t < R) && (tok < wu.n_tok);
                 const int head = row_valid ? P.kv_to_q[wu.kvh * G + g] : 0;
                 float w0 = 0.f, w1 = 0.f, inv_l = 0.f, lse_val = -INFINITY;
                 bool act0 = false, act1 = false;
@@ -580,6 +684,12 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                 }
             }
         }
+#if defined(MSA_PROF) && MSA_PROF != 2
+#ifndef MSA_PROF_CVWARP
+#define MSA_PROF_CVWARP 8
+#endif
+        if (warp == MSA_PROF_CVWARP && lane == 0) { PROF_FLUSH(21, 25); PROF_FLUSH(27, 28); }
+#endif
     } else {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
         if (warp == 12 || warp == 14) {
@@ -590,12 +700,18 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             const CUtensorMap *tm_ctg = which ? P.tm_ctg_v : P.tm_ctg_k;
             const CUtensorMap *tm_ctg128 = which ? &P.tm_ctg_v128 : &P.tm_ctg_k128;
             RingPos rp{static_cast<uint32_t>(which), 1};
-            // KV8 (three ring slots): this loader also waits, in ring order, for the slots of the OTHER loader's entries.
-            // A waiter that does not see every use of a slot cannot tell its barrier's phases apart: with three slots the
-            // V loader could otherwise run from V(i) to V(i+3) -- the same slot two uses later -- while V(i) is still
-            // being multiplied, find the parity it expects and overwrite the tile.
-            RingPos ro{static_cast<uint32_t>(which ^ 1), 1};
-            (void)ro;
+            // KV8: ring positions come from an entry counter (the ring order depends on the unit's mode), and this loader
+            // also waits, in ring order, for the slots of the entries it does not fill: a waiter that does not see every
+            // use of a slot cannot tell its barrier's phases apart (with few slots the V loader could otherwise run two
+            // uses of a slot ahead of a V tile that is still being multiplied, find the parity it expects and overwrite it).
+            uint32_t ent = 0;
+            (void)ent;
+            auto observe_until = [&](uint32_t target) {
+                while (ent < target) {
+                    mbar_wait(bar(kBarKvEmpty + (ent & (C::kStages - 1))), ((ent / C::kStages) & 1u) ^ 1u);
+                    ++ent;
+                }
+            };
             uint32_t ph_qempty = 1;
             PROF_DECL();
             for (int u = u_begin; u < u_end; ++u) {
@@ -606,7 +722,18 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     const int nq = wu.mode == kModePair ? 2 : 1;
                     mbar_wait(bar(kBarQEmpty), ph_qempty);
                     ph_qempty ^= 1;
-                    if (elect_one()) {
+                    if (P.token_major) {
+                        // one box per q tile and 64-element half: G heads x R tokens, rows land as (token, head)
+                        if (elect_one()) {
+                            mbar_arrive_expect_tx(bar(kBarQFull), static_cast<uint32_t>(nq * G * R * D * 2));
+                            const int hq0 = __ldg(P.kv_to_q + wu.kvh * G);
+                            for (int c = 0; c < nq; ++c)
+#pragma unroll
+                                for (int h = 0; h < C::kHalves; ++h)
+                                    tma_load_3d(sQ + c * C::kTileBytes + h * C::kHalfBytes, &P.tm_q3, bar(kBarQFull), h * 64, hq0,
+                                                wu.q_row0 + c * R);
+                        }
+                    } else if (elect_one()) {
                         mbar_arrive_expect_tx(bar(kBarQFull), static_cast<uint32_t>(nq * G * R * D * 2));
                         for (int g = 0; g < G; ++g) {
                             const int hq = __ldg(P.kv_to_q + wu.kvh * G + g);
@@ -620,6 +747,9 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     __syncwarp();
                 }
                 const int c0 = wu.kvh * D;
+                const uint32_t ent_base = ent;
+                const bool pair_u = wu.mode == kModePair;
+                (void)ent_base; (void)pair_u;
                 // lane b < 8 owns virtual block b of a tile: fetch its entry, then resolve its row
                 auto fetch = [&](int tile) -> int4 {
                     int4 e = make_int4(0, 0, 0, 0);
@@ -657,17 +787,20 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     for (int b = 0; b < kVbPerTile; ++b) rows_b[b] = __shfl_sync(0xffffffffu, cur.row, b);
                     const bool run = m_full == 0xffu && m_paged == 0 &&
                                      __all_sync(0xffffffffu, lane >= kVbPerTile || cur.row == rows_b[0] + lane * kBlock);
-                    if (KV8 && which == 1) {                       // K(j) comes before V(j) in the ring
-                        mbar_wait(bar(kBarKvEmpty + ro.slot), ro.phase);
-                        ro.advance2(C::kStages);
+                    uint32_t slot = rp.slot, phase = rp.phase;
+                    if constexpr (KV8) {
+                        observe_until(ent_base + static_cast<uint32_t>(which ? kv8_entry_of_v(j, n, pair_u) : kv8_entry_of_k(j, pair_u)));
+                        slot = ent & (C::kStages - 1);
+                        phase = ((ent / C::kStages) & 1u) ^ 1u;
+                        ++ent;
                     }
                     {
                         PROF_T0();
-                        mbar_wait(bar(kBarKvEmpty + rp.slot), rp.phase);
+                        mbar_wait(bar(kBarKvEmpty + slot), phase);
                         PROF_ADD(16);
                     }
-                    const uint32_t full = bar(kBarKvFull + rp.slot);
-                    const uint32_t dst = sRing + rp.slot * C::kTileBytes;
+                    const uint32_t full = bar(kBarKvFull + slot);
+                    const uint32_t dst = sRing + slot * C::kTileBytes;
                     if (which == 1 && m_full != 0xffu) {
                         // V rows TMA will not write (block tails, blocks past the end / the horizon): zero them
                         // (generic-proxy stores, made visible to the tensor core's async proxy before the tile is armed)
@@ -726,16 +859,13 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     __syncwarp();
                     // second arrival on the slot's empty barrier: here, at once, unless this is a write-back launch (then the
                     // write-back warp gives it for every tile, after its stores -- if any -- have read the slot)
-                    if (kWritebackRing && !wb && elect_one()) mbar_arrive(bar(kBarKvEmpty + rp.slot));
+                    if (kWritebackRing && !wb && elect_one()) mbar_arrive(bar(kBarKvEmpty + slot));
                     rp.advance2(C::kStages);
-                    if (KV8 && which == 0) {                       // V(j) follows K(j)
-                        mbar_wait(bar(kBarKvEmpty + ro.slot), ro.phase);
-                        ro.advance2(C::kStages);
-                    }
                     cur = nxt;
                     nxt = resolve(raw);
                     raw = fetch(wu.tile_begin + j + 3);
                 }
+                if constexpr (KV8) observe_until(ent_base + 2u * static_cast<uint32_t>(n));
             }
 #if defined(MSA_PROF) && MSA_PROF != 2
             if (lane == 0) g_prof[blockIdx.x][16 + which] += prof_acc[16];
@@ -752,21 +882,41 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
 #if defined(MSA_PROF) && MSA_PROF != 2
             const long long prof_mma_start = clock64();
 #endif
+            uint32_t ment = 0;               // KV8: the ring is in the order of the take_k / take_v calls below
+            (void)ment;
             auto take_k = [&]() -> uint32_t {
-                const uint32_t slot = rk.slot;
-                PROF_T0();
-                mbar_wait(bar(kBarKvFull + slot), rk.phase);
-                PROF_ADD(8);
-                rk.advance2(C::kStages);
-                return slot;
+                if constexpr (KV8) {
+                    const uint32_t slot = ment & (C::kStages - 1);
+                    PROF_T0();
+                    mbar_wait(bar(kBarKvFull + slot), (ment / C::kStages) & 1u);
+                    PROF_ADD(8);
+                    ++ment;
+                    return slot;
+                } else {
+                    const uint32_t slot = rk.slot;
+                    PROF_T0();
+                    mbar_wait(bar(kBarKvFull + slot), rk.phase);
+                    PROF_ADD(8);
+                    rk.advance2(C::kStages);
+                    return slot;
+                }
             };
             auto take_v = [&]() -> uint32_t {
-                const uint32_t slot = rv.slot;
-                PROF_T0();
-                mbar_wait(bar(kBarKvFull + slot), rv.phase);
-                PROF_ADD(9);
-                rv.advance2(C::kStages);
-                return slot;
+                if constexpr (KV8) {
+                    const uint32_t slot = ment & (C::kStages - 1);
+                    PROF_T0();
+                    mbar_wait(bar(kBarKvFull + slot), (ment / C::kStages) & 1u);
+                    PROF_ADD(9);
+                    ++ment;
+                    return slot;
+                } else {
+                    const uint32_t slot = rv.slot;
+                    PROF_T0();
+                    mbar_wait(bar(kBarKvFull + slot), rv.phase);
+                    PROF_ADD(9);
+                    rv.advance2(C::kStages);
+                    return slot;
+                }
             };
             // Descriptors: only the 14-bit start-address field (address >> 4) differs between the operands of one
             // tile, and it never carries out of its field (shared memory ends below 256 KB), so a tile's descriptor
@@ -915,81 +1065,98 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
         }
         else if (KV8 && warp == 15) {
             // ======================================================= KV8: loader of the fp8 blocks (staging ring)
-            // For every tile that holds cached blocks: their K codes into one staging slot, their V codes into the next
-            // (block b at b * 16 * D, rows of D bytes, no swizzle).  Independent of the bf16 ring, so the fp8 stream runs
-            // kStgStages tiles ahead of the converters whatever the tensor core is doing.
-            uint32_t st = 0, st_ph = 1;
+            // Ring entries in ring order; for every entry whose tile holds cached blocks, their codes go into the next
+            // staging slot (block b at b * 16 * D, rows of D bytes, no swizzle).  Independent of the bf16 ring, so the fp8
+            // stream runs kStgStages entries ahead of the converters whatever the tensor core is doing.
+            uint32_t stg = 0;
+            PROF_DECL();
+#if defined(MSA_PROF) && MSA_PROF != 2
+            const long long prof_stg_start = clock64();
+#endif
             for (int u = u_begin; u < u_end; ++u) {
                 const WorkUnit wu = P.units[u];
                 const int n = wu.tile_end - wu.tile_begin;
                 if (n <= 0) continue;
                 const int c0 = wu.kvh * D;
-                auto fetch = [&](int tile) -> int4 {
-                    int4 e = make_int4(0, 0, 0, 0);
-                    if (lane < kVbPerTile && tile < wu.tile_end && tile * kVbPerTile + lane < wu.vb_count)
-                        e = __ldg(reinterpret_cast<const int4 *>(P.vblocks + wu.vb_begin + tile * kVbPerTile + lane));
-                    return e;
+                const bool pair_u = wu.mode == kModePair;
+                auto fetch = [&](int e) -> int4 {                 // vblock entry of lane b < 8 for ring entry e (zeros past the unit)
+                    int4 v = make_int4(0, 0, 0, 0);
+                    if (e < 2 * n) {
+                        bool is_v;
+                        int t;
+                        kv8_entry(e, n, pair_u, is_v, t);
+                        const int tile = wu.tile_begin + t;
+                        if (lane < kVbPerTile && tile * kVbPerTile + lane < wu.vb_count)
+                            v = __ldg(reinterpret_cast<const int4 *>(P.vblocks + wu.vb_begin + tile * kVbPerTile + lane));
+                    }
+                    return v;
                 };
-                auto resolve = [&](const int4 &e) -> ResolvedVb {     // nvp = valid slots of a CACHED block (0 otherwise)
+                auto resolve = [&](const int4 &v) -> ResolvedVb {     // nvp = valid slots of a CACHED block (0 otherwise)
                     ResolvedVb r;
-                    const bool pg = e.z > 0 && e.w != 0;
-                    r.nvp = pg ? e.z : 0;
-                    r.row = pg ? __ldg(P.block_table + e.x) * kBlock : 0;
+                    const bool pg = v.z > 0 && v.w != 0;
+                    r.nvp = pg ? v.z : 0;
+                    r.row = pg ? __ldg(P.block_table + v.x) * kBlock : 0;
                     return r;
                 };
-                ResolvedVb cur = resolve(fetch(wu.tile_begin));
-                ResolvedVb nxt = resolve(fetch(wu.tile_begin + 1));
-                int4 raw = fetch(wu.tile_begin + 2);
+                ResolvedVb cur = resolve(fetch(0));
+                ResolvedVb nxt = resolve(fetch(1));
+                int4 raw = fetch(2);
 #pragma unroll 1
-                for (int j = 0; j < n; ++j) {
+                for (int e = 0; e < 2 * n; ++e) {
                     const int nv = cur.nvp;
                     const uint32_t m_paged = __ballot_sync(0xffffffffu, nv > 0) & 0xffu;
                     const uint32_t m_full = __ballot_sync(0xffffffffu, nv == kBlock) & 0xffu;
                     if (m_paged != 0) {
-                        int rows_b[kVbPerTile];
-#pragma unroll
-                        for (int b = 0; b < kVbPerTile; ++b) rows_b[b] = __shfl_sync(0xffffffffu, cur.row, b);
+                        bool is_v;
+                        int t;
+                        kv8_entry(e, n, pair_u, is_v, t);
+                        const CUtensorMap *tm = is_v ? P.tm_pool_v : P.tm_pool_k;
+                        const uint32_t st = stg & static_cast<uint32_t>(C::kStgDiv - 1);
                         const uint32_t rows = __reduce_add_sync(0xffffffffu, static_cast<uint32_t>(nv));
-#pragma unroll 1
-                        for (int which = 0; which < 2; ++which) {
-                            const CUtensorMap *tm = which ? P.tm_pool_v : P.tm_pool_k;
-                            mbar_wait(bar(kBarStgEmpty + st), st_ph);
-                            const uint32_t full = bar(kBarStgFull + st);
-                            const uint32_t dst = sStg + st * C::kStgTileBytes;
-                            if (m_paged == m_full) {
-                                if (elect_one()) {
-                                    mbar_arrive_expect_tx(full, rows * D);
+                        {
+                            PROF_T0();
+                            mbar_wait(bar(kBarStgEmpty + st), ((stg / C::kStgDiv) & 1u) ^ 1u);
+                            PROF_ADD(25);
+                        }
+                        const uint32_t full = bar(kBarStgFull + st);
+                        const uint32_t dst = sStg + st * C::kStgTileBytes;
+                        if (m_paged == m_full) {
+                            int rows_b[kVbPerTile];
 #pragma unroll
-                                    for (int b = 0; b < kVbPerTile; ++b)
-                                        if (m_paged >> b & 1) tma_load_2d(dst + b * (kBlock * D), tm, full, c0, rows_b[b]);
-                                }
-                            } else {
-                                if (elect_one()) mbar_arrive_expect_tx(full, rows * D);
-                                __syncwarp();
-                                if (nv > 0) {     // a partly filled block loads only its valid rows (8/4/2/1-row boxes)
-                                    int off = 0;
+                            for (int b = 0; b < kVbPerTile; ++b) rows_b[b] = __shfl_sync(0xffffffffu, cur.row, b);
+                            if (elect_one()) {
+                                mbar_arrive_expect_tx(full, rows * D);
+#pragma unroll
+                                for (int b = 0; b < kVbPerTile; ++b)
+                                    if (m_paged >> b & 1) tma_load_2d(dst + b * (kBlock * D), tm, full, c0, rows_b[b]);
+                            }
+                        } else {
+                            if (elect_one()) mbar_arrive_expect_tx(full, rows * D);
+                            __syncwarp();
+                            if (nv > 0) {     // a partly filled block loads only its valid rows (8/4/2/1-row boxes)
+                                int off = 0;
 #pragma unroll 1
-                                    for (int i = 0; i < 5; ++i) {
-                                        const int rows_i = kBlock >> i;
-                                        if (nv & rows_i) {
-                                            tma_load_2d(dst + lane * (kBlock * D) + off * D, tm + i, full, c0, cur.row + off);
-                                            off += rows_i;
-                                        }
+                                for (int i = 0; i < 5; ++i) {
+                                    const int rows_i = kBlock >> i;
+                                    if (nv & rows_i) {
+                                        tma_load_2d(dst + lane * (kBlock * D) + off * D, tm + i, full, c0, cur.row + off);
+                                        off += rows_i;
                                     }
                                 }
                             }
-                            __syncwarp();
-                            if (++st == C::kStgStages) {
-                                st = 0;
-                                st_ph ^= 1;
-                            }
                         }
+                        __syncwarp();
+                        ++stg;
                     }
                     cur = nxt;
                     nxt = resolve(raw);
-                    raw = fetch(wu.tile_begin + j + 3);
+                    raw = fetch(e + 3);
                 }
             }
+#if defined(MSA_PROF) && MSA_PROF != 2
+            prof_acc[26] = static_cast<unsigned long long>(clock64() - prof_stg_start);
+            if (lane == 0) PROF_FLUSH(25, 27);
+#endif
         }
         else if (warp == 15 && P.vb_dst != nullptr) {
             // ======================================================= write-back warp (plans from msa_plan_create_writeback)

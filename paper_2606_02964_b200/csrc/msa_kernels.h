@@ -10,6 +10,7 @@ namespace msa {
 
 struct FwdParams {
     CUtensorMap tm_q;        // bf16 [total_q][Hq*D], box 64 x R
+    CUtensorMap tm_q3;       // the same tensor as [total_q][Hq][D], box 64 x G x R (token-major row packing, see token_major)
     // K/V tensors: pool bf16 [num_blocks*16][Hkv*D], arena bf16 [contig_rows][Hkv*D]; boxes of
     // 64 elements x {16, 8, 4, 2, 1} rows: a partly filled block loads only its valid rows.
     // fp8 pool: tm_pool_* are over bytes [num_blocks*16][Hkv*D] with boxes of D bytes x {16, 8, 4, 2, 1} rows, no swizzle.
@@ -26,12 +27,15 @@ struct FwdParams {
     const int32_t *vb_dst;           // fused KV write-back (NULL: none): per virtual block, block-table index of its destination or -1
     const int32_t *tile_writer;      // ... and per context KV tile, q_row0 of the work item that stores it (or -1)
     const int32_t *kv_to_q;          // [Hkv][G] q heads of each kv head
-    const uint32_t *kv8_mul;         // fp8 pool only: [2][Hkv] bf16x2 {2^(112+k), 2^(112+k)} for K then V, scale = 2^k (see e4m3x2_to_bf16x2)
+    const uint32_t *kv8_mul;         // fp8 pool only: [2][Hkv] f16 bits of 2^k for K then V, scale = 2^k (see e4m3x2_to_bf16x2)
     void *o;                         // bf16 [total_q][Hq][D]
     float *lse;                      // [total_q][Hq]
     float *workspace;
     float scale_log2;                // softmax_scale * log2(e)
     int32_t Hq, Hkv, G, R;           // R = tokens per 128-row tile
+    int32_t token_major;             // 1: row r of a q tile = (token r / G, head r % G) -- the valid rows of a short query are
+                                     // a prefix of the tile, so whole softmax warps have nothing to do; needs the q heads of
+                                     // every KV head to be consecutive (one 3-D box loads a tile).  0: r = (head r / R, token r % R)
 };
 
 struct MergeParams {
@@ -68,7 +72,8 @@ cudaError_t launch_append(const AppendParams &p, int num_sms, cudaStream_t strea
 // shared-memory limit on the CURRENT device (once per device and head dim); launch_fwd assumes it was done.
 constexpr int kTilesPerGroup = 2;    // q tiles (of 128 packed rows) one work item covers in pair mode
 cudaError_t configure_fwd(int head_dim, bool kv8);
-cudaError_t launch_fwd(const FwdParams &p, int head_dim, bool kv8, int num_ctas, cudaStream_t stream);
+// one_q_tile (fp8 pool only): the plan has no pair-mode unit, so the layout with one Q tile and the deeper staging ring serves it
+cudaError_t launch_fwd(const FwdParams &p, int head_dim, bool kv8, bool one_q_tile, int num_ctas, cudaStream_t stream);
 cudaError_t launch_merge(const MergeParams &p, int n_items, int max_rows, cudaStream_t stream);
 
 }  // namespace msa

@@ -23,10 +23,10 @@ TOL_O_MAX, TOL_O_MEAN, TOL_LSE = 2e-2, 2e-3, 1e-3
 
 # ------------------------------------------------------------------ CPU: host logic and the quantiser oracle
 def test_scales_must_be_powers_of_two_within_range():
-    ok = msa_create(8, 2, 128, device=-1, pool_format=MSA_POOL_FP8_E4M3, k_scale=[0.25, 2.0 ** -14], v_scale=[2.0 ** 14, 1.0])
+    ok = msa_create(8, 2, 128, device=-1, pool_format=MSA_POOL_FP8_E4M3, k_scale=[0.25, 2.0 ** -14], v_scale=[2.0 ** 7, 1.0])
     msa_destroy(ok)
     msa_destroy(msa_create(8, 2, 128, device=-1, pool_format=MSA_POOL_FP8_E4M3))            # NULL scales: all 1.0
-    for bad in ([0.3, 1.0], [2.0 ** -15, 1.0], [2.0 ** 15, 1.0]):
+    for bad in ([0.3, 1.0], [2.0 ** -15, 1.0], [2.0 ** 8, 1.0]):
         with pytest.raises(MsaError) as e:
             msa_create(8, 2, 128, device=-1, pool_format=MSA_POOL_FP8_E4M3, k_scale=bad)
         assert e.value.status == MSA_ERR_UNSUPPORTED
@@ -129,7 +129,7 @@ CASES = [
 @pytest.mark.parametrize("kw", CASES, ids=lambda k: f"seed{k['seed']}")
 def test_kv8_random_small_problems_against_the_oracle_and_the_bf16_kernel(kw):
     p = W.random_problem(device=DEV, keep_dense=False, **kw)
-    exps = [(-6, -4), (-5, -7), (-7, -5), (-4, -6)]
+    exps = [(-6, -4), (-5, -7), (-7, -5), (-4, -6)] if kw["seed"] != 112 else [(-14, 7), (7, -14)]     # 112: both ends of the range
     p8 = W.to_fp8_pool(p, k_exp=[exps[h % 4][0] for h in range(p.Hkv)], v_exp=[exps[h % 4][1] for h in range(p.Hkv)])
     o, lse, _ = gpu_forward(p8)
     compare(p8, o, lse, strict=False)
