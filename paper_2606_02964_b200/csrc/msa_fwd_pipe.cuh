@@ -189,14 +189,14 @@ __device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t two_codes, uint32_
 
 // The fp8 blocks of one K (or V) tile: staging slot (row-major, D bytes per row, block b at b*16*D) -> the bf16 tile in
 // its ring slot (128-byte swizzle, one 16 KB half per 64 elements, as TMA would have written it).  A warp iteration
-// covers 512 staged bytes (a lane: 16 codes = two 16-byte bf16 chunks); the calling warp takes iterations first,
-// first + stride, ...  Only rows < nvalid of a block are written (the V loader has zeroed the others, K's are masked).
+// covers 512 staged bytes (a lane: 16 codes = two 16-byte bf16 chunks); the calling warp takes the iterations whose bit
+// is set in it_mask.  Only rows < nvalid of a block are written (the V loader has zeroed the others, K's are masked).
 // The two stores of the lanes j and j + 4 of a row go to the same bank group (different 64-element halves): a two-way
 // conflict on the store pipe, which has room; ordering the stores per lane to avoid it costs ten selects per iteration
 // on the ALU pipe, which is what bounds the conversion (measured).
 template <int D>
-__device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uint32_t m_paged, int nvp, uint32_t mul, int first,
-                                                 int stride, int lane)
+__device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uint32_t m_paged, int nvp, uint32_t mul,
+                                                 uint32_t it_mask, int lane)
 {
     constexpr int kLanesPerRow = D / 16, kRowsPerIt = 32 / kLanesPerRow, kItPerBlock = kBlock / kRowsPerIt;
     constexpr int kHalfBytes = kTileM * 128;
@@ -223,24 +223,31 @@ __device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uin
                      : "r"(src0 + static_cast<uint32_t>(row0 * D)));
     };
     const bool all_full = m_paged == 0xffu && __all_sync(0xffffffffu, lane >= kVbPerTile || (nvp & 0xff) == kBlock);
+    it_mask &= (kIters >= 32) ? 0xffffffffu : ((1u << (kIters & 31)) - 1u);
     if (all_full) {
         // the common tile (eight full cached blocks): four loads in flight before the first conversion -- one warp per
         // SM sub-partition converts, and a shared-memory load takes a few hundred cycles next to the tensor core's reads
         constexpr int kBatch = 4;
 #pragma unroll 1
-        for (int it0 = first; it0 < kIters; it0 += kBatch * stride) {
+        while (it_mask != 0) {
             uint32_t w[kBatch][4];
+            int its[kBatch];
+#pragma unroll
+            for (int k = 0; k < kBatch; ++k) {
+                its[k] = it_mask ? __ffs(it_mask) - 1 : -1;
+                it_mask &= it_mask - 1;
+                if (its[k] >= 0) load(its[k], w[k][0], w[k][1], w[k][2], w[k][3]);
+            }
 #pragma unroll
             for (int k = 0; k < kBatch; ++k)
-                if (it0 + k * stride < kIters) load(it0 + k * stride, w[k][0], w[k][1], w[k][2], w[k][3]);
-#pragma unroll
-            for (int k = 0; k < kBatch; ++k)
-                if (it0 + k * stride < kIters) convert_store(it0 + k * stride, w[k][0], w[k][1], w[k][2], w[k][3]);
+                if (its[k] >= 0) convert_store(its[k], w[k][0], w[k][1], w[k][2], w[k][3]);
         }
         return;
     }
 #pragma unroll 1
-    for (int it = first; it < kIters; it += stride) {
+    while (it_mask != 0) {
+        const int it = __ffs(it_mask) - 1;
+        it_mask &= it_mask - 1;
         const int b = it / kItPerBlock;
         const int nv = __shfl_sync(0xffffffffu, nvp, b) & 0xff;
         if (((m_paged >> b) & 1u) && (it % kItPerBlock) * kRowsPerIt + rsub < nv) {
@@ -251,19 +258,38 @@ __device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uin
     }
 }
 
+// Iterations of a tile for converter warp w (0-3) when warp 0 shares its SM sub-partition with the working softmax warps:
+// warp 0 takes iterations 0, 7, 14, 21, 28, the other 27 go to warps 1-3 in turn.
+__device__ __forceinline__ uint32_t kv8_skew_mask(int w)
+{
+    uint32_t m = 0;
+    int k = 0;
+#pragma unroll
+    for (int it = 0; it < 32; ++it) {
+        if (it % 7 == 0) {
+            if (w == 0) m |= 1u << it;
+        } else {
+            if (w == 1 + k % 3) m |= 1u << it;
+            ++k;
+        }
+    }
+    return m;
+}
+
 // KV8 converters (warps 8-11): every ring entry of the unit in ring order; for an entry whose tile holds cached blocks,
-// the calling warp converts iterations first, first + stride, ... of the staged codes into the tile's ring slot
-// (first < 0: nothing) and arrives on the staging slot's "empty" barrier; every warp arrives on the ring slot's "full"
+// the calling warp converts the iterations of its mask (kv8_convert_tile) of the staged codes into the tile's ring slot
+// and arrives on the staging slot's "empty" barrier; every warp arrives on the ring slot's "full"
 // barrier for every entry.  An entry is waited for even when there is nothing to convert: a waiter that skips a use
 // of a slot cannot tell the phases of its barrier apart.
 template <class C, int D>
 __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkUnit &wu, uint32_t bar0, uint32_t sStg, uint32_t sRing,
-                                                 int lane, int first, int stride, uint32_t &cv_ent, uint32_t &cv_stg)
+                                                 int lane, uint32_t it_mask, uint32_t &cv_ent, uint32_t &cv_stg)
 {
     auto bar = [bar0](int i) { return bar0 + static_cast<uint32_t>(i) * 8u; };
     const int n = wu.tile_end - wu.tile_begin;
     const bool pair = wu.mode == kModePair;
     const uint32_t mul_k = __ldg(P.kv8_mul + wu.kvh), mul_v = __ldg(P.kv8_mul + P.Hkv + wu.kvh);
+    PROF_DECL();
     auto fetch_nvp = [&](int e) -> int {             // lane b < 8: nvalid | paged << 8 of virtual block b of entry e's tile
         int r = 0;
         if (e < 2 * n) {
@@ -286,14 +312,24 @@ __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkU
         bool is_v;
         int t;
         kv8_entry(e, n, pair, is_v, t);
-        const uint32_t slot = cv_ent & (C::kStages - 1);
-        mbar_wait(bar(kBarKvEmpty + slot), ((cv_ent / C::kStages) & 1u) ^ 1u);
+        const uint32_t slot = cv_ent % C::kStages;
+        {
+            PROF_T0();
+            mbar_wait(bar(kBarKvEmpty + slot), ((cv_ent / C::kStages) & 1u) ^ 1u);
+            PROF_ADD(21);
+        }
         if (m_paged != 0) {
-            const uint32_t st = cv_stg & static_cast<uint32_t>(C::kStgDiv - 1);
-            mbar_wait(bar(kBarStgFull + st), (cv_stg / C::kStgDiv) & 1u);
-            if (first >= 0)
-                kv8_convert_tile<D>(sStg + st * C::kStgTileBytes, sRing + slot * C::kTileBytes, m_paged, cur, is_v ? mul_v : mul_k,
-                                    first, stride, lane);
+            const uint32_t st = cv_stg % static_cast<uint32_t>(C::kStgDiv);
+            {
+                PROF_T0();
+                mbar_wait(bar(kBarStgFull + st), (cv_stg / C::kStgDiv) & 1u);
+                PROF_ADD(22);
+            }
+            PROF_T0();
+            kv8_convert_tile<D>(sStg + st * C::kStgTileBytes, sRing + slot * C::kTileBytes, m_paged, cur, is_v ? mul_v : mul_k,
+                                it_mask, lane);
+            PROF_ADD(27);
+            PROF_INC(24, 1);
             fence_proxy_async_smem();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(kBarStgEmpty + st));
@@ -304,13 +340,21 @@ __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkU
         ++cv_ent;
         cur = nxt;
     }
+#if defined(MSA_PROF) && MSA_PROF != 2
+#ifndef MSA_PROF_CVWARP
+#define MSA_PROF_CVWARP 8
+#endif
+    if ((threadIdx.x >> 5) == MSA_PROF_CVWARP && lane == 0) {
+        PROF_FLUSH(21, 25);
+        PROF_FLUSH(27, 28);
+    }
+#endif
 }
 
 template <int D, bool KV8, int QT>
 __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_constant__ FwdParams P)
 {
     using C = PipeCfg<D, KV8, QT>;
-    static_assert(!KV8 || (C::kStages & (C::kStages - 1)) == 0, "KV8 ring positions are taken from an entry counter with a mask");
     extern __shared__ __align__(1024) uint8_t smem[];
     const uint32_t sbase = smem_u32(smem);
     const uint32_t sQ = sbase, sRing = sbase + C::kQBytes;
@@ -568,12 +612,13 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             const bool pair = wu.mode == kModePair;
             const int rows_total = wu.n_tok * G;
             if constexpr (KV8) {
-                // ---- converters (kv8_convert_unit): all four warps, unless the unit's valid q rows fit one softmax warp per
-                // chain (token-major packing, short queries) -- those two warps exponentiate on SM sub-partition 0, which warp 8
-                // shares with them, so warps 9-11 take the whole tile and warp 8 only gives its arrivals.
+                // ---- converters (kv8_convert_unit).  Every warp takes every fourth warp iteration of a tile, unless the unit's
+                // valid q rows fit one softmax warp per chain (token-major packing, short queries): those two warps exponentiate
+                // on SM sub-partition 0, which warp 8 shares with them, so warp 8 takes 5 of the 32 iterations and warps 9-11
+                // nine each.
                 const bool one_row_warp = P.token_major && !pair && wu.n_tok * G <= 32;
-                kv8_convert_unit<C, D>(P, wu, bar0, sStg, sRing, lane, one_row_warp ? warp - 9 : warp - 8, one_row_warp ? 3 : 4, cv_ent,
-                                       cv_stg);
+                const uint32_t it_mask = one_row_warp ? kv8_skew_mask(warp - 8) : (0x11111111u << (warp - 8));
+                kv8_convert_unit<C, D>(P, wu, bar0, sStg, sRing, lane, it_mask, cv_ent, cv_stg);
             }
             const int n_out = pair ? 2 : 1;                       // q tiles written by this unit
             for (int qt = 0; qt < n_out; ++qt) {
@@ -685,10 +730,6 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             }
         }
 #if defined(MSA_PROF) && MSA_PROF != 2
-#ifndef MSA_PROF_CVWARP
-#define MSA_PROF_CVWARP 8
-#endif
-        if (warp == MSA_PROF_CVWARP && lane == 0) { PROF_FLUSH(21, 25); PROF_FLUSH(27, 28); }
 #endif
     } else {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
@@ -708,7 +749,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             (void)ent;
             auto observe_until = [&](uint32_t target) {
                 while (ent < target) {
-                    mbar_wait(bar(kBarKvEmpty + (ent & (C::kStages - 1))), ((ent / C::kStages) & 1u) ^ 1u);
+                    mbar_wait(bar(kBarKvEmpty + (ent % C::kStages)), ((ent / C::kStages) & 1u) ^ 1u);
                     ++ent;
                 }
             };
@@ -790,7 +831,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     uint32_t slot = rp.slot, phase = rp.phase;
                     if constexpr (KV8) {
                         observe_until(ent_base + static_cast<uint32_t>(which ? kv8_entry_of_v(j, n, pair_u) : kv8_entry_of_k(j, pair_u)));
-                        slot = ent & (C::kStages - 1);
+                        slot = ent % C::kStages;
                         phase = ((ent / C::kStages) & 1u) ^ 1u;
                         ++ent;
                     }
@@ -886,7 +927,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             (void)ment;
             auto take_k = [&]() -> uint32_t {
                 if constexpr (KV8) {
-                    const uint32_t slot = ment & (C::kStages - 1);
+                    const uint32_t slot = ment % C::kStages;
                     PROF_T0();
                     mbar_wait(bar(kBarKvFull + slot), (ment / C::kStages) & 1u);
                     PROF_ADD(8);
@@ -903,7 +944,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             };
             auto take_v = [&]() -> uint32_t {
                 if constexpr (KV8) {
-                    const uint32_t slot = ment & (C::kStages - 1);
+                    const uint32_t slot = ment % C::kStages;
                     PROF_T0();
                     mbar_wait(bar(kBarKvFull + slot), (ment / C::kStages) & 1u);
                     PROF_ADD(9);
@@ -1111,7 +1152,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                         int t;
                         kv8_entry(e, n, pair_u, is_v, t);
                         const CUtensorMap *tm = is_v ? P.tm_pool_v : P.tm_pool_k;
-                        const uint32_t st = stg & static_cast<uint32_t>(C::kStgDiv - 1);
+                        const uint32_t st = stg % static_cast<uint32_t>(C::kStgDiv);
                         const uint32_t rows = __reduce_add_sync(0xffffffffu, static_cast<uint32_t>(nv));
                         {
                             PROF_T0();
