@@ -295,7 +295,8 @@ def run_mine(args, rank: int, world: int, local_rank: int):
             # the other three performance configs of BASELINE.json, each with its own roofline block and clocks
             del p
             line["secondary"] = []
-            for wl, k in (("cfg5_short_query", 50), ("cfg3_70b_long", 30), ("cfg4_mixed", 20)):
+            # ... and configs[4] again with the cached blocks stored as fp8 E4M3 codes (GB/s on the fp8 bytes)
+            for wl, k in (("cfg5_short_query", 50), ("cfg3_70b_long", 30), ("cfg4_mixed", 20), ("cfg5_short_query_kv8", 30)):
                 torch.cuda.empty_cache()
                 time.sleep(2.0)            # each workload starts from an idle chip, not from the last one's power state
                 sec, psec = bench_workload(wl, max(10, min(args.steps, k)), args.warmup, do_e2e=False)
@@ -303,7 +304,8 @@ def run_mine(args, rank: int, world: int, local_rank: int):
                                               ms_per_step=sec["ms_per_step"], gpu_launches=sec["gpu_launches"],
                                               roofline=sec["roofline"], clocks=sec["clocks"], plan=sec["plan"],
                                               config=dict(requests=psec.n_req, total_q=psec.total_q, kv_tokens=psec.kv_tokens(),
-                                                          Hq=psec.Hq, Hkv=psec.Hkv, head_dim=psec.D)))
+                                                          Hq=psec.Hq, Hkv=psec.Hkv, head_dim=psec.D,
+                                                          pool_format="fp8_e4m3" if psec.k_scale is not None else "bf16")))
                 del psec
             line["config"]["largest_single_gpu_config"] = "cfg4_mixed (in `secondary`; `value` is quoted on cfg2_llama8b = BASELINE.json configs[1])"
     if world > 1:
