@@ -70,7 +70,11 @@ enum { MSA_SEG_PAGED = 0, MSA_SEG_CONTIG = 1, MSA_SEG_SELF = 2 };
  *                          K_j[kvh][d] = e4m3(pool_k byte) * k_scale[kvh],   V_j[kvh][d] = e4m3(pool_v byte) * v_scale[kvh]
  *                      The scales must be powers of two in [2^-14, 2^7] (as in the OCP MX formats): the dequantised
  *                      value is then exactly a bf16, the kernel converts the codes on chip and the result is the bf16
- *                      path's result on the dequantised pool -- same tolerances.  A NaN code dequantises to an
+ *                      path's result on the dequantised pool -- same tolerances.  A launch of short queries reads every
+ *                      cached byte once and converts it in the forward kernel; a launch with prefill chunks, which loads
+ *                      a cached tile once per q-tile group, first dequantises the blocks it refers to into the workspace
+ *                      (once) and runs the bf16 kernel on that copy -- decided by the plan (msa_workspace_bytes grows
+ *                      accordingly), invisible in the results.  A NaN code dequantises to an
  *                      unspecified finite value (non-finite K/V are outside the definition, DESIGN.md c19). */
 enum { MSA_POOL_BF16 = 0, MSA_POOL_FP8_E4M3 = 1 };
 
@@ -152,10 +156,13 @@ int msa_plan_get_info(msa_plan p, msa_plan_info *info);
  *           2  cta_unit_begin      int32     [num_ctas + 1]
  *           3  merge items         {int32 q_row0, n_tok, kvh, n_partials; int64 first_off, stride}
  *           4  tile mask summaries int32[2]  {max_abs, ragged} per context KV tile
+ *           7  fp8 pool: block-table indices the dequantising pre-pass converts (int32; empty when the forward kernel
+ *              converts the codes itself)
  * With buf == NULL only *bytes is set; otherwise *bytes is the capacity on entry. */
 int msa_plan_export(msa_plan p, int which, void *buf, size_t *bytes);
 
-/* Bytes of device scratch msa_forward needs for this plan (split-KV partials); may be 0. */
+/* Bytes of device scratch msa_forward needs for this plan (split-KV partials; on an fp8 handle also the bf16 copy of the
+ * cached blocks of a launch that loads them several times, see MSA_POOL_FP8_E4M3); may be 0. */
 int msa_workspace_bytes(msa_plan p, size_t *bytes);
 
 /* One MSA forward pass, asynchronous on `cuda_stream` (a cudaStream_t; NULL = default

@@ -208,6 +208,7 @@ _EXPORT_DTYPES = {
     4: np.dtype([("max_abs", "<i4"), ("ragged", "<i4")]),
     5: np.dtype("<i4"),
     6: np.dtype("<i4"),
+    7: np.dtype("<i4"),
 }
 
 

@@ -95,10 +95,11 @@ struct msa_handle_s {
     struct MapKey {
         const void *q, *pool_k, *pool_v, *contig_k, *contig_v;
         int64_t total_q, num_blocks, contig_rows;
+        bool pool_fp8;
         bool operator==(const MapKey &o) const
         {
             return q == o.q && pool_k == o.pool_k && pool_v == o.pool_v && contig_k == o.contig_k && contig_v == o.contig_v &&
-                   total_q == o.total_q && num_blocks == o.num_blocks && contig_rows == o.contig_rows;
+                   total_q == o.total_q && num_blocks == o.num_blocks && contig_rows == o.contig_rows && pool_fp8 == o.pool_fp8;
         }
     };
     struct MapEntry { MapKey key; FwdParams maps; uint64_t stamp; };
@@ -124,6 +125,14 @@ struct msa_plan_s {
     const TileInfo *d_tile_info = nullptr;
     const int32_t *d_vb_dst = nullptr;     // write-back plans only
     const int32_t *d_tile_writer = nullptr;
+    // fp8 pool, plans with pair-mode units: the cached blocks are dequantised once into the workspace (msa_dequant.cu)
+    bool deq = false;
+    bool any_pair = false;                 // the plan has pair-mode units (which shared-memory layout the fp8 variant needs)
+    std::vector<int32_t> deq_src;          // distinct block-table indices the plan refers to; block j of the copy <- deq_src[j]
+    std::vector<VBlock> vblocks_deq;       // the plan's virtual blocks with src = index into the copy
+    const int32_t *d_deq_src = nullptr;
+    const VBlock *d_vblocks_deq = nullptr;
+    size_t ws_partials = 0, ws_pool = 0, ws_ident = 0;     // workspace layout in bytes: [partials | copy of K | copy of V | identity table]
 };
 
 struct msa_append_plan_s {
@@ -324,6 +333,44 @@ int plan_create(msa_handle h, const msa_request *requests, int32_t n_req, const 
         delete p;
         return rc;
     }
+    {
+        const HostPlan &hp = p->hp;
+        p->ws_partials = static_cast<size_t>(hp.workspace_floats) * sizeof(float);
+        bool any_pair = false;
+        for (const WorkUnit &wu : hp.units) any_pair = any_pair || (wu.mode == kModePair && wu.tile_end > wu.tile_begin);
+        p->any_pair = any_pair;
+        if (h->kv8 && any_pair && hp.uses_paged) {
+            // Dequantising pre-pass (msa_dequant.cu): in a prefill launch a cached tile is loaded by every q-tile group of its
+            // (run, KV head), and converting it in the forward kernel repeats the conversion as often.  It pays when the cached
+            // blocks are loaded kDeqMinReuse times or more on average: the pre-pass moves 3 bytes per element once and the
+            // forward kernel then reads 2 instead of 1 per load.  Compact, sorted list of the block-table entries referred to.
+            for (const VBlock &vb : hp.vblocks)
+                if (vb.paged && vb.nvalid > 0) p->deq_src.push_back(vb.src);
+            std::sort(p->deq_src.begin(), p->deq_src.end());
+            p->deq_src.erase(std::unique(p->deq_src.begin(), p->deq_src.end()), p->deq_src.end());
+            int64_t loads = 0;                 // (cached 16-token block, KV head) pairs loaded by the launch, over all units
+            for (const WorkUnit &wu : hp.units)
+                for (int t = wu.tile_begin; t < wu.tile_end; ++t)
+                    for (int b = 0; b < kVbPerTile; ++b) {
+                        const int i = t * kVbPerTile + b;
+                        if (i < wu.vb_count && hp.vblocks[wu.vb_begin + i].paged && hp.vblocks[wu.vb_begin + i].nvalid > 0) ++loads;
+                    }
+            constexpr double kDeqMinReuse = 2.0;
+            p->deq = !p->deq_src.empty() &&
+                     static_cast<double>(loads) >= kDeqMinReuse * static_cast<double>(p->deq_src.size()) * h->cfg.num_kv_heads;
+            if (!p->deq) p->deq_src.clear();
+        }
+        if (p->deq) {
+            p->vblocks_deq = hp.vblocks;
+            for (VBlock &vb : p->vblocks_deq)
+                if (vb.paged && vb.nvalid > 0)
+                    vb.src = static_cast<int32_t>(std::lower_bound(p->deq_src.begin(), p->deq_src.end(), vb.src) - p->deq_src.begin());
+            auto al1k = [](size_t x) { return (x + 1023) & ~static_cast<size_t>(1023); };
+            p->ws_partials = al1k(p->ws_partials);
+            p->ws_pool = al1k(p->deq_src.size() * static_cast<size_t>(MSA_BLOCK_SIZE) * h->cfg.num_kv_heads * h->cfg.head_dim * 2);
+            p->ws_ident = al1k(p->deq_src.size() * sizeof(int32_t));
+        }
+    }
     if (!h->planning_only) {
         const HostPlan &hp = p->hp;
         auto al = [](size_t x) { return (x + 255) & ~static_cast<size_t>(255); };
@@ -334,7 +381,9 @@ int plan_create(msa_handle h, const msa_request *requests, int32_t n_req, const 
         const size_t b_ti = al(hp.tile_info.size() * sizeof(TileInfo));
         const size_t b_wb = al(hp.vb_dst.size() * sizeof(int32_t));
         const size_t b_tw = al(hp.tile_writer.size() * sizeof(int32_t));
-        const size_t total = b_vb + b_un + b_cb + b_mg + b_ti + b_wb + b_tw + 256;
+        const size_t b_ds = al(p->deq_src.size() * sizeof(int32_t));
+        const size_t b_vd = al(p->vblocks_deq.size() * sizeof(VBlock));
+        const size_t total = b_vb + b_un + b_cb + b_mg + b_ti + b_wb + b_tw + b_ds + b_vd + 256;
         DeviceGuard guard(h->cfg.device);
         cudaError_t e = guard.err;
         if (e == cudaSuccess) e = cudaMalloc(&p->d_buf, total);
@@ -371,6 +420,15 @@ int plan_create(msa_handle h, const msa_request *requests, int32_t n_req, const 
         if (e == cudaSuccess && !hp.tile_writer.empty())
             e = cudaMemcpy(base + b_vb + b_un + b_cb + b_mg + b_ti + b_wb, hp.tile_writer.data(), hp.tile_writer.size() * sizeof(int32_t),
                            cudaMemcpyHostToDevice);
+        if (p->deq) {
+            char *ds = base + b_vb + b_un + b_cb + b_mg + b_ti + b_wb + b_tw;
+            p->d_deq_src = reinterpret_cast<const int32_t *>(ds);
+            p->d_vblocks_deq = reinterpret_cast<const VBlock *>(ds + b_ds);
+            if (e == cudaSuccess && !p->deq_src.empty())
+                e = cudaMemcpy(ds, p->deq_src.data(), p->deq_src.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+            if (e == cudaSuccess && !p->vblocks_deq.empty())
+                e = cudaMemcpy(ds + b_ds, p->vblocks_deq.data(), p->vblocks_deq.size() * sizeof(VBlock), cudaMemcpyHostToDevice);
+        }
         if (e != cudaSuccess) {
             cudaFree(p->d_buf);
             delete p;
@@ -405,7 +463,7 @@ int msa_plan_get_info(msa_plan p, msa_plan_info *info)
 int msa_workspace_bytes(msa_plan p, size_t *bytes)
 {
     if (!p || !bytes) return MSA_ERR_INVALID_ARG;
-    *bytes = static_cast<size_t>(p->hp.workspace_floats) * sizeof(float);
+    *bytes = p->ws_partials + 2 * p->ws_pool + p->ws_ident;
     return MSA_OK;
 }
 
@@ -413,7 +471,8 @@ int msa_workspace_bytes(msa_plan p, size_t *bytes)
  * which: 0 = virtual blocks (int32 x4 each), 1 = work units (int32 x12 each),
  *        2 = cta_unit_begin (int32), 3 = merge items (int32 x4 + int64 x2 each),
  *        4 = per-tile mask summaries (int32 x2 each), 5 / 6 = write-back plans: destination block-table index per
- *        virtual block, q_row0 of the storing work item per context KV tile (int32 each).
+ *        virtual block, q_row0 of the storing work item per context KV tile (int32 each); 7 = fp8 pool: the block-table
+ *        indices the dequantising pre-pass converts (int32 each; empty when the forward kernel converts the codes itself).
  * Call with buf == NULL to get the byte size. */
 int msa_plan_export(msa_plan p, int which, void *buf, size_t *bytes)
 {
@@ -428,6 +487,7 @@ int msa_plan_export(msa_plan p, int which, void *buf, size_t *bytes)
     case 4: src = p->hp.tile_info.data(); n = p->hp.tile_info.size() * sizeof(TileInfo); break;
     case 5: src = p->hp.vb_dst.data(); n = p->hp.vb_dst.size() * sizeof(int32_t); break;
     case 6: src = p->hp.tile_writer.data(); n = p->hp.tile_writer.size() * sizeof(int32_t); break;
+    case 7: src = p->deq_src.data(); n = p->deq_src.size() * sizeof(int32_t); break;
     default: return MSA_ERR_INVALID_ARG;
     }
     if (buf) {
@@ -486,16 +546,16 @@ bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) ==
 constexpr size_t kMapCacheEntries = 64;
 
 // The 23 tensor maps of one (q, pool, arena) pointer set, encoded once and kept in the handle.
-int cached_tensor_maps(msa_handle h, const HostPlan &hp_in, bool writeback, const void *q, int64_t total_q, const void *pool_k,
-                       const void *pool_v, int64_t num_blocks, const void *contig_k, const void *contig_v, int64_t contig_rows,
-                       FwdParams *out)
+int cached_tensor_maps(msa_handle h, const HostPlan &hp_in, bool writeback, bool pool_fp8, const void *q, int64_t total_q,
+                       const void *pool_k, const void *pool_v, int64_t num_blocks, const void *contig_k, const void *contig_v,
+                       int64_t contig_rows, FwdParams *out)
 {
     const int Hq = h->cfg.num_q_heads, Hkv = h->cfg.num_kv_heads, D = h->cfg.head_dim;
     struct { bool uses_paged, uses_contig; } hp{hp_in.uses_paged || writeback, hp_in.uses_contig};   // write-back stores through the pool maps
     // a plan that uses no paged (or no contiguous) segment never dereferences those maps: they are encoded over q
     msa_handle_s::MapKey key{q, hp.uses_paged ? pool_k : nullptr, hp.uses_paged ? pool_v : nullptr,
                              hp.uses_contig ? contig_k : nullptr, hp.uses_contig ? contig_v : nullptr,
-                             total_q, hp.uses_paged ? num_blocks : 0, hp.uses_contig ? contig_rows : 0};
+                             total_q, hp.uses_paged ? num_blocks : 0, hp.uses_contig ? contig_rows : 0, pool_fp8};
     ++h->map_stamp;
     for (auto &e : h->map_cache)
         if (e.key == key) {
@@ -527,7 +587,7 @@ int cached_tensor_maps(msa_handle h, const HostPlan &hp_in, bool writeback, cons
     const uint64_t prow = hp.uses_paged ? static_cast<uint64_t>(num_blocks) * MSA_BLOCK_SIZE : static_cast<uint64_t>(total_q);
     const uint64_t pin = hp.uses_paged ? static_cast<uint64_t>(Hkv) * D : static_cast<uint64_t>(Hq) * D;
     for (int i = 0; i < 5; ++i) {
-        if (h->kv8 && hp.uses_paged) {
+        if (pool_fp8 && hp.uses_paged) {
             if ((rc = encode_2d_u8(h, &fp.tm_pool_k[i], pk, pin, prow, D, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
             if ((rc = encode_2d_u8(h, &fp.tm_pool_v[i], pv, pin, prow, D, MSA_BLOCK_SIZE >> i)) != MSA_OK) return rc;
             continue;
@@ -588,7 +648,7 @@ int forward_impl(msa_handle h, msa_plan p, const void *q, int64_t total_q, const
     if (!aligned16(q) || !aligned16(o) || !aligned16(pool_k) || !aligned16(pool_v) || !aligned16(contig_k) ||
         !aligned16(contig_v) || (reinterpret_cast<uintptr_t>(lse) & 3u) || (reinterpret_cast<uintptr_t>(block_table) & 3u))
         return MSA_ERR_MISALIGNED;
-    const size_t need = static_cast<size_t>(hp.workspace_floats) * sizeof(float);
+    const size_t need = p->ws_partials + 2 * p->ws_pool + p->ws_ident;
     if (need > 0) {
         if (!workspace || workspace_bytes < need) return MSA_ERR_WORKSPACE;
         if (!aligned16(workspace)) return MSA_ERR_MISALIGNED;
@@ -597,14 +657,22 @@ int forward_impl(msa_handle h, msa_plan p, const void *q, int64_t total_q, const
     const int Hq = h->cfg.num_q_heads, Hkv = h->cfg.num_kv_heads, D = h->cfg.head_dim;
     DeviceGuard guard(h->cfg.device);      // the caller's current device may be another one
     if (guard.err != cudaSuccess) return cuda_fail(guard.err, "msa_forward: cudaSetDevice");
+    // fp8 pool and prefill units: the cached blocks are dequantised once into the workspace, the bf16 kernel runs on that copy
+    char *ws = static_cast<char *>(workspace);
+    void *copy_k = p->deq ? ws + p->ws_partials : nullptr, *copy_v = p->deq ? ws + p->ws_partials + p->ws_pool : nullptr;
+    int32_t *ident = p->deq ? reinterpret_cast<int32_t *>(ws + p->ws_partials + 2 * p->ws_pool) : nullptr;
+    const bool pool_fp8 = h->kv8 && !p->deq;
     FwdParams fp;
-    int rc = cached_tensor_maps(h, hp, writeback, q, total_q, pool_k, pool_v, num_blocks, contig_k, contig_v, contig_rows, &fp);
+    int rc = p->deq ? cached_tensor_maps(h, hp, false, false, q, total_q, copy_k, copy_v, static_cast<int64_t>(p->deq_src.size()), contig_k,
+                                         contig_v, contig_rows, &fp)
+                    : cached_tensor_maps(h, hp, writeback, pool_fp8, q, total_q, pool_k, pool_v, num_blocks, contig_k, contig_v,
+                                         contig_rows, &fp);
     if (rc != MSA_OK) return rc;
-    fp.vblocks = p->d_vblocks;
+    fp.vblocks = p->deq ? p->d_vblocks_deq : p->d_vblocks;
     fp.units = p->d_units;
     fp.cta_unit_begin = p->d_cta_begin;
     fp.tile_info = p->d_tile_info;
-    fp.block_table = block_table;
+    fp.block_table = p->deq ? ident : block_table;
     fp.vb_dst = writeback ? p->d_vb_dst : nullptr;
     fp.tile_writer = writeback ? p->d_tile_writer : nullptr;
     fp.kv_to_q = h->d_kv_to_q;
@@ -622,11 +690,26 @@ int forward_impl(msa_handle h, msa_plan p, const void *q, int64_t total_q, const
     const bool rec = h->timing && static_cast<size_t>(h->ev_steps) * 3 + 3 <= h->ev.size();
     cudaEvent_t *ev = rec ? &h->ev[static_cast<size_t>(h->ev_steps) * 3] : nullptr;
     if (rec) MSA_CUDA(cudaEventRecord(ev[0], stream));
-    bool any_pair = false;
-    for (const WorkUnit &wu : hp.units) any_pair = any_pair || (wu.mode == kModePair && wu.tile_end > wu.tile_begin);
-    MSA_CUDA(launch_fwd(fp, D, h->kv8, !any_pair, hp.info.num_ctas, stream));
+    int launches = 0;
+    if (p->deq) {
+        DequantParams dq;
+        dq.src_bt = p->d_deq_src;
+        dq.block_table = block_table;
+        dq.pool_k = pool_k;
+        dq.pool_v = pool_v;
+        dq.out_k = copy_k;
+        dq.out_v = copy_v;
+        dq.ident = ident;
+        dq.kv8_mul = h->d_kv8_mul;
+        dq.n_blocks = static_cast<int32_t>(p->deq_src.size());
+        dq.Hkv = Hkv;
+        dq.D = D;
+        MSA_CUDA(launch_dequant(dq, h->num_sms, stream));
+        ++launches;
+    }
+    MSA_CUDA(launch_fwd(fp, D, pool_fp8, !p->any_pair, hp.info.num_ctas, stream));
     if (rec) MSA_CUDA(cudaEventRecord(ev[1], stream));
-    h->last_launches = 1;
+    h->last_launches = ++launches;
     if (!hp.merge_items.empty()) {
         MergeParams mp;
         mp.items = p->d_merge;
@@ -640,7 +723,7 @@ int forward_impl(msa_handle h, msa_plan p, const void *q, int64_t total_q, const
         int max_rows = 0;
         for (const MergeItem &mi : hp.merge_items) max_rows = std::max(max_rows, mi.n_tok * h->G);
         MSA_CUDA(launch_merge(mp, static_cast<int>(hp.merge_items.size()), max_rows, stream));
-        h->last_launches = 2;
+        h->last_launches = ++launches;
     }
     if (rec) {
         MSA_CUDA(cudaEventRecord(ev[2], stream));
@@ -687,7 +770,7 @@ int msa_forward_host(msa_handle h, msa_plan p, const void *q_host, int64_t total
     const size_t b_lse = static_cast<size_t>(total_q) * Hq * 4;
     const size_t b_c = static_cast<size_t>(contig_rows) * Hkv * D * 2;
     const size_t b_bt = static_cast<size_t>(block_table_len) * 4;
-    const size_t b_ws = static_cast<size_t>(p->hp.workspace_floats) * 4;
+    const size_t b_ws = p->ws_partials + 2 * p->ws_pool + p->ws_ident;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     DeviceGuard guard(h->cfg.device);
     if (guard.err != cudaSuccess) return cuda_fail(guard.err, "msa_forward_host: cudaSetDevice");

@@ -17,17 +17,20 @@ static void launch_one(const FwdParams &p, int num_ctas, cudaStream_t stream)
 }
 
 // The kernel needs more dynamic shared memory than the default limit; the attribute is per device and
-// per function, so the handle sets it once for its own device (msa_create).  kv8: the fp8-pool variants
-// (two shared-memory layouts: with room for the two Q tiles of pair-mode units, or -- short queries only --
-// for one Q tile and a deeper staging ring).
+// per function, so the handle sets it once for its own device (msa_create).  A handle with an fp8 pool uses three
+// kernels: the fp8 variant in its two shared-memory layouts (room for the two Q tiles of pair-mode units, or -- short
+// queries only -- one Q tile and a deeper staging ring), and the bf16 kernel behind the dequantising pre-pass for
+// launches that load their cached tiles several times (msa_dequant.cu).
 cudaError_t configure_fwd(int head_dim, bool kv8)
 {
-    if (!kv8) return head_dim == 128 ? configure_one<128, false, 2>() : configure_one<64, false, 2>();
-    cudaError_t e = head_dim == 128 ? configure_one<128, true, 2>() : configure_one<64, true, 2>();
+    cudaError_t e = head_dim == 128 ? configure_one<128, false, 2>() : configure_one<64, false, 2>();
+    if (e != cudaSuccess || !kv8) return e;
+    e = head_dim == 128 ? configure_one<128, true, 2>() : configure_one<64, true, 2>();
     if (e != cudaSuccess) return e;
     return head_dim == 128 ? configure_one<128, true, 1>() : configure_one<64, true, 1>();
 }
 
+// kv8: the pool tensor maps are over E4M3 codes; one_q_tile: the plan has no pair-mode unit
 cudaError_t launch_fwd(const FwdParams &p, int head_dim, bool kv8, bool one_q_tile, int num_ctas, cudaStream_t stream)
 {
     if (num_ctas <= 0) return cudaSuccess;

@@ -65,6 +65,18 @@ struct AppendParams {
     int32_t Hkv, D;
 };
 
+// fp8 pool, dequantising pre-pass (msa_dequant.cu): block j of the bf16 copy = pool block block_table[src_bt[j]]
+struct DequantParams {
+    const int32_t *src_bt;        // [n_blocks] block-table indices, distinct
+    const int32_t *block_table;
+    const void *pool_k, *pool_v;  // E4M3 codes [num_blocks][16][Hkv][D]
+    void *out_k, *out_v;          // bf16 [n_blocks][16][Hkv][D]
+    int32_t *ident;               // [n_blocks], written 0, 1, 2, ...: the block table of the copy
+    const uint32_t *kv8_mul;      // as in FwdParams
+    int32_t n_blocks, Hkv, D;
+};
+cudaError_t launch_dequant(const DequantParams &p, int num_sms, cudaStream_t stream);
+
 cudaError_t configure_append();   // per device, like configure_fwd
 cudaError_t launch_append(const AppendParams &p, int num_sms, cudaStream_t stream);
 
@@ -72,7 +84,7 @@ cudaError_t launch_append(const AppendParams &p, int num_sms, cudaStream_t strea
 // shared-memory limit on the CURRENT device (once per device and head dim); launch_fwd assumes it was done.
 constexpr int kTilesPerGroup = 2;    // q tiles (of 128 packed rows) one work item covers in pair mode
 cudaError_t configure_fwd(int head_dim, bool kv8);
-// one_q_tile (fp8 pool only): the plan has no pair-mode unit, so the layout with one Q tile and the deeper staging ring serves it
+// kv8: the pool tensor maps are over E4M3 codes (the fp8 variant converts them); one_q_tile: the plan has no pair-mode unit
 cudaError_t launch_fwd(const FwdParams &p, int head_dim, bool kv8, bool one_q_tile, int num_ctas, cudaStream_t stream);
 cudaError_t launch_merge(const MergeParams &p, int n_items, int max_rows, cudaStream_t stream);
 

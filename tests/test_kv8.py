@@ -49,6 +49,52 @@ def test_fused_writeback_is_refused_on_an_fp8_pool():
     msa_destroy(h)
 
 
+def _kv8_path(p, device=-1):
+    """Which way an fp8 handle would serve this batch: 'prepass' (cached blocks dequantised once, bf16 kernel), 'kernel_pair'
+    or 'kernel_split' (codes converted inside the forward kernel, layout with two / one Q tiles)."""
+    from paper_2606_02964_b200 import msa_plan_create, msa_plan_destroy, msa_workspace_bytes
+    h = msa_create(p.Hq, p.Hkv, p.D, p.q_to_kv, device=device, pool_format=MSA_POOL_FP8_E4M3)
+    R, n_req, S, n_seg = make_descriptors(p.req, p.seg_kind, p.seg_abs_start, p.seg_len, p.seg_block_off, p.seg_row_off)
+    pl = msa_plan_create(h, R, n_req, S, n_seg)
+    deq = msa_plan_export(pl, 7)
+    units = msa_plan_export(pl, 1)
+    ws = msa_workspace_bytes(pl)
+    msa_plan_destroy(pl)
+    msa_destroy(h)
+    pair = bool(((units["mode"] == 0) & (units["tile_end"] > units["tile_begin"])).any())
+    return ("prepass" if len(deq) else "kernel_pair" if pair else "kernel_split"), deq, ws
+
+
+def _three_paths(device="cpu"):
+    mk = lambda name, ctx, q0, T: build_problem(name, 8, 2, 128, [ContextSpec(ctx + [(SEG_SELF, q0, T)])], [RunSpec(0, q0, T)], seed=21,
+                                                device=device)
+    return dict(prepass=mk("reuse5", [(SEG_PAGED, 0, 500), (SEG_CONTIG, 500, 100)], 600, 300),      # five q-tile groups load every cached tile
+                kernel_pair=mk("reuse1", [(SEG_PAGED, 0, 500), (SEG_CONTIG, 500, 100)], 600, 64),    # one group: converted in the kernel
+                kernel_split=mk("short", [(SEG_PAGED, 0, 500), (SEG_CONTIG, 500, 100)], 600, 4))
+
+
+def test_plan_chooses_prepass_by_reuse_of_the_cached_blocks():
+    for want, p in _three_paths().items():
+        path, deq, ws = _kv8_path(p)
+        assert path == want, (want, path)
+        if want == "prepass":
+            # 500 cached tokens = 32 blocks, each listed once, in block-table order; the workspace holds their bf16 copy
+            assert np.array_equal(deq, np.arange(32, dtype=np.int32))
+            assert ws >= 2 * 32 * 16 * p.Hkv * p.D * 2
+        else:
+            # nothing but the split-KV partials a bf16 handle needs too
+            from paper_2606_02964_b200 import msa_plan_create, msa_plan_destroy, msa_workspace_bytes
+            hb = msa_create(p.Hq, p.Hkv, p.D, device=-1)
+            R, n_req, S, n_seg = make_descriptors(p.req, p.seg_kind, p.seg_abs_start, p.seg_len, p.seg_block_off, p.seg_row_off)
+            pl = msa_plan_create(hb, R, n_req, S, n_seg)
+            assert ws == msa_workspace_bytes(pl)
+            msa_plan_destroy(pl)
+            msa_destroy(hb)
+    # cfg2 loads every cached tile eight times, cfg5 once
+    assert _kv8_path(W.cfg2_llama8b(layout_only=True))[0] == "prepass"
+    assert _kv8_path(W.cfg5_short_query(layout_only=True))[0] == "kernel_split"
+
+
 def test_quantiser_oracle_against_torch_and_closed_forms():
     rng = np.random.default_rng(11)
     x = np.concatenate([rng.standard_normal(4000) * 3, rng.uniform(-448, 448, 2000), rng.standard_normal(500) * 1e-3,
@@ -134,6 +180,19 @@ def test_kv8_random_small_problems_against_the_oracle_and_the_bf16_kernel(kw):
     o, lse, _ = gpu_forward(p8)
     compare(p8, o, lse, strict=False)
     # code * 2^k is exactly a bf16 and the conversion happens before the same MMAs: bit-identical to the bf16 kernel
+    o2, lse2, _ = gpu_forward(_dequantised_twin(p8))
+    assert np.array_equal(o, o2) and np.array_equal(lse, lse2)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("want", ["prepass", "kernel_pair", "kernel_split"])
+def test_kv8_each_path_against_the_oracle_and_the_bf16_kernel(want):
+    """The three ways an fp8 handle serves a batch (dequantising pre-pass + bf16 kernel; conversion in the kernel with two / one
+    Q tiles) on the same context: each against the oracle, each bit-identical to the bf16 kernel on the dequantised pool."""
+    p8 = W.to_fp8_pool(_three_paths(DEV)[want], k_exp=[-6, -4], v_exp=[-5, -7])
+    assert _kv8_path(p8, device=0)[0] == want
+    o, lse, _ = gpu_forward(p8)
+    compare(p8, o, lse, strict=False)
     o2, lse2, _ = gpu_forward(_dequantised_twin(p8))
     assert np.array_equal(o, o2) and np.array_equal(lse, lse2)
 
