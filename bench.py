@@ -120,7 +120,7 @@ class ClockSampler:
 
 
 def oracle_sample(p, n_rows: int, seed: int, reqs=None):
-    """Time the fp64 oracle, as it stands, on a bounded row sample.  Returns (seconds, flops, pairs)."""
+    """Time the fp64 oracle, as it stands, on a bounded row sample.  Returns (seconds, flops, K/V bytes of the visible keys, rows)."""
     import oracle
     rng = np.random.default_rng(seed)
     if reqs is None:
@@ -135,15 +135,18 @@ def oracle_sample(p, n_rows: int, seed: int, reqs=None):
     rr, ii = np.asarray(rr, np.int32), np.asarray(ii, np.int32)
     arrays = p.host_arrays(reqs=reqs)
     pairs = 0
+    kv_bytes = 0              # K and V bytes of the visible keys (all KV heads): one byte per cached element of an fp8 pool
     for r, i in zip(rr, ii):
         pos = int(p.req[r, 2]) + int(i)
         sb, sc = int(p.req[r, 3]), int(p.req[r, 4])
         for s in range(sb, sb + sc):
-            pairs += int(np.clip(pos - int(p.seg_abs_start[s]) + 1, 0, int(p.seg_len[s])))
+            vis = int(np.clip(pos - int(p.seg_abs_start[s]) + 1, 0, int(p.seg_len[s])))
+            pairs += vis
+            kv_bytes += vis * p.Hkv * p.D * 2 * (1 if (p.k_scale is not None and int(p.seg_kind[s]) == 0) else 2)
     t0 = time.perf_counter()
     oracle.forward(arrays, p.Hq, p.Hkv, p.D, p.scale, rr, ii)
     dt = time.perf_counter() - t0
-    return dt, 4.0 * p.D * p.Hq * pairs, pairs, len(rr)
+    return dt, 4.0 * p.D * p.Hq * pairs, kv_bytes, len(rr)
 
 
 def dist_max(value: float, device="cpu") -> float:
@@ -287,7 +290,7 @@ def run_mine(args, rank: int, world: int, local_rank: int):
         if unit == "TFLOP/s":
             cv = fl / dt / 1e12
         else:
-            cv = pairs * p.Hkv * p.D * 2 * 2 / dt / 1e9     # K and V bytes of the visible keys, per kv head
+            cv = pairs / dt / 1e9                            # K and V bytes of the visible keys
         line["cpu_baseline"] = dict(value=cv, unit=unit, cores=oracle.num_threads(), kind="oracle",
                                     sample=f"{n} query rows of requests {reqs} (all {p.Hq} heads), {dt:.2f} s",
                                     seconds=dt)
@@ -674,7 +677,7 @@ def run_reference(args, rank: int, world: int):
     if bound == "tensor":
         value = f_sum / t_sum / 1e12
     else:
-        value = p_sum * p.Hkv * p.D * 2 * 2 / t_sum / 1e9      # K and V bytes of the visible keys, per kv head
+        value = p_sum / t_sum / 1e9                            # K and V bytes of the visible keys
     sample = f"{n_sum // max(1, args.steps)} query rows per step of requests {reqs} (all {p.Hq} heads)"
     line = dict(impl="reference", metric=metric, value=value, unit=unit, n_gpus=world, steps=args.steps,
                 warmup=args.warmup, ms_per_step=1e3 * t_sum / max(1, args.steps), higher_is_better=True,
