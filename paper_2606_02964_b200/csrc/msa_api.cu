@@ -88,7 +88,8 @@ struct msa_handle_s {
     bool kv8 = false;                  // fp8 (E4M3) paged pool
     std::vector<float> kv_scale;       // kv8: [2][Hkv] K scales then V scales (powers of two)
     uint32_t *d_kv8_mul = nullptr;     // kv8: [2][Hkv] f16 bits of 2^k (forward kernel)
-    float *d_kv8_inv = nullptr;        // kv8: [2][Hkv] 1 / scale (quantising msa_kv_append)
+    float *d_kv8_inv = nullptr;        // kv8: [2][Hkv] 1 / scale (quantising msa_kv_append; f16 short-query variant)
+    float *d_kv8_scale = nullptr;      // kv8: [2][Hkv] the scales
     EncodeTiledFn encode = nullptr;
     // Tensor maps depend only on (base pointer, extent) of q / pool / arena: a model calls msa_forward once per
     // layer with the same few pointer sets step after step, so the 23 encoded maps are kept per pointer set.
@@ -252,6 +253,8 @@ int msa_create(const msa_config *cfg, msa_handle *out)
     if (kv8) {
         if (e == cudaSuccess) e = cudaMalloc(&h->d_kv8_mul, kv8_mul.size() * sizeof(uint32_t));
         if (e == cudaSuccess) e = cudaMemcpy(h->d_kv8_mul, kv8_mul.data(), kv8_mul.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMalloc(&h->d_kv8_scale, kv_scale.size() * sizeof(float));
+        if (e == cudaSuccess) e = cudaMemcpy(h->d_kv8_scale, kv_scale.data(), kv_scale.size() * sizeof(float), cudaMemcpyHostToDevice);
         if (e == cudaSuccess) e = cudaMalloc(&h->d_kv8_inv, kv8_inv.size() * sizeof(float));
         if (e == cudaSuccess) e = cudaMemcpy(h->d_kv8_inv, kv8_inv.data(), kv8_inv.size() * sizeof(float), cudaMemcpyHostToDevice);
     }
@@ -262,6 +265,7 @@ int msa_create(const msa_config *cfg, msa_handle *out)
         if (h->d_kv_to_q) cudaFree(h->d_kv_to_q);
         if (h->d_kv8_mul) cudaFree(h->d_kv8_mul);
         if (h->d_kv8_inv) cudaFree(h->d_kv8_inv);
+        if (h->d_kv8_scale) cudaFree(h->d_kv8_scale);
         delete h;
         return e != cudaSuccess ? cuda_fail(e, "msa_create") : MSA_ERR_NO_DEVICE;
     }
@@ -278,6 +282,7 @@ void msa_destroy(msa_handle h)
         if (h->d_kv_to_q) cudaFree(h->d_kv_to_q);
         if (h->d_kv8_mul) cudaFree(h->d_kv8_mul);
         if (h->d_kv8_inv) cudaFree(h->d_kv8_inv);
+        if (h->d_kv8_scale) cudaFree(h->d_kv8_scale);
         for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
         h->s_q.release(); h->s_o.release(); h->s_lse.release(); h->s_ck.release();
         h->s_cv.release(); h->s_bt.release(); h->s_ws.release();
@@ -677,6 +682,8 @@ int forward_impl(msa_handle h, msa_plan p, const void *q, int64_t total_q, const
     fp.tile_writer = writeback ? p->d_tile_writer : nullptr;
     fp.kv_to_q = h->d_kv_to_q;
     fp.kv8_mul = h->d_kv8_mul;
+    fp.kv8_scale = h->d_kv8_scale;
+    fp.kv8_inv = h->d_kv8_inv;
     fp.o = o;
     fp.lse = lse;
     fp.workspace = static_cast<float *>(workspace);

@@ -109,7 +109,9 @@ enum PipeBar : int {
     kBarPQ3 = 26,        // [2] P of keys 96-127 in TMEM
     kBarStgFull = 28,    // [4] KV8: fp8 blocks of a K (or V) tile have landed in a staging slot
     kBarStgEmpty = 32,   // [4] KV8: the four converter warps are done with a staging slot
-    kBarCount = 36
+    kBarQReady = 36,     // f16 variant: the converter warps have turned the unit's Q tile into f16
+    kBarKvDirect = 37,   // [5] f16 variant: the arena (bf16) blocks of a ring slot have landed and wait for their conversion
+    kBarCount = 42
 };
 constexpr int kConvWarps = 4;          // KV8: warps 8-11 convert (and, per unit, do the epilogue)
 
@@ -173,13 +175,13 @@ struct ResolvedVb {
 // The fp8 blocks of one K (or V) tile: staging slot (row-major, D bytes per row, block b at b*16*D) -> the bf16 tile in
 // its ring slot (128-byte swizzle, one 16 KB half per 64 elements, as TMA would have written it).  A warp iteration
 // covers 512 staged bytes (a lane: 16 codes = two 16-byte bf16 chunks); the calling warp takes the iterations whose bit
-// is set in it_mask.  Only rows < nvalid of a block are written (the V loader has zeroed the others, K's are masked).
+// is set in it_mask (even_w >= 0: the mask is the even split's, warp even_w of four).  Only rows < nvalid of a block are written (the V loader has zeroed the others, K's are masked).
 // The two stores of the lanes j and j + 4 of a row go to the same bank group (different 64-element halves): a two-way
 // conflict on the store pipe, which has room; ordering the stores per lane to avoid it costs ten selects per iteration
 // on the ALU pipe, which is what bounds the conversion (measured).
-template <int D>
+template <int D, bool F16 = false>
 __device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uint32_t m_paged, int nvp, uint32_t mul,
-                                                 uint32_t it_mask, int lane)
+                                                 uint32_t it_mask, int even_w, int lane)
 {
     constexpr int kLanesPerRow = D / 16, kRowsPerIt = 32 / kLanesPerRow, kItPerBlock = kBlock / kRowsPerIt;
     constexpr int kHalfBytes = kTileM * 128;
@@ -192,10 +194,10 @@ __device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uin
         const int row0 = (it / kItPerBlock) * kBlock + (it % kItPerBlock) * kRowsPerIt;      // tile row of the iteration's first row
         const uint32_t base = dst0 + static_cast<uint32_t>(row0 * 128);
         const uint32_t x = static_cast<uint32_t>((row0 + rsub) & 7);
-        const uint32_t o0 = e4m3x2_to_bf16x2(w0, mul), o1 = e4m3x2_to_bf16x2(w0 >> 16, mul);
-        const uint32_t o2 = e4m3x2_to_bf16x2(w1, mul), o3 = e4m3x2_to_bf16x2(w1 >> 16, mul);
-        const uint32_t o4 = e4m3x2_to_bf16x2(w2, mul), o5 = e4m3x2_to_bf16x2(w2 >> 16, mul);
-        const uint32_t o6 = e4m3x2_to_bf16x2(w3, mul), o7 = e4m3x2_to_bf16x2(w3 >> 16, mul);
+        // F16: the codes' f16 image, unscaled (one cvt per pair); else code * 2^k as bf16
+        auto cv = [mul](uint32_t two) { return F16 ? e4m3x2_to_f16x2(two) : e4m3x2_to_bf16x2(two, mul); };
+        const uint32_t o0 = cv(w0), o1 = cv(w0 >> 16), o2 = cv(w1), o3 = cv(w1 >> 16);
+        const uint32_t o4 = cv(w2), o5 = cv(w2 >> 16), o6 = cv(w3), o7 = cv(w3 >> 16);
         asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(base + ((c0 ^ x) << 4)), "r"(o0), "r"(o1), "r"(o2), "r"(o3) : "memory");
         asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(base + (((c0 + 1) ^ x) << 4)), "r"(o4), "r"(o5), "r"(o6), "r"(o7) : "memory");
     };
@@ -206,24 +208,37 @@ __device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uin
                      : "r"(src0 + static_cast<uint32_t>(row0 * D)));
     };
     const bool all_full = m_paged == 0xffu && __all_sync(0xffffffffu, lane >= kVbPerTile || (nvp & 0xff) == kBlock);
-    it_mask &= (kIters >= 32) ? 0xffffffffu : ((1u << (kIters & 31)) - 1u);
-    if (all_full) {
-        // the common tile (eight full cached blocks): four loads in flight before the first conversion -- one warp per
-        // SM sub-partition converts, and a shared-memory load takes a few hundred cycles next to the tensor core's reads
-        constexpr int kBatch = 4;
-#pragma unroll 1
-        while (it_mask != 0) {
-            uint32_t w[kBatch][4];
-            int its[kBatch];
+    if (all_full && even_w >= 0) {
+        // The common tile (eight full cached blocks), iterations dealt out evenly: warp w takes w, w + 4, ...  Four
+        // iterations further on is 2048 staged bytes and a whole number of 8-row swizzle groups further on, so a lane's load
+        // and store addresses are its first ones plus compile-time constants: nothing but the loads, the conversions and the
+        // stores is left in the unrolled loop (a warp instruction of the integer pipe issues every other cycle, and the
+        // address arithmetic of the general loop below costs more of them than the conversion itself).
+        constexpr int kPerWarp = kIters / kConvWarps;
+        constexpr uint32_t kSrcStep = 4u * kRowsPerIt * D, kDstStep = 4u * kRowsPerIt * 128u;
+        const int row_w = (even_w / kItPerBlock) * kBlock + (even_w % kItPerBlock) * kRowsPerIt + rsub;
+        const uint32_t x = static_cast<uint32_t>(row_w & 7);
+        const uint32_t src_l = stg + static_cast<uint32_t>(row_w * D + chunk * 16);
+        const uint32_t dst_l = dst + static_cast<uint32_t>((chunk >> 2) * kHalfBytes + row_w * 128);
+        const uint32_t d0 = dst_l + ((c0 ^ x) << 4), d1 = dst_l + (((c0 + 1) ^ x) << 4);
+        auto cv = [mul](uint32_t two) { return F16 ? e4m3x2_to_f16x2(two) : e4m3x2_to_bf16x2(two, mul); };
 #pragma unroll
-            for (int k = 0; k < kBatch; ++k) {
-                its[k] = it_mask ? __ffs(it_mask) - 1 : -1;
-                it_mask &= it_mask - 1;
-                if (its[k] >= 0) load(its[k], w[k][0], w[k][1], w[k][2], w[k][3]);
-            }
+        for (int k0 = 0; k0 < kPerWarp; k0 += 4) {
+            uint32_t w[4][4];
 #pragma unroll
-            for (int k = 0; k < kBatch; ++k)
-                if (its[k] >= 0) convert_store(its[k], w[k][0], w[k][1], w[k][2], w[k][3]);
+            for (int k = 0; k < 4; ++k)
+                if (k0 + k < kPerWarp)
+                    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
+                                 : "=r"(w[k][0]), "=r"(w[k][1]), "=r"(w[k][2]), "=r"(w[k][3])
+                                 : "r"(src_l + (k0 + k) * kSrcStep));
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (k0 + k < kPerWarp) {
+                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(d0 + (k0 + k) * kDstStep), "r"(cv(w[k][0])),
+                                 "r"(cv(w[k][0] >> 16)), "r"(cv(w[k][1])), "r"(cv(w[k][1] >> 16)) : "memory");
+                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(d1 + (k0 + k) * kDstStep), "r"(cv(w[k][2])),
+                                 "r"(cv(w[k][2] >> 16)), "r"(cv(w[k][3])), "r"(cv(w[k][3] >> 16)) : "memory");
+                }
         }
         return;
     }
@@ -241,38 +256,58 @@ __device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uin
     }
 }
 
-// Iterations of a tile for converter warp w (0-3) when warp 0 shares its SM sub-partition with the working softmax warps:
-// warp 0 takes iterations 0, 7, 14, 21, 28, the other 27 go to warps 1-3 in turn.
-__device__ __forceinline__ uint32_t kv8_skew_mask(int w)
-{
-    uint32_t m = 0;
-    int k = 0;
-#pragma unroll
-    for (int it = 0; it < 32; ++it) {
-        if (it % 7 == 0) {
-            if (w == 0) m |= 1u << it;
-        } else {
-            if (w == 1 + k % 3) m |= 1u << it;
-            ++k;
-        }
-    }
-    return m;
-}
-
 // KV8 converters (warps 8-11): every ring entry of the unit in ring order; for an entry whose tile holds cached blocks,
 // the calling warp converts the iterations of its mask (kv8_convert_tile) of the staged codes into the tile's ring slot
 // and arrives on the staging slot's "empty" barrier; every warp arrives on the ring slot's "full"
 // barrier for every entry.  An entry is waited for even when there is nothing to convert: a waiter that skips a use
 // of a slot cannot tell the phases of its barrier apart.
-template <class C, int D>
-__device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkUnit &wu, uint32_t bar0, uint32_t sStg, uint32_t sRing,
-                                                 int lane, uint32_t it_mask, uint32_t &cv_ent, uint32_t &cv_stg)
+// f16 variant: 16-byte chunks [first, n) in steps of stride * 32 of a shared-memory region, bf16 -> f16 in place, times `mult`
+// (a power of two or 1: exact unless the result leaves the f16 range).
+__device__ __forceinline__ void bf16_to_f16_inplace(uint32_t base, int n_chunks, int first, int stride, int lane, float mult)
+{
+    for (int i = first * 32 + lane; i < n_chunks; i += stride * 32) {
+        uint32_t w[4];
+        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "r"(base + i * 16u));
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            w[k] = pack_f16x2(__uint_as_float(w[k] << 16) * mult, __uint_as_float(w[k] & 0xffff0000u) * mult);
+        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(base + i * 16u), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]) : "memory");
+    }
+}
+
+// F16 (the short-query variant, see the kernel): the ring holds f16 tiles.  The codes become their f16 image, the arena
+// blocks of a tile -- loaded as bf16 by the ring loaders, complete on the slot's "direct" barrier -- are rewritten in place
+// as f16 divided by the KV head's scale, and at the start of the unit the Q tile is rewritten as f16 (cw_first / cw_stride:
+// this warp's share of that work; cw_first < 0: none).
+template <class C, int D, bool F16>
+__device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkUnit &wu, uint32_t bar0, uint32_t sQ, uint32_t sStg,
+                                                 uint32_t sRing, int lane, uint32_t it_mask, int even_w, int cw_first, int cw_stride,
+                                                 uint32_t &cv_ent, uint32_t &cv_stg, uint32_t &cv_phq, uint32_t &dir_par)
 {
     auto bar = [bar0](int i) { return bar0 + static_cast<uint32_t>(i) * 8u; };
     const int n = wu.tile_end - wu.tile_begin;
     const bool pair = wu.mode == kModePair;
     const uint32_t mul_k = __ldg(P.kv8_mul + wu.kvh), mul_v = __ldg(P.kv8_mul + P.Hkv + wu.kvh);
     PROF_DECL();
+    float inv_k = 1.f, inv_v = 1.f;
+    if constexpr (F16) {
+        if (n <= 0) return;
+        inv_k = __ldg(P.kv8_inv + wu.kvh);
+        inv_v = __ldg(P.kv8_inv + P.Hkv + wu.kvh);
+        // Q: bf16 -> f16 in place (the rows that hold tokens; all of them with head-major packing), then "Q ready"
+        PROF_T0();
+        mbar_wait(bar(kBarQFull), cv_phq);
+        cv_phq ^= 1;
+        const int rows_q = P.token_major ? min(kTileM, (wu.n_tok * P.G + 31) & ~31) : kTileM;     // whole softmax warps
+        if (cw_first >= 0) {
+#pragma unroll 1
+            for (int h = 0; h < C::kHalves; ++h) bf16_to_f16_inplace(sQ + h * C::kHalfBytes, rows_q * 8, cw_first, cw_stride, lane, 1.f);
+        }
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(kBarQReady));
+        PROF_ADD(30);
+    }
     auto fetch_nvp = [&](int e) -> int {             // lane b < 8: nvalid | paged << 8 of virtual block b of entry e's tile
         int r = 0;
         if (e < 2 * n) {
@@ -292,6 +327,7 @@ __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkU
     for (int e = 0; e < 2 * n; ++e) {
         const int nxt = fetch_nvp(e + 1);
         const uint32_t m_paged = __ballot_sync(0xffffffffu, (cur >> 8) != 0) & 0xffu;
+        const uint32_t m_dir = __ballot_sync(0xffffffffu, (cur >> 8) == 0 && (cur & 0xff) != 0) & 0xffu;
         bool is_v;
         int t;
         kv8_entry(e, n, pair, is_v, t);
@@ -309,14 +345,59 @@ __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkU
                 PROF_ADD(22);
             }
             PROF_T0();
-            kv8_convert_tile<D>(sStg + st * C::kStgTileBytes, sRing + slot * C::kTileBytes, m_paged, cur, is_v ? mul_v : mul_k,
-                                it_mask, lane);
+            kv8_convert_tile<D, F16>(sStg + st * C::kStgTileBytes, sRing + slot * C::kTileBytes, m_paged, cur, is_v ? mul_v : mul_k,
+                                     it_mask, even_w, lane);
             PROF_ADD(27);
             PROF_INC(24, 1);
             fence_proxy_async_smem();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(kBarStgEmpty + st));
             ++cv_stg;
+        }
+        if constexpr (F16) {
+            // the arena blocks (and the V loader's zero fill) of this entry, if it has any, are in the slot
+            const uint32_t m_full = __ballot_sync(0xffffffffu, (cur & 0xff) == kBlock) & 0xffu;
+            if (m_dir != 0 || (is_v && m_full != 0xffu)) {
+                PROF_T0();
+                mbar_wait(bar(kBarKvDirect + slot), (dir_par >> slot) & 1u);
+                PROF_ADD(28);
+                dir_par ^= 1u << slot;
+            }
+            PROF_T0();
+            if (m_dir != 0 && cw_first >= 0) {
+                const float mult = is_v ? inv_v : inv_k;
+                const uint32_t tile = sRing + slot * C::kTileBytes;
+#pragma unroll 1
+                for (int b = 0; b < kVbPerTile; ++b) {
+                    if (!((m_dir >> b) & 1u)) continue;
+                    const int nv = __shfl_sync(0xffffffffu, cur, b) & 0xff;
+                    if (nv == kBlock && cw_stride == kConvWarps) {
+                        // a full block: 16 rows x 128 B per 64-element half; the four warps take equal, fixed shares
+                        constexpr int kChunks = kBlock * 8 * C::kHalves;         // 16-byte chunks of the block
+                        constexpr int kPerLane = kChunks / (kConvWarps * 32);     // 2 (D = 128) or 1 (D = 64)
+                        uint32_t w[kPerLane][4], addr[kPerLane];
+#pragma unroll
+                        for (int k = 0; k < kPerLane; ++k) {
+                            const int i = (cw_first * kPerLane + k) * 32 + lane;  // chunk of the block, halves one after the other
+                            addr[k] = tile + static_cast<uint32_t>((i / (kBlock * 8)) * C::kHalfBytes + b * (kBlock * 128) + (i % (kBlock * 8)) * 16);
+                            asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(w[k][0]), "=r"(w[k][1]), "=r"(w[k][2]), "=r"(w[k][3]) : "r"(addr[k]));
+                        }
+#pragma unroll
+                        for (int k = 0; k < kPerLane; ++k) {
+#pragma unroll
+                            for (int j = 0; j < 4; ++j)
+                                w[k][j] = pack_f16x2(__uint_as_float(w[k][j] << 16) * mult, __uint_as_float(w[k][j] & 0xffff0000u) * mult);
+                            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr[k]), "r"(w[k][0]), "r"(w[k][1]), "r"(w[k][2]), "r"(w[k][3]) : "memory");
+                        }
+                    } else {
+#pragma unroll 1
+                        for (int h = 0; h < C::kHalves; ++h)
+                            bf16_to_f16_inplace(tile + h * C::kHalfBytes + b * (kBlock * 128), nv * 8, cw_first, cw_stride, lane, mult);
+                    }
+                }
+                fence_proxy_async_smem();
+            }
+            PROF_ADD(29);
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar(kBarKvFull + slot));
@@ -329,7 +410,7 @@ __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkU
 #endif
     if ((threadIdx.x >> 5) == MSA_PROF_CVWARP && lane == 0) {
         PROF_FLUSH(21, 25);
-        PROF_FLUSH(27, 28);
+        PROF_FLUSH(27, 31);
     }
 #endif
 }
@@ -338,6 +419,11 @@ template <int D, bool KV8, int QT>
 __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_constant__ FwdParams P)
 {
     using C = PipeCfg<D, KV8, QT>;
+    // The fp8 short-query variant multiplies in f16: the codes' exact f16 image is one instruction per pair (the bf16 image costs
+    // four), so Q, the arena blocks of a tile and P are f16 as well -- kind::f16 cannot mix the two formats in one MMA.  The
+    // scales move out of the operands: S is scaled by k_scale through the softmax scale, O by v_scale in the epilogue, the arena
+    // rows are divided by the scale when they are converted (all powers of two: exact).
+    constexpr bool F16 = KV8 && QT == 1;
     extern __shared__ __align__(1024) uint8_t smem[];
     const uint32_t sbase = smem_u32(smem);
     const uint32_t sQ = sbase, sRing = sbase + C::kQBytes;
@@ -356,9 +442,11 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
     // one-time setup: barriers, TMEM
     if (threadIdx.x == 0) {
         mbar_init(bar(kBarQFull), 1);
+        mbar_init(bar(kBarQReady), kConvWarps);
         mbar_init(bar(kBarQEmpty), 1);
         for (int i = 0; i < C::kStages; ++i) {
-            mbar_init(bar(kBarKvFull + i), KV8 ? 1 + kConvWarps : 1);  // the loader (+ KV8: every converter warp)
+            mbar_init(bar(kBarKvFull + i), F16 ? kConvWarps : KV8 ? 1 + kConvWarps : 1);  // the loader (+ KV8: every converter warp; f16: only they)
+            mbar_init(bar(kBarKvDirect + i), 1);
             mbar_init(bar(kBarKvEmpty + i), kWritebackRing ? 2 : 1);   // the MMA warp's commit + the loader (or the write-back warp)
         }
         for (int i = 0; i < C::kStgStages; ++i) {
@@ -386,7 +474,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
     const uint32_t tmem = *tmem_slot;
     const int u_begin = P.cta_unit_begin[blockIdx.x], u_end = P.cta_unit_begin[blockIdx.x + 1];
     const int G = P.G, R = P.R;
-    const float sl = P.scale_log2;
+    const float sl0 = P.scale_log2;
 
     if (warp < 8) {
         // =========================================================== softmax warpgroups
@@ -409,6 +497,8 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             if (steps <= 0) continue;
             const int p_row = wu.q_abs0 + (pair ? c * R : 0) + t;
             const int p_min = wu.q_abs0 + (pair ? c * R : 0);
+            // f16 variant: K's scale is not in the operand (the codes are multiplied as they are), it scales S
+            const float sl = F16 ? sl0 * __ldg(P.kv8_scale + wu.kvh) : sl0;
             // Token-major packing: the valid rows of the tile are its first tok * G rows.  A warp whose 32 rows lie beyond
             // them skips the unit's tiles altogether (its rows of S, P and O hold garbage nobody reads); the first warp of
             // the chain gives the idle warps' arrivals on the P barriers along with its own.
@@ -485,7 +575,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     // fast path: stale reference, tile max found alongside, P handed over in parts
                     move_reference(true);
                     float tile_sum, tile_max;
-                    done = softmax_fast_tile(tS, sl, ref, tile_sum, tile_max, [&](int part) {
+                    done = softmax_fast_tile<F16>(tS, sl, ref, tile_sum, tile_max, [&](int part) {
                         __syncwarp();
                         if (lane == 0) mbar_arrive_n(bar((part == 0 ? kBarPLo : kBarPQ2) + c), p_arrivals);
                         if ((threadIdx.x & 127) == 0 && part == 0) PROF_TRACE(1 + c, s, 4);
@@ -537,7 +627,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                             const float p1 = ex2_approx(fmaf(__uint_as_float(sr[q * 32 + 2 * j + 1]), sl, -ref));
                             sum0 += p0;
                             sum1 += p1;
-                            pk[j] = pack_bf16x2(p0, p1);
+                            pk[j] = F16 ? pack_f16x2(p0, p1) : pack_bf16x2(p0, p1);
                         }
                     };
                     auto publish = [&](int b) {
@@ -587,7 +677,9 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
         const uint32_t trow = tmem + (static_cast<uint32_t>((warp & 3) * 32) << 16);
         uint32_t ph_o[2] = {0, 0};
         uint32_t cv_ent = 0, cv_stg = 0;       // KV8: ring entry / staging entry the converters are at (CTA-wide counters)
-        (void)cv_ent; (void)cv_stg;
+        uint32_t cv_phq = 0;                   // f16 variant: phase of the "Q landed" barrier the converters wait on
+        uint32_t cv_dirpar = 0;                // f16 variant: per ring slot, parity of its "direct" barrier (used by some entries only)
+        (void)cv_ent; (void)cv_stg; (void)cv_phq; (void)cv_dirpar;
         PROF_DECL();
         for (int u = u_begin; u < u_end; ++u) {
             const WorkUnit wu = P.units[u];
@@ -595,13 +687,9 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             const bool pair = wu.mode == kModePair;
             const int rows_total = wu.n_tok * G;
             if constexpr (KV8) {
-                // ---- converters (kv8_convert_unit).  Every warp takes every fourth warp iteration of a tile, unless the unit's
-                // valid q rows fit one softmax warp per chain (token-major packing, short queries): those two warps exponentiate
-                // on SM sub-partition 0, which warp 8 shares with them, so warp 8 takes 5 of the 32 iterations and warps 9-11
-                // nine each.
-                const bool one_row_warp = P.token_major && !pair && wu.n_tok * G <= 32;
-                const uint32_t it_mask = one_row_warp ? kv8_skew_mask(warp - 8) : (0x11111111u << (warp - 8));
-                kv8_convert_unit<C, D>(P, wu, bar0, sStg, sRing, lane, it_mask, cv_ent, cv_stg);
+                // ---- converters (kv8_convert_unit): warp w of the four takes every fourth warp iteration of a tile
+                kv8_convert_unit<C, D, F16>(P, wu, bar0, sQ, sStg, sRing, lane, 0x11111111u << (warp - 8), warp - 8, warp - 8, 4, cv_ent,
+                                            cv_stg, cv_phq, cv_dirpar);
             }
             const int n_out = pair ? 2 : 1;                       // q tiles written by this unit
             for (int qt = 0; qt < n_out; ++qt) {
@@ -640,6 +728,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                         inv_l = 1.f / lt;
                         lse_val = (mm + log2f(lt)) * 0.6931471805599453f;
                     }
+                    if constexpr (F16) inv_l *= __ldg(P.kv8_scale + P.Hkv + wu.kvh);      // V's scale (the codes were multiplied as they are)
                     w0 *= inv_l;
                     w1 *= inv_l;
                     if (act0) {
@@ -823,7 +912,9 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                         mbar_wait(bar(kBarKvEmpty + slot), phase);
                         PROF_ADD(16);
                     }
-                    const uint32_t full = bar(kBarKvFull + slot);
+                    // f16 variant: the arena blocks land as bf16 and the converter warps rewrite them in place, so the loads (and
+                    // this warp's zero fill) complete on the slot's "direct" barrier, every entry, and only the converters arrive on "full"
+                    const uint32_t full = bar((F16 ? kBarKvDirect : kBarKvFull) + slot);
                     const uint32_t dst = sRing + slot * C::kTileBytes;
                     if (which == 1 && m_full != 0xffu) {
                         // V rows TMA will not write (block tails, blocks past the end / the horizon): zero them
@@ -840,7 +931,11 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                         fence_proxy_async_smem();
                         __syncwarp();
                     }
-                    if (run) {
+                    // f16 variant: an entry with neither arena blocks nor a zero fill does not use the "direct" barrier at all
+                    // (the converter warps make the same test): no extra barrier hop on the common, all-cached tile
+                    const bool skip_direct = F16 && m_dir == 0 && !(which == 1 && m_full != 0xffu);
+                    if (skip_direct) {
+                    } else if (run) {
                         if (elect_one()) {
                             mbar_arrive_expect_tx(full, static_cast<uint32_t>(kTileN * D * 2));
 #pragma unroll
@@ -896,8 +991,8 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
 #endif
         } else if (warp == 13 && elect_one()) {
             // ======================================================= MMA issuer (one thread)
-            constexpr uint32_t idesc_s = make_idesc(128, 128, false);
-            constexpr uint32_t idesc_o = make_idesc(128, D, true);
+            constexpr uint32_t idesc_s = make_idesc(128, 128, false, F16);
+            constexpr uint32_t idesc_o = make_idesc(128, D, true, F16);
             RingPos rk{0, 0}, rv{1, 0};
             uint32_t ph_q = 0, ph_p[2] = {0, 0}, ph_ofree[2] = {1, 1};
             int u = u_begin, tr_step = 0;    // (trace builds: which unit / KV step the issuer is in)
@@ -1012,7 +1107,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                 if (n <= 0) continue;
                 {
                     PROF_T0();
-                    mbar_wait(bar(kBarQFull), ph_q);
+                    mbar_wait(bar(F16 ? kBarQReady : kBarQFull), ph_q);
                     PROF_ADD(13);
                 }
                 ph_q ^= 1;

@@ -23,4 +23,12 @@ __device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t two_codes, uint32_
     return r;
 }
 
+// Two codes -> their exact f16 image, unscaled (the short-query variant multiplies in f16 and applies the scales outside the MMAs).
+__device__ __forceinline__ uint32_t e4m3x2_to_f16x2(uint32_t two_codes)
+{
+    uint32_t h;
+    asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(h) : "h"(static_cast<uint16_t>(two_codes)));
+    return h;
+}
+
 }  // namespace msa

@@ -176,12 +176,13 @@ __device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr, uint32_t lbo_
     d |= static_cast<uint64_t>(2) << 61;
     return d;
 }
-// Instruction descriptor for kind::f16: D fp32, A/B bf16, A K-major, dense.
-//   [4,6) D fmt (1=f32)  [7,10) A fmt (1=bf16)  [10,13) B fmt (1=bf16)
+// Instruction descriptor for kind::f16: D fp32, A and B both bf16 or both f16 (one MMA cannot mix the two: it traps),
+// A K-major, dense.
+//   [4,6) D fmt (1=f32)  [7,10) A fmt (0=f16, 1=bf16)  [10,13) B fmt (0=f16, 1=bf16)
 //   [15] A major  [16] B major (1 = MN-major)  [17,23) N>>3  [24,29) M>>4
-__host__ __device__ constexpr uint32_t make_idesc(int M, int N, bool b_mn_major)
+__host__ __device__ constexpr uint32_t make_idesc(int M, int N, bool b_mn_major, bool f16 = false)
 {
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn_major ? 1u : 0u) << 16) |
+    return (1u << 4) | ((f16 ? 0u : 1u) << 7) | ((f16 ? 0u : 1u) << 10) | ((b_mn_major ? 1u : 0u) << 16) |
            (static_cast<uint32_t>(N >> 3) << 17) | (static_cast<uint32_t>(M >> 4) << 24);
 }
 
@@ -305,6 +306,13 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi)
 {
     uint32_t r;
     asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
+// {lo, hi} -> packed f16x2 (lo in bits [0,16))
+__device__ __forceinline__ uint32_t pack_f16x2(float lo, float hi)
+{
+    uint32_t r;
+    asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
     return r;
 }
 // Packed fp32 pairs (sm_100 FFMA2 / FADD2): one issue slot for two lanes of the softmax row.

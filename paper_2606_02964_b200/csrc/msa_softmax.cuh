@@ -31,7 +31,8 @@
 
 namespace msa {
 
-constexpr float kGuardLog2 = 64.f;    // largest s*scale_log2 - ref the fast path accepts
+constexpr float kGuardLog2 = 64.f;    // largest s*scale_log2 - ref the fast path accepts (P in bf16)
+constexpr float kGuardLog2F16 = 14.f; // ... when P is handed over in f16 (fp8-pool short-query variant): P <= 2^14 < 65504
 
 struct SoftmaxRow {
     float2 sl2;       // scale_log2
@@ -59,7 +60,7 @@ __device__ __forceinline__ float chunk_max(const uint32_t (&sr)[32])
 
 // Pairs [J0, J1) of a 32-column chunk: scores -> packed bf16 pairs; two sum accumulators keep
 // the dependent FADD2 chain short.
-template <int J0, int J1>
+template <int J0, int J1, bool F16 = false>
 __device__ __forceinline__ void softmax_pairs(const uint32_t (&sr)[32], const SoftmaxRow &t, float2 &sa, float2 &sb,
                                               uint32_t (&pk)[16])
 {
@@ -71,7 +72,7 @@ __device__ __forceinline__ void softmax_pairs(const uint32_t (&sr)[32], const So
         pp.x = ex2_approx(x.x);
         pp.y = ex2_approx(x.y);
         if (j & 1) sb = fadd2(sb, pp); else sa = fadd2(sa, pp);
-        pk[j] = pack_bf16x2(pp.x, pp.y);
+        pk[j] = F16 ? pack_f16x2(pp.x, pp.y) : pack_bf16x2(pp.x, pp.y);
     }
 }
 
@@ -82,7 +83,7 @@ __device__ __forceinline__ void softmax_pairs(const uint32_t (&sr)[32], const So
 // (no-op in the shipped build).  tile_sum = sum of p against `ref`, tile_max = max raw score.
 // The waits for the P stores name registers of the chunk computed in between (tmem_wait_st_after):
 // without that the compiler is free to schedule the wait -- and the stall -- right behind the store.
-template <class Arrive, class Mark>
+template <bool F16 = false, class Arrive, class Mark>
 __device__ __forceinline__ bool softmax_fast_tile(uint32_t tS, float sl, float ref, float &tile_sum,
                                                   float &tile_max, Arrive &&arrive, Mark &&mark)
 {
@@ -98,31 +99,31 @@ __device__ __forceinline__ bool softmax_fast_tile(uint32_t tS, float sl, float r
     tmem_ld32(tS + 96, c3);
     mark(1);
     float mx = fmaxf(chunk_max(c0), chunk_max(c1));
-    softmax_pairs<0, 16>(c0, t, sa, sb, pk0);
+    softmax_pairs<0, 16, F16>(c0, t, sa, sb, pk0);
     // the second half has landed by now: its row max is found among the arithmetic of chunk 1,
     // so the guard is ready as soon as the first half of P is
     tmem_wait_ld_regs(c2);
     tmem_wait_ld_regs(c3);
     mx = fmaxf(mx, fmaxf(chunk_max(c2), chunk_max(c3)));
-    softmax_pairs<0, 16>(c1, t, sa, sb, pk1);
+    softmax_pairs<0, 16, F16>(c1, t, sa, sb, pk1);
     mark(2);
     tile_max = mx;
-    if (__any_sync(0xffffffffu, !(fmaf(mx, sl, -ref) <= kGuardLog2))) return false;
+    if (__any_sync(0xffffffffu, !(fmaf(mx, sl, -ref) <= (F16 ? kGuardLog2F16 : kGuardLog2)))) return false;
     mark(3);
     tmem_st16(tS, pk0);
     tmem_st16(tS + 16, pk1);
     // each part is published while the next one is computed: its stores have completed by then
     // (no stall), and O += P V of the published keys finishes before the next part is ready
-    softmax_pairs<0, 16>(c2, t, sa, sb, pk0);
+    softmax_pairs<0, 16, F16>(c2, t, sa, sb, pk0);
     tmem_wait_st_after(pk0[12], pk0[13], pk0[14], pk0[15]);
     tc_fence_before();
     arrive(0);
     tmem_st16(tS + 32, pk0);
-    softmax_pairs<0, 8>(c3, t, sa, sb, pk1);
+    softmax_pairs<0, 8, F16>(c3, t, sa, sb, pk1);
     tmem_wait_st_after(pk1[4], pk1[5], pk1[6], pk1[7]);
     tc_fence_before();
     arrive(1);
-    softmax_pairs<8, 16>(c3, t, sa, sb, pk1);
+    softmax_pairs<8, 16, F16>(c3, t, sa, sb, pk1);
     tmem_st16(tS + 48, pk1);
     tile_sum = (sa.x + sb.x) + (sa.y + sb.y);
     mark(5);

@@ -157,6 +157,21 @@ def _dequantised_twin(p8):
     return p
 
 
+def _against_the_bf16_kernel(p8, o, lse):
+    """code * 2^k is exactly a bf16.  The pre-pass and the two-Q-tile kernel variant feed those bf16 values to the same MMAs:
+    bit-identical to the bf16 kernel on the dequantised pool.  The short-query variant multiplies the codes' f16 image and hands P
+    over in f16 (three more mantissa bits than bf16): not the same bits, but the same scores up to fp32 rounding of the scale
+    product and an O within the bf16 path's own distance from the oracle."""
+    o2, lse2, _ = gpu_forward(_dequantised_twin(p8))
+    if _kv8_path(p8, device=0)[0] != "kernel_split":
+        assert np.array_equal(o, o2) and np.array_equal(lse, lse2)
+    else:
+        fin = np.isfinite(lse2)
+        assert np.array_equal(np.isfinite(lse), fin)
+        assert np.abs(lse[fin] - lse2[fin]).max() <= 1e-5 if fin.any() else True
+        assert np.all(np.abs(o - o2) <= TOL_O_MAX * np.maximum(1.0, np.abs(o2) / 2.0))
+
+
 CASES = [
     dict(seed=101, Hq=4, Hkv=2, D=64, max_ctx=700, max_q=96),
     dict(seed=102, Hq=8, Hkv=2, D=128, max_ctx=900, max_q=70),
@@ -179,9 +194,7 @@ def test_kv8_random_small_problems_against_the_oracle_and_the_bf16_kernel(kw):
     p8 = W.to_fp8_pool(p, k_exp=[exps[h % 4][0] for h in range(p.Hkv)], v_exp=[exps[h % 4][1] for h in range(p.Hkv)])
     o, lse, _ = gpu_forward(p8)
     compare(p8, o, lse, strict=False)
-    # code * 2^k is exactly a bf16 and the conversion happens before the same MMAs: bit-identical to the bf16 kernel
-    o2, lse2, _ = gpu_forward(_dequantised_twin(p8))
-    assert np.array_equal(o, o2) and np.array_equal(lse, lse2)
+    _against_the_bf16_kernel(p8, o, lse)
 
 
 @pytest.mark.gpu
@@ -193,8 +206,7 @@ def test_kv8_each_path_against_the_oracle_and_the_bf16_kernel(want):
     assert _kv8_path(p8, device=0)[0] == want
     o, lse, _ = gpu_forward(p8)
     compare(p8, o, lse, strict=False)
-    o2, lse2, _ = gpu_forward(_dequantised_twin(p8))
-    assert np.array_equal(o, o2) and np.array_equal(lse, lse2)
+    _against_the_bf16_kernel(p8, o, lse)
 
 
 @pytest.mark.gpu
