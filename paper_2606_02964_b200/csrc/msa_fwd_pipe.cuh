@@ -207,6 +207,9 @@ __device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uin
                      : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3)
                      : "r"(src0 + static_cast<uint32_t>(row0 * D)));
     };
+#ifdef MSA_KV8_SKIP_CONVERT           /* timing experiments only: wrong results */
+    return;
+#endif
     const bool all_full = m_paged == 0xffu && __all_sync(0xffffffffu, lane >= kVbPerTile || (nvp & 0xff) == kBlock);
     if (all_full && even_w >= 0) {
         // The common tile (eight full cached blocks), iterations dealt out evenly: warp w takes w, w + 4, ...  Four
@@ -220,7 +223,12 @@ __device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uin
         const uint32_t x = static_cast<uint32_t>(row_w & 7);
         const uint32_t src_l = stg + static_cast<uint32_t>(row_w * D + chunk * 16);
         const uint32_t dst_l = dst + static_cast<uint32_t>((chunk >> 2) * kHalfBytes + row_w * 128);
-        const uint32_t d0 = dst_l + ((c0 ^ x) << 4), d1 = dst_l + (((c0 + 1) ^ x) << 4);
+        // The lanes j and j + 4 of a row write the same bank group (different 64-element halves): the upper four store their two
+        // chunks in the other order, so that the eight lanes of a quarter-warp hit eight different bank groups (the conversion is
+        // bound by the shared-memory pipe: a two-way conflict on every store costs a third of its time)
+        const bool sw = kLanesPerRow == 8 && (chunk & 4) != 0;
+        const uint32_t da = dst_l + ((c0 ^ x) << 4), db = dst_l + (((c0 + 1) ^ x) << 4);
+        const uint32_t d0 = sw ? db : da, d1 = sw ? da : db;
         auto cv = [mul](uint32_t two) { return F16 ? e4m3x2_to_f16x2(two) : e4m3x2_to_bf16x2(two, mul); };
 #pragma unroll
         for (int k0 = 0; k0 < kPerWarp; k0 += 4) {
@@ -234,10 +242,13 @@ __device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uin
 #pragma unroll
             for (int k = 0; k < 4; ++k)
                 if (k0 + k < kPerWarp) {
-                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(d0 + (k0 + k) * kDstStep), "r"(cv(w[k][0])),
-                                 "r"(cv(w[k][0] >> 16)), "r"(cv(w[k][1])), "r"(cv(w[k][1] >> 16)) : "memory");
-                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(d1 + (k0 + k) * kDstStep), "r"(cv(w[k][2])),
-                                 "r"(cv(w[k][2] >> 16)), "r"(cv(w[k][3])), "r"(cv(w[k][3] >> 16)) : "memory");
+                    // (the codes are swapped, not the converted values: two selects per store)
+                    const uint32_t a0 = sw ? w[k][2] : w[k][0], a1 = sw ? w[k][3] : w[k][1];
+                    const uint32_t b0 = sw ? w[k][0] : w[k][2], b1 = sw ? w[k][1] : w[k][3];
+                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(d0 + (k0 + k) * kDstStep), "r"(cv(a0)),
+                                 "r"(cv(a0 >> 16)), "r"(cv(a1)), "r"(cv(a1 >> 16)) : "memory");
+                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(d1 + (k0 + k) * kDstStep), "r"(cv(b0)),
+                                 "r"(cv(b0 >> 16)), "r"(cv(b1)), "r"(cv(b1 >> 16)) : "memory");
                 }
         }
         return;
