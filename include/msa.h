@@ -207,6 +207,21 @@ int msa_forward_host(msa_handle h, msa_plan p,
                      float softmax_scale,
                      void *o_host, float *lse_host, void *cuda_stream);
 
+/* The same call without the wait, for a caller that keeps two steps in flight: the uploads run on a stream of the handle's
+ * own, the kernels on `cuda_stream`, the read-back on a second stream of the handle's, chained by events, and each of the
+ * two `slot`s (0 or 1) has its own staging buffers -- so the upload of one call overlaps the kernels and the read-back of the
+ * call before it (PCIe is full duplex).  o_host / lse_host of a call are valid after msa_forward_host_wait(h, slot) (or after
+ * the next msa_forward_host_async on the same slot, which waits for it first); the host input buffers must stay unchanged
+ * until then.  msa_forward_host = msa_forward_host_async on slot 0 + msa_forward_host_wait. */
+int msa_forward_host_async(msa_handle h, msa_plan p,
+                           const void *q_host, int64_t total_q,
+                           const void *pool_k, const void *pool_v, int64_t num_blocks,
+                           const int32_t *block_table_host, int64_t block_table_len,
+                           const void *contig_k_host, const void *contig_v_host, int64_t contig_rows,
+                           float softmax_scale,
+                           void *o_host, float *lse_host, void *cuda_stream, int32_t slot);
+int msa_forward_host_wait(msa_handle h, int32_t slot);
+
 /* ---- KV write-back (PAPER.md:92 step 2: recomputed K/V are written into cache blocks) ----
  * After a step, the K/V rows a request has just (re)computed -- CONTIG and SELF segments of the arena -- are appended
  * to the paged cache so that the next step can reach them as PAGED segments.  One job copies arena rows

@@ -9,6 +9,6 @@ from .binding import (  # noqa: F401
     MSA_SEG_PAGED, MSA_SEG_CONTIG, MSA_SEG_SELF, MSA_POOL_BF16, MSA_POOL_FP8_E4M3,
     MsaError, MsaSession, MsaEvictor, make_descriptors,
     msa_create, msa_destroy, msa_plan_create, msa_plan_destroy, msa_plan_get_info, msa_plan_export,
-    msa_workspace_bytes, msa_forward, msa_forward_host, msa_append_plan_create, msa_append_plan_destroy, msa_kv_append, msa_plan_create_writeback, msa_forward_writeback, msa_last_launch_count, msa_set_timing, msa_get_timing, msa_version,
+    msa_workspace_bytes, msa_forward, msa_forward_host, msa_forward_host_async, msa_forward_host_wait, msa_append_plan_create, msa_append_plan_destroy, msa_kv_append, msa_plan_create_writeback, msa_forward_writeback, msa_last_launch_count, msa_set_timing, msa_get_timing, msa_version,
 )
 from ._build import build, LIB_PATH  # noqa: F401

@@ -61,7 +61,7 @@ EXPORTS = ["msa_create", "msa_destroy", "msa_plan_create", "msa_plan_destroy", "
            "msa_plan_export", "msa_workspace_bytes", "msa_forward", "msa_forward_host",
            "msa_last_launch_count", "msa_set_timing", "msa_get_timing", "msa_strerror", "msa_last_cuda_error", "msa_version",
            "msa_append_plan_create", "msa_append_plan_destroy", "msa_kv_append",
-           "msa_plan_create_writeback", "msa_forward_writeback"]
+           "msa_plan_create_writeback", "msa_forward_writeback", "msa_forward_host_async", "msa_forward_host_wait"]
 EVICTOR_EXPORTS = ["msa_evictor_create", "msa_evictor_destroy", "msa_evictor_add", "msa_evictor_remove", "msa_evictor_evict",
                    "msa_evictor_evict_linear", "msa_evictor_set_lambda", "msa_evictor_size", "msa_evictor_weight"]
 
@@ -95,6 +95,8 @@ def _lib() -> ctypes.CDLL:
         lib.msa_workspace_bytes.argtypes = [vp, ctypes.POINTER(sz)]
         lib.msa_forward.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, i64, f32, vp, vp, vp, sz, vp]
         lib.msa_forward_host.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, i64, f32, vp, vp, vp]
+        lib.msa_forward_host_async.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, i64, f32, vp, vp, vp, i32]
+        lib.msa_forward_host_wait.argtypes = [vp, i32]
         lib.msa_last_launch_count.argtypes = [vp]
         lib.msa_set_timing.argtypes = [vp, ctypes.c_int]
         lib.msa_get_timing.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(ctypes.c_double),
@@ -252,6 +254,23 @@ def msa_forward_host(h, p, q_host, pool_k, pool_v, block_table_host, contig_k_ho
                                    _dptr(block_table_host), bt_len, _dptr(contig_k_host), _dptr(contig_v_host), rows,
                                    ctypes.c_float(softmax_scale), _dptr(o_host), _dptr(lse_host), stream),
            "msa_forward_host")
+
+
+def msa_forward_host_async(h, p, q_host, pool_k, pool_v, block_table_host, contig_k_host, contig_v_host,
+                           softmax_scale: float, o_host, lse_host, stream: Optional[int] = None, slot: int = 0) -> None:
+    """msa_forward_host without the wait (two slots; results valid after msa_forward_host_wait(h, slot))."""
+    total_q = int(q_host.shape[0])
+    num_blocks = 0 if pool_k is None else int(pool_k.shape[0])
+    bt_len = 0 if block_table_host is None else int(block_table_host.numel())
+    rows = 0 if contig_k_host is None else int(contig_k_host.shape[0])
+    _check(_lib().msa_forward_host_async(h, p, _dptr(q_host), total_q, _dptr(pool_k), _dptr(pool_v), num_blocks,
+                                         _dptr(block_table_host), bt_len, _dptr(contig_k_host), _dptr(contig_v_host), rows,
+                                         ctypes.c_float(softmax_scale), _dptr(o_host), _dptr(lse_host), stream, slot),
+           "msa_forward_host_async")
+
+
+def msa_forward_host_wait(h, slot: int = 0) -> None:
+    _check(_lib().msa_forward_host_wait(h, slot), "msa_forward_host_wait")
 
 
 def msa_last_launch_count(h) -> int:

@@ -111,8 +111,15 @@ struct msa_handle_s {
     bool timing = false;
     std::vector<cudaEvent_t> ev;
     int ev_steps = 0;
-    // staging for msa_forward_host
-    DevBuf s_q, s_o, s_lse, s_ck, s_cv, s_bt, s_ws;
+    // staging for msa_forward_host / msa_forward_host_async: two slots, so that the upload of one call overlaps the kernels and the
+    // read-back of the one before it; copies run on two streams of the handle's own, chained to the caller's stream by events
+    struct HostSlot {
+        DevBuf s_q, s_o, s_lse, s_ck, s_cv, s_bt, s_ws;
+        cudaEvent_t in_done = nullptr, k_done = nullptr, out_done = nullptr;
+        bool busy = false;
+    };
+    HostSlot hs[2];
+    cudaStream_t st_in = nullptr, st_out = nullptr;
 };
 
 struct msa_plan_s {
@@ -284,8 +291,16 @@ void msa_destroy(msa_handle h)
         if (h->d_kv8_inv) cudaFree(h->d_kv8_inv);
         if (h->d_kv8_scale) cudaFree(h->d_kv8_scale);
         for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
-        h->s_q.release(); h->s_o.release(); h->s_lse.release(); h->s_ck.release();
-        h->s_cv.release(); h->s_bt.release(); h->s_ws.release();
+        for (auto &sl : h->hs) {
+            if (sl.busy && sl.out_done) cudaEventSynchronize(sl.out_done);
+            sl.s_q.release(); sl.s_o.release(); sl.s_lse.release(); sl.s_ck.release();
+            sl.s_cv.release(); sl.s_bt.release(); sl.s_ws.release();
+            if (sl.in_done) cudaEventDestroy(sl.in_done);
+            if (sl.k_done) cudaEventDestroy(sl.k_done);
+            if (sl.out_done) cudaEventDestroy(sl.out_done);
+        }
+        if (h->st_in) cudaStreamDestroy(h->st_in);
+        if (h->st_out) cudaStreamDestroy(h->st_out);
     }
     delete h;
 }
@@ -761,12 +776,12 @@ int msa_forward_writeback(msa_handle h, msa_plan p, const void *q, int64_t total
                         softmax_scale, o, lse, workspace, workspace_bytes, cuda_stream, true);
 }
 
-int msa_forward_host(msa_handle h, msa_plan p, const void *q_host, int64_t total_q, const void *pool_k,
-                     const void *pool_v, int64_t num_blocks, const int32_t *block_table_host, int64_t block_table_len,
-                     const void *contig_k_host, const void *contig_v_host, int64_t contig_rows, float softmax_scale,
-                     void *o_host, float *lse_host, void *cuda_stream)
+int msa_forward_host_async(msa_handle h, msa_plan p, const void *q_host, int64_t total_q, const void *pool_k,
+                           const void *pool_v, int64_t num_blocks, const int32_t *block_table_host, int64_t block_table_len,
+                           const void *contig_k_host, const void *contig_v_host, int64_t contig_rows, float softmax_scale,
+                           void *o_host, float *lse_host, void *cuda_stream, int32_t slot)
 {
-    if (!h || !p || p->h != h) return MSA_ERR_INVALID_ARG;
+    if (!h || !p || p->h != h || slot < 0 || slot > 1) return MSA_ERR_INVALID_ARG;
     if (h->planning_only) return MSA_ERR_NO_DEVICE;
     if (total_q < 0 || block_table_len < 0 || contig_rows < 0) return MSA_ERR_INVALID_ARG;
     if (total_q > 0 && (!q_host || !o_host || !lse_host)) return MSA_ERR_INVALID_ARG;
@@ -781,29 +796,67 @@ int msa_forward_host(msa_handle h, msa_plan p, const void *q_host, int64_t total
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     DeviceGuard guard(h->cfg.device);
     if (guard.err != cudaSuccess) return cuda_fail(guard.err, "msa_forward_host: cudaSetDevice");
-    MSA_CUDA(h->s_q.reserve(b_q + 16));
-    MSA_CUDA(h->s_o.reserve(b_q + 16));
-    MSA_CUDA(h->s_lse.reserve(b_lse + 16));
-    MSA_CUDA(h->s_ck.reserve(b_c + 16));
-    MSA_CUDA(h->s_cv.reserve(b_c + 16));
-    MSA_CUDA(h->s_bt.reserve(b_bt + 16));
-    MSA_CUDA(h->s_ws.reserve(b_ws + 16));
-    if (b_q) MSA_CUDA(cudaMemcpyAsync(h->s_q.p, q_host, b_q, cudaMemcpyHostToDevice, stream));
-    if (b_bt) MSA_CUDA(cudaMemcpyAsync(h->s_bt.p, block_table_host, b_bt, cudaMemcpyHostToDevice, stream));
+    if (!h->st_in) MSA_CUDA(cudaStreamCreateWithFlags(&h->st_in, cudaStreamNonBlocking));
+    if (!h->st_out) MSA_CUDA(cudaStreamCreateWithFlags(&h->st_out, cudaStreamNonBlocking));
+    msa_handle_s::HostSlot &sl = h->hs[slot];
+    if (!sl.in_done) MSA_CUDA(cudaEventCreateWithFlags(&sl.in_done, cudaEventDisableTiming));
+    if (!sl.k_done) MSA_CUDA(cudaEventCreateWithFlags(&sl.k_done, cudaEventDisableTiming));
+    if (!sl.out_done) MSA_CUDA(cudaEventCreateWithFlags(&sl.out_done, cudaEventDisableTiming));
+    // the slot's last call must be over before its staging buffers (and the caller's output buffers) are used again
+    if (sl.busy) MSA_CUDA(cudaEventSynchronize(sl.out_done));
+    sl.busy = false;
+    MSA_CUDA(sl.s_q.reserve(b_q + 16));
+    MSA_CUDA(sl.s_o.reserve(b_q + 16));
+    MSA_CUDA(sl.s_lse.reserve(b_lse + 16));
+    MSA_CUDA(sl.s_ck.reserve(b_c + 16));
+    MSA_CUDA(sl.s_cv.reserve(b_c + 16));
+    MSA_CUDA(sl.s_bt.reserve(b_bt + 16));
+    MSA_CUDA(sl.s_ws.reserve(b_ws + 16));
+    if (b_q) MSA_CUDA(cudaMemcpyAsync(sl.s_q.p, q_host, b_q, cudaMemcpyHostToDevice, h->st_in));
+    if (b_bt) MSA_CUDA(cudaMemcpyAsync(sl.s_bt.p, block_table_host, b_bt, cudaMemcpyHostToDevice, h->st_in));
     if (b_c) {
-        MSA_CUDA(cudaMemcpyAsync(h->s_ck.p, contig_k_host, b_c, cudaMemcpyHostToDevice, stream));
-        MSA_CUDA(cudaMemcpyAsync(h->s_cv.p, contig_v_host, b_c, cudaMemcpyHostToDevice, stream));
+        MSA_CUDA(cudaMemcpyAsync(sl.s_ck.p, contig_k_host, b_c, cudaMemcpyHostToDevice, h->st_in));
+        MSA_CUDA(cudaMemcpyAsync(sl.s_cv.p, contig_v_host, b_c, cudaMemcpyHostToDevice, h->st_in));
     }
-    int rc = msa_forward(h, p, h->s_q.p, total_q, pool_k, pool_v, num_blocks, static_cast<const int32_t *>(h->s_bt.p),
-                         block_table_len, h->s_ck.p, h->s_cv.p, contig_rows, softmax_scale, h->s_o.p,
-                         static_cast<float *>(h->s_lse.p), h->s_ws.p, h->s_ws.cap, stream);
+    MSA_CUDA(cudaEventRecord(sl.in_done, h->st_in));
+    MSA_CUDA(cudaStreamWaitEvent(stream, sl.in_done, 0));
+    int rc = msa_forward(h, p, sl.s_q.p, total_q, pool_k, pool_v, num_blocks, static_cast<const int32_t *>(sl.s_bt.p),
+                         block_table_len, sl.s_ck.p, sl.s_cv.p, contig_rows, softmax_scale, sl.s_o.p,
+                         static_cast<float *>(sl.s_lse.p), sl.s_ws.p, sl.s_ws.cap, stream);
     if (rc != MSA_OK) return rc;
+    MSA_CUDA(cudaEventRecord(sl.k_done, stream));
+    MSA_CUDA(cudaStreamWaitEvent(h->st_out, sl.k_done, 0));
     if (b_q) {
-        MSA_CUDA(cudaMemcpyAsync(o_host, h->s_o.p, b_q, cudaMemcpyDeviceToHost, stream));
-        MSA_CUDA(cudaMemcpyAsync(lse_host, h->s_lse.p, b_lse, cudaMemcpyDeviceToHost, stream));
+        MSA_CUDA(cudaMemcpyAsync(o_host, sl.s_o.p, b_q, cudaMemcpyDeviceToHost, h->st_out));
+        MSA_CUDA(cudaMemcpyAsync(lse_host, sl.s_lse.p, b_lse, cudaMemcpyDeviceToHost, h->st_out));
     }
-    MSA_CUDA(cudaStreamSynchronize(stream));
+    MSA_CUDA(cudaEventRecord(sl.out_done, h->st_out));
+    sl.busy = true;
     return MSA_OK;
+}
+
+int msa_forward_host_wait(msa_handle h, int32_t slot)
+{
+    if (!h || slot < 0 || slot > 1) return MSA_ERR_INVALID_ARG;
+    if (h->planning_only) return MSA_ERR_NO_DEVICE;
+    msa_handle_s::HostSlot &sl = h->hs[slot];
+    if (!sl.busy) return MSA_OK;
+    DeviceGuard guard(h->cfg.device);
+    if (guard.err != cudaSuccess) return cuda_fail(guard.err, "msa_forward_host_wait: cudaSetDevice");
+    MSA_CUDA(cudaEventSynchronize(sl.out_done));
+    sl.busy = false;
+    return MSA_OK;
+}
+
+int msa_forward_host(msa_handle h, msa_plan p, const void *q_host, int64_t total_q, const void *pool_k,
+                     const void *pool_v, int64_t num_blocks, const int32_t *block_table_host, int64_t block_table_len,
+                     const void *contig_k_host, const void *contig_v_host, int64_t contig_rows, float softmax_scale,
+                     void *o_host, float *lse_host, void *cuda_stream)
+{
+    int rc = msa_forward_host_async(h, p, q_host, total_q, pool_k, pool_v, num_blocks, block_table_host, block_table_len, contig_k_host,
+                                    contig_v_host, contig_rows, softmax_scale, o_host, lse_host, cuda_stream, 0);
+    if (rc != MSA_OK) return rc;
+    return msa_forward_host_wait(h, 0);
 }
 
 int msa_append_plan_create(msa_handle h, const msa_append *jobs, int32_t n_jobs, msa_append_plan *out)

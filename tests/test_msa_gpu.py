@@ -14,7 +14,7 @@ import oracle
 import workloads as W
 from paper_2606_02964_b200 import (MsaError, MsaSession, MSA_ERR_MISALIGNED, MSA_ERR_OUT_OF_RANGE,
                                    MSA_ERR_WORKSPACE, make_descriptors, msa_create, msa_destroy, msa_forward,
-                                   msa_forward_host, msa_last_launch_count, msa_plan_create, msa_plan_destroy, msa_plan_export,
+                                   msa_forward_host, msa_forward_host_async, msa_forward_host_wait, msa_last_launch_count, msa_plan_create, msa_plan_destroy, msa_plan_export,
                                    msa_workspace_bytes)
 from workloads import SEG_CONTIG, SEG_PAGED, SEG_SELF, ContextSpec, RunSpec, build_problem
 
@@ -493,3 +493,30 @@ def test_f1_hybrid_prefill_plus_decode_full_size_plan_aligned_rows():
 def test_f3_policy_trace_full_size_plan_aligned_rows():
     """Residency decided by the evictor (Algorithm 1): shared prefix and suffix cached, middle recomputed."""
     _full_config_sampled("f3_policy_trace", 10, 4, 7)
+
+
+def test_host_buffer_call_two_steps_in_flight():
+    """msa_forward_host_async / _wait on both slots, calls overlapping: every call's O / LSE equal msa_forward's, bit for bit."""
+    p = W.random_problem(77, n_req=4, Hq=8, Hkv=2, D=128, max_ctx=900, max_q=120, device=DEV)
+    with MsaSession(p) as s:
+        o_ref, l_ref = s.forward()
+        torch.cuda.synchronize()
+        o_ref, l_ref = o_ref.cpu(), l_ref.cpu()
+        qh, bt = p.q.cpu().pin_memory(), p.block_table.cpu().pin_memory()
+        ck, cv = p.contig_k.cpu().pin_memory(), p.contig_v.cpu().pin_memory()
+        oh = [torch.zeros_like(qh).pin_memory() for _ in range(2)]
+        lh = [torch.zeros(p.total_q, p.Hq, dtype=torch.float32).pin_memory() for _ in range(2)]
+        st = torch.cuda.current_stream().cuda_stream
+        for i in range(6):
+            oh[i & 1].zero_()
+            msa_forward_host_async(s.h, s.plan, qh, p.pool_k, p.pool_v, bt, ck, cv, p.scale, oh[i & 1], lh[i & 1], st, i & 1)
+            if i > 0:
+                msa_forward_host_wait(s.h, (i - 1) & 1)
+                assert torch.equal(oh[(i - 1) & 1], o_ref) and torch.equal(lh[(i - 1) & 1], l_ref)
+        msa_forward_host_wait(s.h, 1)
+        assert torch.equal(oh[1], o_ref) and torch.equal(lh[1], l_ref)
+        msa_forward_host_wait(s.h, 0)          # nothing in flight: returns at once
+        # the blocking call is the same thing on slot 0
+        oh[0].zero_()
+        msa_forward_host(s.h, s.plan, qh, p.pool_k, p.pool_v, bt, ck, cv, p.scale, oh[0], lh[0], st)
+        assert torch.equal(oh[0], o_ref) and torch.equal(lh[0], l_ref)
