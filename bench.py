@@ -650,10 +650,23 @@ def run_kv_append(args):
     msa_plan_destroy(plan)
     msa_append_plan_destroy(ap)
     msa_destroy(h)
+    # the same jobs into an fp8 (E4M3) pool: the rows are quantised on the way (2 bytes read, 1 written per element)
+    from paper_2606_02964_b200 import MSA_POOL_FP8_E4M3
+    scales = np.full(p.Hkv, 2.0 ** -6, np.float32)
+    h8 = msa_create(p.Hq, p.Hkv, p.D, p.q_to_kv, device=0, pool_format=MSA_POOL_FP8_E4M3, k_scale=scales, v_scale=scales)
+    ap8 = msa_append_plan_create(h8, jobs)
+    pk8 = torch.zeros(tuple(pool_k.shape), dtype=torch.uint8, device=dev)
+    pv8 = torch.zeros(tuple(pool_v.shape), dtype=torch.uint8, device=dev)
+    ms8 = timed(lambda: msa_kv_append(h8, ap8, p.contig_k, p.contig_v, pk8, pv8, bt, stream))
+    nbytes8 = 1.5 * tokens * p.Hkv * p.D * 2 * 2
+    msa_append_plan_destroy(ap8)
+    msa_destroy(h8)
     print(json.dumps(dict(metric="msa_kv_append_hbm_gbs", value=gbs, unit="GB/s", n_gpus=1, steps=args.steps, warmup=max(3, args.warmup),
                           ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="bf16", data="synthetic",
                           config=dict(workload="kv_append", tokens=tokens, jobs=len(jobs), bytes_per_step=nbytes,
                                       l2_policy="working set %.0f MB per step (read + write), larger than L2" % (nbytes / 1e6)),
+                          fp8_pool=dict(ms_per_step=ms8, bytes_per_step=nbytes8, gbs=nbytes8 / (ms8 * 1e-3) / 1e9,
+                                        frac=nbytes8 / (ms8 * 1e-3) / 1e9 / gbs_peak, kernel="msa_kv_append_q8_kernel"),
                           clocks=clocks, gpu_launches=args.steps,
                           fused=dict(forward_only_ms=fwd_only, forward_plus_kv_append_ms=two, forward_writeback_ms=fused,
                                      writeback_cost_ms=fused - fwd_only, separate_cost_ms=two - fwd_only,

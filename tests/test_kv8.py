@@ -310,3 +310,19 @@ def test_kv8_append_quantises_like_the_oracle_and_feeds_the_forward():
     p2.seg_kind, p2.seg_block_off, p2.num_blocks = kind2, boff2, n_pool + extra
     o, lse, _ = gpu_forward(p2)
     compare(p2, o, lse, strict=False)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("want", ["prepass", "kernel_split"])
+def test_kv8_host_buffer_call_equals_the_device_call(want):
+    """msa_forward_host on an fp8 handle (the pool stays on the device; the pre-pass's copy lives in the handle's staging workspace)."""
+    from paper_2606_02964_b200 import msa_forward_host
+    p8 = W.to_fp8_pool(_three_paths(DEV)[want], k_exp=[-6, -4], v_exp=[-5, -7])
+    with MsaSession(p8) as s:
+        o_ref, l_ref = s.forward()
+        torch.cuda.synchronize()
+        qh, bt = p8.q.cpu().pin_memory(), p8.block_table.cpu().pin_memory()
+        ck, cv = p8.contig_k.cpu().pin_memory(), p8.contig_v.cpu().pin_memory()
+        oh, lh = torch.zeros_like(qh).pin_memory(), torch.zeros(p8.total_q, p8.Hq, dtype=torch.float32).pin_memory()
+        msa_forward_host(s.h, s.plan, qh, p8.pool_k, p8.pool_v, bt, ck, cv, p8.scale, oh, lh, torch.cuda.current_stream().cuda_stream)
+        assert torch.equal(oh, o_ref.cpu()) and torch.equal(lh, l_ref.cpu())
