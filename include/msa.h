@@ -69,13 +69,15 @@ enum { MSA_SEG_PAGED = 0, MSA_SEG_CONTIG = 1, MSA_SEG_SELF = 2 };
  *                      infinity, S.1111.111 = NaN), and one scale per KV head for K and one for V:
  *                          K_j[kvh][d] = e4m3(pool_k byte) * k_scale[kvh],   V_j[kvh][d] = e4m3(pool_v byte) * v_scale[kvh]
  *                      The scales must be powers of two in [2^-14, 2^7] (as in the OCP MX formats): the dequantised
- *                      value is then exactly a bf16 and the kernels multiply exactly that value (converted on chip to bf16,
- *                      or to f16 with the scale applied outside the MMA): same tolerances as the bf16 pool.  A launch of short queries reads every
- *                      cached byte once and converts it in the forward kernel; a launch with prefill chunks, which loads
- *                      a cached tile once per q-tile group, first dequantises the blocks it refers to into the workspace
- *                      (once) and runs the bf16 kernel on that copy -- decided by the plan (msa_workspace_bytes grows
- *                      accordingly), invisible in the results.  A NaN code dequantises to an
- *                      unspecified finite value (non-finite K/V are outside the definition, DESIGN.md c19). */
+ *                      value is then exactly a bf16, and the kernels multiply exactly that value (converted on chip
+ *                      to bf16, or to f16 with the scale applied outside the MMA): same tolerances as the bf16 pool.
+ *                      The plan decides how a launch is served, invisibly in the results: a launch of short queries
+ *                      reads every cached byte once and converts it inside the forward kernel; a launch with prefill
+ *                      chunks, which loads a cached tile once per q-tile group, first dequantises the blocks it refers
+ *                      to into the workspace, once, and runs the bf16 kernel on that copy (msa_workspace_bytes grows
+ *                      accordingly).  Arena values beyond 65504 * scale saturate in the short-query variant (it
+ *                      multiplies in f16; E4M3 with that scale tops out at 448 * scale).  A NaN code dequantises to
+ *                      an unspecified finite value (non-finite K/V are outside the definition, DESIGN.md c19). */
 enum { MSA_POOL_BF16 = 0, MSA_POOL_FP8_E4M3 = 1 };
 
 typedef struct {
