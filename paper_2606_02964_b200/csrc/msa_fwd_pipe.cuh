@@ -273,7 +273,7 @@ __device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uin
 // barrier for every entry.  An entry is waited for even when there is nothing to convert: a waiter that skips a use
 // of a slot cannot tell the phases of its barrier apart.
 // f16 variant: 16-byte chunks [first, n) in steps of stride * 32 of a shared-memory region, bf16 -> f16 in place, times `mult`
-// (a power of two or 1: exact unless the result leaves the f16 range).
+// (a power of two or 1: exact unless the result leaves the f16 range; beyond +-65504 it saturates).
 __device__ __forceinline__ void bf16_to_f16_inplace(uint32_t base, int n_chunks, int first, int stride, int lane, float mult)
 {
     for (int i = first * 32 + lane; i < n_chunks; i += stride * 32) {
@@ -281,7 +281,7 @@ __device__ __forceinline__ void bf16_to_f16_inplace(uint32_t base, int n_chunks,
         asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "r"(base + i * 16u));
 #pragma unroll
         for (int k = 0; k < 4; ++k)
-            w[k] = pack_f16x2(__uint_as_float(w[k] << 16) * mult, __uint_as_float(w[k] & 0xffff0000u) * mult);
+            w[k] = pack_f16x2_sat(__uint_as_float(w[k] << 16) * mult, __uint_as_float(w[k] & 0xffff0000u) * mult);
         asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(base + i * 16u), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]) : "memory");
     }
 }
@@ -397,7 +397,7 @@ __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkU
                         for (int k = 0; k < kPerLane; ++k) {
 #pragma unroll
                             for (int j = 0; j < 4; ++j)
-                                w[k][j] = pack_f16x2(__uint_as_float(w[k][j] << 16) * mult, __uint_as_float(w[k][j] & 0xffff0000u) * mult);
+                                w[k][j] = pack_f16x2_sat(__uint_as_float(w[k][j] << 16) * mult, __uint_as_float(w[k][j] & 0xffff0000u) * mult);
                             asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr[k]), "r"(w[k][0]), "r"(w[k][1]), "r"(w[k][2]), "r"(w[k][3]) : "memory");
                         }
                     } else {

@@ -315,6 +315,13 @@ __device__ __forceinline__ uint32_t pack_f16x2(float lo, float hi)
     asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
     return r;
 }
+// ... saturating at +-65504 instead of overflowing to infinity (operands that come from caller data)
+__device__ __forceinline__ uint32_t pack_f16x2_sat(float lo, float hi)
+{
+    uint32_t r;
+    asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
 // Packed fp32 pairs (sm_100 FFMA2 / FADD2): one issue slot for two lanes of the softmax row.
 __device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c)
 {
