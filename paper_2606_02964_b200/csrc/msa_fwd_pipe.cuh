@@ -293,8 +293,14 @@ __device__ __forceinline__ void bf16_to_f16_inplace(uint32_t base, int n_chunks,
 template <class C, int D, bool F16>
 __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkUnit &wu, uint32_t bar0, uint32_t sQ, uint32_t sStg,
                                                  uint32_t sRing, int lane, uint32_t it_mask, int even_w, int cw_first, int cw_stride,
-                                                 uint32_t &cv_ent, uint32_t &cv_stg, uint32_t &cv_phq, uint32_t &dir_par)
+                                                 uint32_t &cv_ent, uint32_t &cv_stg, uint32_t &cv_phq, uint32_t &dir_par, bool trace = false)
 {
+#if defined(MSA_PROF) && MSA_PROF == 2
+#define CV_TRACE(step, ev) do { if (trace && (step) < 64) g_trace[3][step][ev] = clock64(); } while (0)
+#else
+#define CV_TRACE(step, ev)
+    (void)trace;
+#endif
     auto bar = [bar0](int i) { return bar0 + static_cast<uint32_t>(i) * 8u; };
     const int n = wu.tile_end - wu.tile_begin;
     const bool pair = wu.mode == kModePair;
@@ -348,6 +354,7 @@ __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkU
             mbar_wait(bar(kBarKvEmpty + slot), ((cv_ent / C::kStages) & 1u) ^ 1u);
             PROF_ADD(21);
         }
+        CV_TRACE(e, 0);
         if (m_paged != 0) {
             const uint32_t st = cv_stg % static_cast<uint32_t>(C::kStgDiv);
             {
@@ -355,6 +362,7 @@ __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkU
                 mbar_wait(bar(kBarStgFull + st), (cv_stg / C::kStgDiv) & 1u);
                 PROF_ADD(22);
             }
+            CV_TRACE(e, 1);
             PROF_T0();
             kv8_convert_tile<D, F16>(sStg + st * C::kStgTileBytes, sRing + slot * C::kTileBytes, m_paged, cur, is_v ? mul_v : mul_k,
                                      it_mask, even_w, lane);
@@ -378,6 +386,29 @@ __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkU
             if (m_dir != 0 && cw_first >= 0) {
                 const float mult = is_v ? inv_v : inv_k;
                 const uint32_t tile = sRing + slot * C::kTileBytes;
+                if (m_dir == 0xffu && m_full == 0xffu && cw_stride == kConvWarps) {
+                    // a tile of eight full arena blocks (the inside of a recomputed run): the whole slot, flat -- the 64-element
+                    // halves follow each other -- in 16-byte chunks, a warp's share interleaved with the others', four loads in
+                    // flight, every address a constant away from the lane's first
+                    constexpr int kChunks = C::kTileBytes / 16, kPerLane = kChunks / (kConvWarps * 32);
+                    const uint32_t a0 = tile + static_cast<uint32_t>((cw_first * 32 + lane) * 16);
+#pragma unroll
+                    for (int k0 = 0; k0 < kPerLane; k0 += 4) {
+                        uint32_t w[4][4];
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)
+                            asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(w[k][0]), "=r"(w[k][1]), "=r"(w[k][2]), "=r"(w[k][3])
+                                         : "r"(a0 + (k0 + k) * (kConvWarps * 32 * 16)));
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+#pragma unroll
+                            for (int j = 0; j < 4; ++j)
+                                w[k][j] = pack_f16x2_sat(__uint_as_float(w[k][j] << 16) * mult, __uint_as_float(w[k][j] & 0xffff0000u) * mult);
+                            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a0 + (k0 + k) * (kConvWarps * 32 * 16)), "r"(w[k][0]),
+                                         "r"(w[k][1]), "r"(w[k][2]), "r"(w[k][3]) : "memory");
+                        }
+                    }
+                } else
 #pragma unroll 1
                 for (int b = 0; b < kVbPerTile; ++b) {
                     if (!((m_dir >> b) & 1u)) continue;
@@ -412,6 +443,7 @@ __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkU
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar(kBarKvFull + slot));
+        CV_TRACE(e, 2);
         ++cv_ent;
         cur = nxt;
     }
@@ -700,7 +732,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             if constexpr (KV8) {
                 // ---- converters (kv8_convert_unit): warp w of the four takes every fourth warp iteration of a tile
                 kv8_convert_unit<C, D, F16>(P, wu, bar0, sQ, sStg, sRing, lane, 0x11111111u << (warp - 8), warp - 8, warp - 8, 4, cv_ent,
-                                            cv_stg, cv_phq, cv_dirpar);
+                                            cv_stg, cv_phq, cv_dirpar, blockIdx.x == 0 && u == u_begin && warp == 9 && lane == 0);
             }
             const int n_out = pair ? 2 : 1;                       // q tiles written by this unit
             for (int qt = 0; qt < n_out; ++qt) {
@@ -1174,14 +1206,20 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                     if (n <= 2) umma_commit(bar(kBarQEmpty));
                     for (int j = 0; j < n; ++j) {
                         const int c = j & 1;
+                        tr_step = j;
+                        PROF_TRACE(0, j, 0);
                         const uint32_t vs = take_v();
+                        PROF_TRACE(0, j, 1);
                         pv(c, vs, j < 2);
+                        PROF_TRACE(0, j, 2);
                         umma_commit(bar(kBarKvEmpty + vs));
                         if (j + 2 >= n) umma_commit(bar(kBarOFull + c));
                         if (j + 2 < n) {
                             ks = take_k();
+                            PROF_TRACE(0, j, 3);
                             tc_fence_after();
                             qk(c, 0, ks);
+                            PROF_TRACE(0, j, 4);
                             umma_commit(bar(kBarKvEmpty + ks));
                             if (j + 3 == n) umma_commit(bar(kBarQEmpty));
                         }
