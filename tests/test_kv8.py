@@ -326,3 +326,19 @@ def test_kv8_host_buffer_call_equals_the_device_call(want):
         oh, lh = torch.zeros_like(qh).pin_memory(), torch.zeros(p8.total_q, p8.Hq, dtype=torch.float32).pin_memory()
         msa_forward_host(s.h, s.plan, qh, p8.pool_k, p8.pool_v, bt, ck, cv, p8.scale, oh, lh, torch.cuda.current_stream().cuda_stream)
         assert torch.equal(oh, o_ref.cpu()) and torch.equal(lh, l_ref.cpu())
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name,want", [("cfg4_mixed", "prepass"), ("f1_hybrid_pod", "kernel_pair")])
+def test_kv8_full_size_sampled_rows_on_the_other_paths(name, want):
+    """The largest config through the dequantising pre-pass and the mixed prefill + decode batch through the two-Q-tile kernel
+    variant (the launches `bench.py --workload <name>_kv8` times), on a row sample of a few runs."""
+    base = {**W.CONFIGS, **W.EXTRA_CONFIGS}[name](device=DEV)
+    p8 = W.to_fp8_pool(base)
+    del base
+    assert _kv8_path(p8, device=0)[0] == want
+    o, lse, _ = gpu_forward(p8)
+    reqs = list(range(0, p8.n_req, max(1, p8.n_req // 6)))[:6]
+    rr, ii = W.pick_rows(p8, n_random=6, seed=5, reqs=reqs)
+    mx, mean, dl = compare(p8, o, lse, rr, ii)
+    print(f"{name}_kv8 ({want}): {len(rr)} rows x {p8.Hq} heads compared, max|dO|={mx:.3e} mean|dO|={mean:.3e} max|dLSE|={dl:.3e}")
