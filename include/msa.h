@@ -53,7 +53,9 @@ enum {
     MSA_ERR_MISALIGNED = -6,       /* device pointer not 16-byte aligned */
     MSA_ERR_WORKSPACE = -7,        /* workspace NULL / too small */
     MSA_ERR_CUDA = -8,             /* a CUDA runtime / driver call failed (see msa_last_cuda_error) */
-    MSA_ERR_NO_DEVICE = -9         /* no CUDA device, or the device is not sm_100 */
+    MSA_ERR_NO_DEVICE = -9,        /* no CUDA device, or the device is not sm_100 */
+    MSA_ERR_STATIC_WS = -10        /* msa_forward_static_ws: the plan needs more scratch than MSA_STATIC_WS_BYTES (or the
+                                      device ordinal is beyond the 64 the built-in scratch is tracked for) */
 };
 
 /* Segment kinds (BASELINE.json north_star):
@@ -191,6 +193,48 @@ int msa_forward(msa_handle h, msa_plan p,
                 float softmax_scale,
                 void *o, float *lse,
                 void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* ---- msa_forward without a workspace argument: the scratch is built into the library ----
+ * Who this is for.  msa_forward wants `workspace` bytes from the caller, and a caller normally gets them from cudaMalloc.
+ * Two kinds of caller of this library cannot do that at step time:
+ *   - a serving engine that sized its paged KV pool to whatever HBM was free at start-up (the pool's size is what decides
+ *     how much context stays resident): nothing is left for cudaMalloc to hand out later, and the
+ *     workspace size changes with every batch's split-KV schedule, so it cannot be sized once either;
+ *   - code that runs while other streams have steps in flight and must not stall them: cudaMalloc and cudaFree
+ *     synchronise the whole device, and some hosts (a plugin inside another framework's memory manager) are simply not
+ *     allowed to call them.
+ * For them the library carries MSA_STATIC_WS_BYTES of device memory of its own -- a fixed array inside libmsa.so's device
+ * image -- and this call uses it as the workspace: split-KV partials written by the forward kernel and read by the LSE-merge
+ * kernel, and on an fp8 handle the bf16 copy of the cached blocks a prefill launch dequantises first.
+ *
+ * Arguments, results and status codes are those of msa_forward (same kernels, bit-identical O / LSE), minus `workspace` /
+ * `workspace_bytes`.  A plan whose msa_workspace_bytes() exceeds MSA_STATIC_WS_BYTES is refused with MSA_ERR_STATIC_WS and
+ * nothing is launched (32 MiB covers every bf16-pool batch of BASELINE.json: the largest, cfg3, needs 26.7 MiB; an fp8
+ * prefill plan that copies more than that much of the pool does not fit -- use msa_forward there).
+ *
+ * Cost: every GPU on which the array's module gets loaded gives up MSA_STATIC_WS_BYTES until the process exits, whether
+ * or not this call is ever used again.
+ *
+ * The call itself allocates no device memory and frees none (no cudaMalloc / cudaFree / cudaMallocAsync, no library
+ * routine that allocates; msa_create and msa_plan_create, which own small device buffers, are set-up calls and are not
+ * covered by this promise).  The FIRST call on a device does a one-time set-up: it looks up the array's device address
+ * (which makes the CUDA runtime load that part of the library, and that is where the 32 MiB are actually reserved) and
+ * reserves the handle's host-side tensor-map table.  Make that first call at start-up, on any small split-KV or ordinary
+ * plan, before the engine takes the rest of the memory and before any stream capture is begun.
+ *
+ * Sharing: there is ONE array per device, shared by every handle, plan and thread of the process.  Two calls that may
+ * run on the GPU at the same time (different streams, or different threads without ordering) overwrite each other's
+ * partials: issue them on one stream, or order them with events.  The array keeps whatever the last call left in it.
+ * Nothing in it has to start at zero -- every float the merge kernel reads was written by the forward kernel of the same
+ * call, and the fp8 copy and its index table are rewritten in full by the pre-pass -- so the call clears nothing. */
+#define MSA_STATIC_WS_BYTES (32u << 20)
+int msa_forward_static_ws(msa_handle h, msa_plan p,
+                          const void *q, int64_t total_q,
+                          const void *pool_k, const void *pool_v, int64_t num_blocks,
+                          const int32_t *block_table, int64_t block_table_len,
+                          const void *contig_k, const void *contig_v, int64_t contig_rows,
+                          float softmax_scale,
+                          void *o, float *lse, void *cuda_stream);
 
 /* End-to-end convenience call with HOST buffers for everything a serving step produces:
  * q, the block table, the contiguous arena (recomputed runs + own chunk) come from host

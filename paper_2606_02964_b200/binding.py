@@ -17,6 +17,8 @@ from ._build import LIB_PATH
 MSA_OK = 0
 MSA_ERR_INVALID_ARG, MSA_ERR_UNSUPPORTED, MSA_ERR_OVERLAP, MSA_ERR_UNSORTED = -1, -2, -3, -4
 MSA_ERR_OUT_OF_RANGE, MSA_ERR_MISALIGNED, MSA_ERR_WORKSPACE, MSA_ERR_CUDA, MSA_ERR_NO_DEVICE = -5, -6, -7, -8, -9
+MSA_ERR_STATIC_WS = -10
+MSA_STATIC_WS_BYTES = 32 << 20
 MSA_SEG_PAGED, MSA_SEG_CONTIG, MSA_SEG_SELF = 0, 1, 2
 MSA_POOL_BF16, MSA_POOL_FP8_E4M3 = 0, 1
 
@@ -61,7 +63,8 @@ EXPORTS = ["msa_create", "msa_destroy", "msa_plan_create", "msa_plan_destroy", "
            "msa_plan_export", "msa_workspace_bytes", "msa_forward", "msa_forward_host",
            "msa_last_launch_count", "msa_set_timing", "msa_get_timing", "msa_strerror", "msa_last_cuda_error", "msa_version",
            "msa_append_plan_create", "msa_append_plan_destroy", "msa_kv_append",
-           "msa_plan_create_writeback", "msa_forward_writeback", "msa_forward_host_async", "msa_forward_host_wait"]
+           "msa_plan_create_writeback", "msa_forward_writeback", "msa_forward_host_async", "msa_forward_host_wait",
+           "msa_forward_static_ws"]
 EVICTOR_EXPORTS = ["msa_evictor_create", "msa_evictor_destroy", "msa_evictor_add", "msa_evictor_remove", "msa_evictor_evict",
                    "msa_evictor_evict_linear", "msa_evictor_set_lambda", "msa_evictor_size", "msa_evictor_weight"]
 
@@ -95,6 +98,7 @@ def _lib() -> ctypes.CDLL:
         lib.msa_workspace_bytes.argtypes = [vp, ctypes.POINTER(sz)]
         lib.msa_forward.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, i64, f32, vp, vp, vp, sz, vp]
         lib.msa_forward_host.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, i64, f32, vp, vp, vp]
+        lib.msa_forward_static_ws.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, i64, f32, vp, vp, vp]
         lib.msa_forward_host_async.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, i64, f32, vp, vp, vp, i32]
         lib.msa_forward_host_wait.argtypes = [vp, i32]
         lib.msa_last_launch_count.argtypes = [vp]
@@ -241,6 +245,21 @@ def msa_forward(h, p, q, pool_k, pool_v, block_table, contig_k, contig_v, softma
     _check(_lib().msa_forward(h, p, _dptr(q), total_q, _dptr(pool_k), _dptr(pool_v), num_blocks, _dptr(block_table),
                               bt_len, _dptr(contig_k), _dptr(contig_v), rows, ctypes.c_float(softmax_scale), _dptr(o),
                               _dptr(lse), _dptr(workspace), ws_bytes, stream), "msa_forward")
+
+
+def msa_forward_static_ws(h, p, q, pool_k, pool_v, block_table, contig_k, contig_v, softmax_scale: float, o, lse,
+                          stream: Optional[int] = None) -> None:
+    """msa_forward for a caller that cannot allocate the workspace (all HBM already belongs to its KV pool, or cudaMalloc is
+    off limits while steps are in flight): the library's built-in MSA_STATIC_WS_BYTES array is the workspace.  Raises
+    MsaError(MSA_ERR_STATIC_WS) when the plan needs more.  One array per device: calls that overlap on the GPU race."""
+    total_q = int(q.shape[0])
+    num_blocks = 0 if pool_k is None else int(pool_k.shape[0])
+    bt_len = 0 if block_table is None else int(block_table.numel())
+    rows = 0 if contig_k is None else int(contig_k.shape[0])
+    _check(_lib().msa_forward_static_ws(h, p, _dptr(q), total_q, _dptr(pool_k), _dptr(pool_v), num_blocks,
+                                        _dptr(block_table), bt_len, _dptr(contig_k), _dptr(contig_v), rows,
+                                        ctypes.c_float(softmax_scale), _dptr(o), _dptr(lse), stream),
+           "msa_forward_static_ws")
 
 
 def msa_forward_host(h, p, q_host, pool_k, pool_v, block_table_host, contig_k_host, contig_v_host,

@@ -8,6 +8,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -170,6 +171,9 @@ const char *msa_strerror(int status)
     case MSA_ERR_WORKSPACE: return "workspace missing or too small";
     case MSA_ERR_CUDA: return "CUDA error";
     case MSA_ERR_NO_DEVICE: return "no sm_100 CUDA device (there is no CPU fallback)";
+    case MSA_ERR_STATIC_WS:
+        return "msa_forward_static_ws: the plan needs more scratch than the library's built-in array holds "
+               "(MSA_STATIC_WS_BYTES = 32 MiB); pass a workspace of your own to msa_forward";
     default: return "unknown status";
     }
 }
@@ -996,3 +1000,53 @@ int msa_get_timing(msa_handle h, int32_t *steps, double *fwd_ms_avg, double *mer
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------------
+// msa_forward_static_ws (include/msa.h): msa_forward for callers that cannot allocate the workspace -- an engine that has
+// already given all free HBM to its KV pool, or code that may not call cudaMalloc / cudaFree (they synchronise the device)
+// while steps are in flight.  The workspace is this array: part of the library's device image, one copy per device, held
+// from the moment the CUDA runtime loads this module on a device until the process ends.
+//
+// In host code `g_static_ws` is only a handle for the symbol, not a device address (handing it to a kernel would fault, or
+// quietly touch host memory on a system where the GPU can reach it): the device address comes from
+// cudaGetSymbolAddress, looked up once per device with that device current, and that pointer is what the forward and merge
+// kernels receive through their parameter structs.
+static __device__ __align__(256) unsigned char g_static_ws[MSA_STATIC_WS_BYTES];
+
+namespace {
+constexpr int kStaticWsMaxDevices = 64;
+std::mutex g_static_ws_mu;
+void *g_static_ws_ptr[kStaticWsMaxDevices] = {};     // device address of g_static_ws on device i; NULL = not looked up yet
+}  // namespace
+
+extern "C" int msa_forward_static_ws(msa_handle h, msa_plan p, const void *q, int64_t total_q, const void *pool_k,
+                                     const void *pool_v, int64_t num_blocks, const int32_t *block_table,
+                                     int64_t block_table_len, const void *contig_k, const void *contig_v, int64_t contig_rows,
+                                     float softmax_scale, void *o, float *lse, void *cuda_stream)
+{
+    if (!h || !p || p->h != h) return MSA_ERR_INVALID_ARG;
+    if (h->planning_only) return MSA_ERR_NO_DEVICE;
+    const int device = h->cfg.device;
+    if (device >= kStaticWsMaxDevices) return MSA_ERR_STATIC_WS;
+    const size_t need = p->ws_partials + 2 * p->ws_pool + p->ws_ident;
+    if (need > static_cast<size_t>(MSA_STATIC_WS_BYTES)) return MSA_ERR_STATIC_WS;      // refused before anything is launched
+    void *ws = nullptr;
+    {
+        DeviceGuard guard(device);      // the symbol's address differs per device: look it up with the handle's device current
+        if (guard.err != cudaSuccess) return cuda_fail(guard.err, "msa_forward_static_ws: cudaSetDevice");
+        std::lock_guard<std::mutex> lock(g_static_ws_mu);
+        if (!g_static_ws_ptr[device]) {
+            // one-time set-up on this device (the first call; documented to come before any stream capture)
+            void *ptr = nullptr;
+            MSA_CUDA(cudaGetSymbolAddress(&ptr, g_static_ws));
+            if (!ptr) return MSA_ERR_CUDA;
+            g_static_ws_ptr[device] = ptr;
+        }
+        ws = g_static_ws_ptr[device];
+        // host side of "allocates nothing": the handle's tensor-map table gets its full capacity on the handle's first call here,
+        // so that a later call with a new pointer set appends to it without touching the heap
+        if (h->map_cache.capacity() < kMapCacheEntries) h->map_cache.reserve(kMapCacheEntries);
+    }
+    return forward_impl(h, p, q, total_q, pool_k, pool_v, num_blocks, block_table, block_table_len, contig_k, contig_v, contig_rows,
+                        softmax_scale, o, lse, ws, static_cast<size_t>(MSA_STATIC_WS_BYTES), cuda_stream, false);
+}
