@@ -77,9 +77,12 @@ enum { MSA_SEG_PAGED = 0, MSA_SEG_CONTIG = 1, MSA_SEG_SELF = 2 };
  *                      reads every cached byte once and converts it inside the forward kernel; a launch with prefill
  *                      chunks, which loads a cached tile once per q-tile group, first dequantises the blocks it refers
  *                      to into the workspace, once, and runs the bf16 kernel on that copy (msa_workspace_bytes grows
- *                      accordingly).  Arena values beyond 65504 * scale saturate in the short-query variant (it
- *                      multiplies in f16; E4M3 with that scale tops out at 448 * scale).  A NaN code dequantises to
- *                      an unspecified finite value (non-finite K/V are outside the definition, DESIGN.md c19). */
+ *                      accordingly).  The short-query launch multiplies in f16: code * 2^k is exact in f16 for every
+ *                      legal scale, and q and the arena rows it meets are converted bf16 -> f16 as they are.  An fp8
+ *                      handle therefore asks |q|, |arena K|, |arena V| <= 65504 whatever the scales are (larger magnitudes
+ *                      saturate to +-65504; magnitudes below 2^-14 are rounded to a multiple of 2^-24).  A NaN code
+ *                      dequantises to an unspecified value, possibly NaN (non-finite K/V are outside the definition,
+ *                      DESIGN.md c19); codes in slots no query row can see never reach O. */
 enum { MSA_POOL_BF16 = 0, MSA_POOL_FP8_E4M3 = 1 };
 
 typedef struct {
@@ -171,6 +174,9 @@ int msa_workspace_bytes(msa_plan p, size_t *bytes);
 
 /* One MSA forward pass, asynchronous on `cuda_stream` (a cudaStream_t; NULL = default
  * stream).  Never allocates, never synchronises, never reads device memory on the host.
+ * Calls on ONE handle (msa_forward*, msa_kv_append, msa_set/get_timing) must not run concurrently on
+ * several host threads: the handle keeps the encoded tensor maps of the last 64 pointer sets and the
+ * launch counter.  Different handles are independent.
  *
  *   q            device bf16 [total_q][Hq][D]
  *   pool_k/v     device bf16 [num_blocks][16][Hkv][D]      (paged KV cache; E4M3 bytes of the same shape when the
@@ -218,9 +224,9 @@ int msa_forward(msa_handle h, msa_plan p,
  * The call itself allocates no device memory and frees none (no cudaMalloc / cudaFree / cudaMallocAsync, no library
  * routine that allocates; msa_create and msa_plan_create, which own small device buffers, are set-up calls and are not
  * covered by this promise).  The FIRST call on a device does a one-time set-up: it looks up the array's device address
- * (which makes the CUDA runtime load that part of the library, and that is where the 32 MiB are actually reserved) and
- * reserves the handle's host-side tensor-map table.  Make that first call at start-up, on any small split-KV or ordinary
- * plan, before the engine takes the rest of the memory and before any stream capture is begun.
+ * (which makes the CUDA runtime load that part of the library, and that is where the 32 MiB are actually reserved).
+ * Make that first call at start-up, on any small split-KV or ordinary plan, before the engine takes the rest of the
+ * memory and before any stream capture is begun.
  *
  * Sharing: there is ONE array per device, shared by every handle, plan and thread of the process.  Two calls that may
  * run on the GPU at the same time (different streams, or different threads without ordering) overwrite each other's

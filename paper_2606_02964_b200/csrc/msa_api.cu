@@ -78,6 +78,8 @@ struct DevBuf {
 
 }  // namespace
 
+constexpr size_t kMapCacheEntries = 64;
+
 struct msa_handle_s {
     msa_config cfg{};
     int G = 0, R = 0;
@@ -89,8 +91,7 @@ struct msa_handle_s {
     bool kv8 = false;                  // fp8 (E4M3) paged pool
     std::vector<float> kv_scale;       // kv8: [2][Hkv] K scales then V scales (powers of two)
     uint32_t *d_kv8_mul = nullptr;     // kv8: [2][Hkv] f16 bits of 2^k (forward kernel)
-    float *d_kv8_inv = nullptr;        // kv8: [2][Hkv] 1 / scale (quantising msa_kv_append; f16 short-query variant)
-    float *d_kv8_scale = nullptr;      // kv8: [2][Hkv] the scales
+    float *d_kv8_inv = nullptr;        // kv8: [2][Hkv] 1 / scale (quantising msa_kv_append)
     EncodeTiledFn encode = nullptr;
     // Tensor maps depend only on (base pointer, extent) of q / pool / arena: a model calls msa_forward once per
     // layer with the same few pointer sets step after step, so the 23 encoded maps are kept per pointer set.
@@ -125,6 +126,7 @@ struct msa_handle_s {
 
 struct msa_plan_s {
     msa_handle h = nullptr;
+    int device = -1;                       // the handle's ordinal, kept here: a plan may be destroyed after its handle
     HostPlan hp;
     void *d_buf = nullptr;
     const VBlock *d_vblocks = nullptr;
@@ -146,6 +148,7 @@ struct msa_plan_s {
 
 struct msa_append_plan_s {
     msa_handle h = nullptr;
+    int device = -1;               // as in msa_plan_s
     std::vector<AppendUnit> units;
     AppendUnit *d_units = nullptr;
     int64_t max_row = -1;          // extents the jobs need at msa_kv_append
@@ -264,8 +267,6 @@ int msa_create(const msa_config *cfg, msa_handle *out)
     if (kv8) {
         if (e == cudaSuccess) e = cudaMalloc(&h->d_kv8_mul, kv8_mul.size() * sizeof(uint32_t));
         if (e == cudaSuccess) e = cudaMemcpy(h->d_kv8_mul, kv8_mul.data(), kv8_mul.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
-        if (e == cudaSuccess) e = cudaMalloc(&h->d_kv8_scale, kv_scale.size() * sizeof(float));
-        if (e == cudaSuccess) e = cudaMemcpy(h->d_kv8_scale, kv_scale.data(), kv_scale.size() * sizeof(float), cudaMemcpyHostToDevice);
         if (e == cudaSuccess) e = cudaMalloc(&h->d_kv8_inv, kv8_inv.size() * sizeof(float));
         if (e == cudaSuccess) e = cudaMemcpy(h->d_kv8_inv, kv8_inv.data(), kv8_inv.size() * sizeof(float), cudaMemcpyHostToDevice);
     }
@@ -276,11 +277,11 @@ int msa_create(const msa_config *cfg, msa_handle *out)
         if (h->d_kv_to_q) cudaFree(h->d_kv_to_q);
         if (h->d_kv8_mul) cudaFree(h->d_kv8_mul);
         if (h->d_kv8_inv) cudaFree(h->d_kv8_inv);
-        if (h->d_kv8_scale) cudaFree(h->d_kv8_scale);
         delete h;
         return e != cudaSuccess ? cuda_fail(e, "msa_create") : MSA_ERR_NO_DEVICE;
     }
     h->encode = reinterpret_cast<EncodeTiledFn>(fn);
+    h->map_cache.reserve(kMapCacheEntries);      // msa_forward appends to it: no heap traffic on the hot path
     *out = h;
     return MSA_OK;
 }
@@ -293,7 +294,6 @@ void msa_destroy(msa_handle h)
         if (h->d_kv_to_q) cudaFree(h->d_kv_to_q);
         if (h->d_kv8_mul) cudaFree(h->d_kv8_mul);
         if (h->d_kv8_inv) cudaFree(h->d_kv8_inv);
-        if (h->d_kv8_scale) cudaFree(h->d_kv8_scale);
         for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
         for (auto &sl : h->hs) {
             if (sl.busy && sl.out_done) cudaEventSynchronize(sl.out_done);
@@ -352,6 +352,7 @@ int plan_create(msa_handle h, const msa_request *requests, int32_t n_req, const 
     msa_plan p = new (std::nothrow) msa_plan_s();
     if (!p) return MSA_ERR_INVALID_ARG;
     p->h = h;
+    p->device = h->cfg.device;
     int rc = build_plan(pc, requests, n_req, segments, n_seg, &p->hp, jobs, n_jobs);
     if (rc != MSA_OK) {
         delete p;
@@ -471,7 +472,7 @@ void msa_plan_destroy(msa_plan p)
 {
     if (!p) return;
     if (p->d_buf) {
-        DeviceGuard guard(p->h->cfg.device);
+        DeviceGuard guard(p->device);
         cudaFree(p->d_buf);
     }
     delete p;
@@ -566,8 +567,6 @@ int encode_2d_u8(msa_handle h, CUtensorMap *tm, const void *base, uint64_t inner
 }
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
-
-constexpr size_t kMapCacheEntries = 64;
 
 // The 23 tensor maps of one (q, pool, arena) pointer set, encoded once and kept in the handle.
 int cached_tensor_maps(msa_handle h, const HostPlan &hp_in, bool writeback, bool pool_fp8, const void *q, int64_t total_q,
@@ -685,7 +684,7 @@ int forward_impl(msa_handle h, msa_plan p, const void *q, int64_t total_q, const
     char *ws = static_cast<char *>(workspace);
     void *copy_k = p->deq ? ws + p->ws_partials : nullptr, *copy_v = p->deq ? ws + p->ws_partials + p->ws_pool : nullptr;
     int32_t *ident = p->deq ? reinterpret_cast<int32_t *>(ws + p->ws_partials + 2 * p->ws_pool) : nullptr;
-    const bool pool_fp8 = h->kv8 && !p->deq;
+    const bool pool_fp8 = h->kv8 && !p->deq && hp.uses_paged;     // no cached segment in the plan: nothing to convert, the bf16 kernel
     FwdParams fp;
     int rc = p->deq ? cached_tensor_maps(h, hp, false, false, q, total_q, copy_k, copy_v, static_cast<int64_t>(p->deq_src.size()), contig_k,
                                          contig_v, contig_rows, &fp)
@@ -701,8 +700,6 @@ int forward_impl(msa_handle h, msa_plan p, const void *q, int64_t total_q, const
     fp.tile_writer = writeback ? p->d_tile_writer : nullptr;
     fp.kv_to_q = h->d_kv_to_q;
     fp.kv8_mul = h->d_kv8_mul;
-    fp.kv8_scale = h->d_kv8_scale;
-    fp.kv8_inv = h->d_kv8_inv;
     fp.o = o;
     fp.lse = lse;
     fp.workspace = static_cast<float *>(workspace);
@@ -803,6 +800,17 @@ int msa_forward_host_async(msa_handle h, msa_plan p, const void *q_host, int64_t
     if (!h->st_in) MSA_CUDA(cudaStreamCreateWithFlags(&h->st_in, cudaStreamNonBlocking));
     if (!h->st_out) MSA_CUDA(cudaStreamCreateWithFlags(&h->st_out, cudaStreamNonBlocking));
     msa_handle_s::HostSlot &sl = h->hs[slot];
+    // a staging buffer that is about to be re-allocated takes the tensor maps encoded over it with it
+    if (b_q + 16 > sl.s_q.cap || b_c + 16 > sl.s_ck.cap || b_c + 16 > sl.s_cv.cap) {
+        const void *gone[3] = {sl.s_q.p, sl.s_ck.p, sl.s_cv.p};
+        h->map_cache.erase(std::remove_if(h->map_cache.begin(), h->map_cache.end(),
+                                          [&](const msa_handle_s::MapEntry &e) {
+                                              for (const void *g : gone)
+                                                  if (g && (e.key.q == g || e.key.contig_k == g || e.key.contig_v == g)) return true;
+                                              return false;
+                                          }),
+                           h->map_cache.end());
+    }
     if (!sl.in_done) MSA_CUDA(cudaEventCreateWithFlags(&sl.in_done, cudaEventDisableTiming));
     if (!sl.k_done) MSA_CUDA(cudaEventCreateWithFlags(&sl.k_done, cudaEventDisableTiming));
     if (!sl.out_done) MSA_CUDA(cudaEventCreateWithFlags(&sl.out_done, cudaEventDisableTiming));
@@ -870,6 +878,7 @@ int msa_append_plan_create(msa_handle h, const msa_append *jobs, int32_t n_jobs,
     msa_append_plan ap = new (std::nothrow) msa_append_plan_s();
     if (!ap) return MSA_ERR_INVALID_ARG;
     ap->h = h;
+    ap->device = h->cfg.device;
     std::vector<std::pair<int64_t, int64_t>> spans;      // destination block-table ranges, for the overlap check
     for (int32_t j = 0; j < n_jobs; ++j) {
         const msa_append &a = jobs[j];
@@ -920,7 +929,7 @@ void msa_append_plan_destroy(msa_append_plan ap)
 {
     if (!ap) return;
     if (ap->d_units) {
-        DeviceGuard guard(ap->h->cfg.device);
+        DeviceGuard guard(ap->device);
         cudaFree(ap->d_units);
     }
     delete ap;
@@ -1043,10 +1052,8 @@ extern "C" int msa_forward_static_ws(msa_handle h, msa_plan p, const void *q, in
             g_static_ws_ptr[device] = ptr;
         }
         ws = g_static_ws_ptr[device];
-        // host side of "allocates nothing": the handle's tensor-map table gets its full capacity on the handle's first call here,
-        // so that a later call with a new pointer set appends to it without touching the heap
-        if (h->map_cache.capacity() < kMapCacheEntries) h->map_cache.reserve(kMapCacheEntries);
     }
+    // (host side of "allocates nothing": msa_create reserved the handle's tensor-map table, a new pointer set appends in place)
     return forward_impl(h, p, q, total_q, pool_k, pool_v, num_blocks, block_table, block_table_len, contig_k, contig_v, contig_rows,
                         softmax_scale, o, lse, ws, static_cast<size_t>(MSA_STATIC_WS_BYTES), cuda_stream, false);
 }

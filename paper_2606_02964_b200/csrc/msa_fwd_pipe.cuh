@@ -190,12 +190,13 @@ __device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uin
     const uint32_t src0 = stg + static_cast<uint32_t>(rsub * D + chunk * 16);
     const uint32_t dst0 = dst + static_cast<uint32_t>((chunk >> 2) * kHalfBytes + rsub * 128);
     constexpr int kIters = kVbPerTile * kItPerBlock;
+    const uint32_t mul2 = (mul & 0xffffu) * 0x10001u;      // f16 bits of 2^k in both halves
     auto convert_store = [&](int it, uint32_t w0, uint32_t w1, uint32_t w2, uint32_t w3) {
         const int row0 = (it / kItPerBlock) * kBlock + (it % kItPerBlock) * kRowsPerIt;      // tile row of the iteration's first row
         const uint32_t base = dst0 + static_cast<uint32_t>(row0 * 128);
         const uint32_t x = static_cast<uint32_t>((row0 + rsub) & 7);
-        // F16: the codes' f16 image, unscaled (one cvt per pair); else code * 2^k as bf16
-        auto cv = [mul](uint32_t two) { return F16 ? e4m3x2_to_f16x2(two) : e4m3x2_to_bf16x2(two, mul); };
+        // code * 2^k, exactly: as f16 (F16: one cvt and one packed multiply per pair) or as bf16
+        auto cv = [mul, mul2](uint32_t two) { return F16 ? e4m3x2_to_f16x2(two, mul2) : e4m3x2_to_bf16x2(two, mul); };
         const uint32_t o0 = cv(w0), o1 = cv(w0 >> 16), o2 = cv(w1), o3 = cv(w1 >> 16);
         const uint32_t o4 = cv(w2), o5 = cv(w2 >> 16), o6 = cv(w3), o7 = cv(w3 >> 16);
         asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(base + ((c0 ^ x) << 4)), "r"(o0), "r"(o1), "r"(o2), "r"(o3) : "memory");
@@ -229,7 +230,7 @@ __device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uin
         const bool sw = kLanesPerRow == 8 && (chunk & 4) != 0;
         const uint32_t da = dst_l + ((c0 ^ x) << 4), db = dst_l + (((c0 + 1) ^ x) << 4);
         const uint32_t d0 = sw ? db : da, d1 = sw ? da : db;
-        auto cv = [mul](uint32_t two) { return F16 ? e4m3x2_to_f16x2(two) : e4m3x2_to_bf16x2(two, mul); };
+        auto cv = [mul, mul2](uint32_t two) { return F16 ? e4m3x2_to_f16x2(two, mul2) : e4m3x2_to_bf16x2(two, mul); };
 #pragma unroll
         for (int k0 = 0; k0 < kPerWarp; k0 += 4) {
             uint32_t w[4][4];
@@ -272,23 +273,23 @@ __device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uin
 // and arrives on the staging slot's "empty" barrier; every warp arrives on the ring slot's "full"
 // barrier for every entry.  An entry is waited for even when there is nothing to convert: a waiter that skips a use
 // of a slot cannot tell the phases of its barrier apart.
-// f16 variant: 16-byte chunks [first, n) in steps of stride * 32 of a shared-memory region, bf16 -> f16 in place, times `mult`
-// (a power of two or 1: exact unless the result leaves the f16 range; beyond +-65504 it saturates).
-__device__ __forceinline__ void bf16_to_f16_inplace(uint32_t base, int n_chunks, int first, int stride, int lane, float mult)
+// f16 variant: 16-byte chunks [first, n) in steps of stride * 32 of a shared-memory region, bf16 -> f16 in place (exact for
+// magnitudes in [2^-14, 65504]; beyond +-65504 it saturates, below 2^-14 the value is rounded to a multiple of 2^-24).
+__device__ __forceinline__ void bf16_to_f16_inplace(uint32_t base, int n_chunks, int first, int stride, int lane)
 {
     for (int i = first * 32 + lane; i < n_chunks; i += stride * 32) {
         uint32_t w[4];
         asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "r"(base + i * 16u));
 #pragma unroll
         for (int k = 0; k < 4; ++k)
-            w[k] = pack_f16x2_sat(__uint_as_float(w[k] << 16) * mult, __uint_as_float(w[k] & 0xffff0000u) * mult);
+            w[k] = pack_f16x2_sat(__uint_as_float(w[k] << 16), __uint_as_float(w[k] & 0xffff0000u));
         asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(base + i * 16u), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]) : "memory");
     }
 }
 
-// F16 (the short-query variant, see the kernel): the ring holds f16 tiles.  The codes become their f16 image, the arena
-// blocks of a tile -- loaded as bf16 by the ring loaders, complete on the slot's "direct" barrier -- are rewritten in place
-// as f16 divided by the KV head's scale, and at the start of the unit the Q tile is rewritten as f16 (cw_first / cw_stride:
+// F16 (the short-query variant, see the kernel): the ring holds f16 tiles.  The codes become code * 2^k in f16 (exact for
+// every legal scale), the arena blocks of a tile -- loaded as bf16 by the ring loaders, complete on the slot's "direct"
+// barrier -- are rewritten in place as f16, and at the start of the unit the Q tile is rewritten as f16 (cw_first / cw_stride:
 // this warp's share of that work; cw_first < 0: none).
 template <class C, int D, bool F16>
 __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkUnit &wu, uint32_t bar0, uint32_t sQ, uint32_t sStg,
@@ -306,11 +307,8 @@ __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkU
     const bool pair = wu.mode == kModePair;
     const uint32_t mul_k = __ldg(P.kv8_mul + wu.kvh), mul_v = __ldg(P.kv8_mul + P.Hkv + wu.kvh);
     PROF_DECL();
-    float inv_k = 1.f, inv_v = 1.f;
     if constexpr (F16) {
         if (n <= 0) return;
-        inv_k = __ldg(P.kv8_inv + wu.kvh);
-        inv_v = __ldg(P.kv8_inv + P.Hkv + wu.kvh);
         // Q: bf16 -> f16 in place (the rows that hold tokens; all of them with head-major packing), then "Q ready"
         PROF_T0();
         mbar_wait(bar(kBarQFull), cv_phq);
@@ -318,7 +316,7 @@ __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkU
         const int rows_q = P.token_major ? min(kTileM, (wu.n_tok * P.G + 31) & ~31) : kTileM;     // whole softmax warps
         if (cw_first >= 0) {
 #pragma unroll 1
-            for (int h = 0; h < C::kHalves; ++h) bf16_to_f16_inplace(sQ + h * C::kHalfBytes, rows_q * 8, cw_first, cw_stride, lane, 1.f);
+            for (int h = 0; h < C::kHalves; ++h) bf16_to_f16_inplace(sQ + h * C::kHalfBytes, rows_q * 8, cw_first, cw_stride, lane);
         }
         fence_proxy_async_smem();
         __syncwarp();
@@ -384,7 +382,6 @@ __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkU
             }
             PROF_T0();
             if (m_dir != 0 && cw_first >= 0) {
-                const float mult = is_v ? inv_v : inv_k;
                 const uint32_t tile = sRing + slot * C::kTileBytes;
                 if (m_dir == 0xffu && m_full == 0xffu && cw_stride == kConvWarps) {
                     // a tile of eight full arena blocks (the inside of a recomputed run): the whole slot, flat -- the 64-element
@@ -403,7 +400,7 @@ __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkU
                         for (int k = 0; k < 4; ++k) {
 #pragma unroll
                             for (int j = 0; j < 4; ++j)
-                                w[k][j] = pack_f16x2_sat(__uint_as_float(w[k][j] << 16) * mult, __uint_as_float(w[k][j] & 0xffff0000u) * mult);
+                                w[k][j] = pack_f16x2_sat(__uint_as_float(w[k][j] << 16), __uint_as_float(w[k][j] & 0xffff0000u));
                             asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a0 + (k0 + k) * (kConvWarps * 32 * 16)), "r"(w[k][0]),
                                          "r"(w[k][1]), "r"(w[k][2]), "r"(w[k][3]) : "memory");
                         }
@@ -428,13 +425,13 @@ __device__ __forceinline__ void kv8_convert_unit(const FwdParams &P, const WorkU
                         for (int k = 0; k < kPerLane; ++k) {
 #pragma unroll
                             for (int j = 0; j < 4; ++j)
-                                w[k][j] = pack_f16x2_sat(__uint_as_float(w[k][j] << 16) * mult, __uint_as_float(w[k][j] & 0xffff0000u) * mult);
+                                w[k][j] = pack_f16x2_sat(__uint_as_float(w[k][j] << 16), __uint_as_float(w[k][j] & 0xffff0000u));
                             asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr[k]), "r"(w[k][0]), "r"(w[k][1]), "r"(w[k][2]), "r"(w[k][3]) : "memory");
                         }
                     } else {
 #pragma unroll 1
                         for (int h = 0; h < C::kHalves; ++h)
-                            bf16_to_f16_inplace(tile + h * C::kHalfBytes + b * (kBlock * 128), nv * 8, cw_first, cw_stride, lane, mult);
+                            bf16_to_f16_inplace(tile + h * C::kHalfBytes + b * (kBlock * 128), nv * 8, cw_first, cw_stride, lane);
                     }
                 }
                 fence_proxy_async_smem();
@@ -462,10 +459,10 @@ template <int D, bool KV8, int QT>
 __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_constant__ FwdParams P)
 {
     using C = PipeCfg<D, KV8, QT>;
-    // The fp8 short-query variant multiplies in f16: the codes' exact f16 image is one instruction per pair (the bf16 image costs
-    // four), so Q, the arena blocks of a tile and P are f16 as well -- kind::f16 cannot mix the two formats in one MMA.  The
-    // scales move out of the operands: S is scaled by k_scale through the softmax scale, O by v_scale in the epilogue, the arena
-    // rows are divided by the scale when they are converted (all powers of two: exact).
+    // The fp8 short-query variant multiplies in f16: code * 2^k as an f16 pair is two instructions per pair of codes (the bf16
+    // image costs four) and exact for every legal scale, so Q, the arena blocks of a tile and P are f16 as well -- kind::f16
+    // cannot mix the two formats in one MMA.  Q and the arena rows are converted as they are: what the variant asks of its
+    // inputs (|q|, |arena k / v| <= 65504, include/msa.h) does not depend on the scales.
     constexpr bool F16 = KV8 && QT == 1;
     extern __shared__ __align__(1024) uint8_t smem[];
     const uint32_t sbase = smem_u32(smem);
@@ -540,8 +537,7 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
             if (steps <= 0) continue;
             const int p_row = wu.q_abs0 + (pair ? c * R : 0) + t;
             const int p_min = wu.q_abs0 + (pair ? c * R : 0);
-            // f16 variant: K's scale is not in the operand (the codes are multiplied as they are), it scales S
-            const float sl = F16 ? sl0 * __ldg(P.kv8_scale + wu.kvh) : sl0;
+            const float sl = sl0;
             // Token-major packing: the valid rows of the tile are its first tok * G rows.  A warp whose 32 rows lie beyond
             // them skips the unit's tiles altogether (its rows of S, P and O hold garbage nobody reads); the first warp of
             // the chain gives the idle warps' arrivals on the P barriers along with its own.
@@ -771,7 +767,6 @@ __global__ void __launch_bounds__(512, 1) msa_fwd_pipe_kernel(const __grid_const
                         inv_l = 1.f / lt;
                         lse_val = (mm + log2f(lt)) * 0.6931471805599453f;
                     }
-                    if constexpr (F16) inv_l *= __ldg(P.kv8_scale + P.Hkv + wu.kvh);      // V's scale (the codes were multiplied as they are)
                     w0 *= inv_l;
                     w1 *= inv_l;
                     if (act0) {

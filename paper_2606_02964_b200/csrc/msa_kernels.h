@@ -28,8 +28,6 @@ struct FwdParams {
     const int32_t *tile_writer;      // ... and per context KV tile, q_row0 of the work item that stores it (or -1)
     const int32_t *kv_to_q;          // [Hkv][G] q heads of each kv head
     const uint32_t *kv8_mul;         // fp8 pool only: [2][Hkv] f16 bits of 2^k for K then V, scale = 2^k (see e4m3x2_to_bf16x2)
-    const float *kv8_scale;          // fp8 pool only: [2][Hkv] the scales themselves, K then V, and
-    const float *kv8_inv;            //                [2][Hkv] their reciprocals (both powers of two)
     void *o;                         // bf16 [total_q][Hq][D]
     float *lse;                      // [total_q][Hq]
     float *workspace;

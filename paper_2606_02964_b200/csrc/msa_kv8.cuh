@@ -23,12 +23,16 @@ __device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t two_codes, uint32_
     return r;
 }
 
-// Two codes -> their exact f16 image, unscaled (the short-query variant multiplies in f16 and applies the scales outside the MMAs).
-__device__ __forceinline__ uint32_t e4m3x2_to_f16x2(uint32_t two_codes)
+// Two codes -> code * 2^k as an f16 pair, exactly (the short-query variant multiplies in f16): cvt gives the codes' exact f16
+// image, one packed multiply applies the KV head's scale.  For every legal k in [-14, 7] the product is an f16 -- the
+// largest, 448 * 2^7 = 57344, is below 65504 and the smallest, the subnormal code 2^-9 times 2^-14 = 2^-23, is a multiple of
+// f16's 2^-24 -- so nothing is rounded.  `mul2` = f16 bits of 2^k in both halves.
+__device__ __forceinline__ uint32_t e4m3x2_to_f16x2(uint32_t two_codes, uint32_t mul2)
 {
-    uint32_t h;
+    uint32_t h, r;
     asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(h) : "h"(static_cast<uint16_t>(two_codes)));
-    return h;
+    asm("mul.rn.f16x2 %0, %1, %2;" : "=r"(r) : "r"(h), "r"(mul2));
+    return r;
 }
 
 }  // namespace msa

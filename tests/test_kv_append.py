@@ -69,7 +69,9 @@ def test_append_plan_validation():
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("seed,kw", [(311, dict(Hq=8, Hkv=2, D=128, max_ctx=900, max_q=150)),
-                                     (312, dict(Hq=4, Hkv=4, D=64, max_ctx=300, max_q=33, hybrid=True, n_req=5))])
+                                     (312, dict(Hq=4, Hkv=4, D=64, max_ctx=300, max_q=33, hybrid=True, n_req=5)),
+                                     # an arena row of 4 KB: wider than the bulk-copy kernel's row limit, the plain copy kernel
+                                     (313, dict(Hq=16, Hkv=16, D=128, max_ctx=260, max_q=40, n_req=2))])
 def test_kv_append_matches_the_oracle_bit_for_bit_and_forward_sees_the_same_values(seed, kw):
     dev = "cuda:0"
     p = W.random_problem(seed, device=dev, fill="nan", **kw)

@@ -495,6 +495,26 @@ def test_f3_policy_trace_full_size_plan_aligned_rows():
     _full_config_sampled("f3_policy_trace", 10, 4, 7)
 
 
+def test_plans_may_outlive_their_handle():
+    """msa_plan_destroy / msa_append_plan_destroy after msa_destroy: the plans keep the device ordinal themselves."""
+    from paper_2606_02964_b200 import msa_append_plan_create, msa_append_plan_destroy
+    p = W.random_problem(78, n_req=2, Hq=8, Hkv=2, D=128, max_ctx=300, max_q=40, device=DEV)
+    for _ in range(3):
+        h = msa_create(p.Hq, p.Hkv, p.D, p.q_to_kv)
+        R, n_req, S, n_seg = make_descriptors(p.req, p.seg_kind, p.seg_abs_start, p.seg_len, p.seg_block_off, p.seg_row_off)
+        plan = msa_plan_create(h, R, n_req, S, n_seg)
+        ap = msa_append_plan_create(h, [(0, 20, 0)])
+        msa_destroy(h)
+        junk = [msa_create(4, 2, 64) for _ in range(4)]         # the freed handle's memory is likely to be handed out again
+        msa_plan_destroy(plan)
+        msa_append_plan_destroy(ap)
+        for j in junk:
+            msa_destroy(j)
+    torch.cuda.synchronize()
+    o, lse, _ = gpu_forward(p)                                  # the device is still healthy
+    compare(p, o, lse, strict=False)
+
+
 def test_host_buffer_call_two_steps_in_flight():
     """msa_forward_host_async / _wait on both slots, calls overlapping: every call's O / LSE equal msa_forward's, bit for bit."""
     p = W.random_problem(77, n_req=4, Hq=8, Hkv=2, D=128, max_ctx=900, max_q=120, device=DEV)
