@@ -189,7 +189,7 @@ int msa_workspace_bytes(msa_plan p, size_t *bytes);
  *
  * Rows of q/o/lse not covered by any run are left untouched.  pool/contig pointers may be
  * NULL when the plan references no segment of that kind.  Block ids are trusted (they live
- * on the device); slots past a segment's length and unused blocks may hold anything,
+ * on the device; msa_check_block_ids validates them on request); slots past a segment's length and unused blocks may hold anything,
  * including NaN: they never reach O. */
 int msa_forward(msa_handle h, msa_plan p,
                 const void *q, int64_t total_q,
@@ -295,7 +295,7 @@ void msa_append_plan_destroy(msa_append_plan ap);
 /* Asynchronous on `cuda_stream`, one kernel launch; never allocates or synchronises.  contig_* / pool_* / block_table as
  * in msa_forward, except that the pool is written.  The destination blocks must not be read by a kernel running
  * concurrently on another stream.  MSA_ERR_OUT_OF_RANGE if a job exceeds contig_rows or block_table_len (block ids
- * themselves are trusted, they live on the device); MSA_ERR_MISALIGNED for pointers not 16-byte aligned. */
+ * themselves are trusted, they live on the device -- and here a bad id is a wild write: msa_check_block_ids checks them); MSA_ERR_MISALIGNED for pointers not 16-byte aligned. */
 /* fp8 pool: the rows are quantised on the way, code = E4M3 code nearest to arena value / scale (ties to the even code,
  * |value / scale| > 448 saturates to +-448, NaN gives the NaN code), so that e4m3(code) * scale is what a later PAGED
  * segment reads. */
@@ -333,6 +333,19 @@ int msa_forward_writeback(msa_handle h, msa_plan p,
                           float softmax_scale,
                           void *o, float *lse,
                           void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* ---- Debug check of the block ids (ids live on the device and are validated only on request) ----
+ * msa_forward, msa_forward_writeback and msa_kv_append trust the ids in block_table: the loads and the fused write-back go
+ * through tensor maps, which clip a box that leaves the pool, but msa_kv_append forms global addresses from the ids, so a
+ * bad id there is a wild write.  A caller that wants to be sure runs this first: one small kernel looks at exactly the
+ * block-table entries the plan refers to (the PAGED segments of `p`, its write-back destinations, the jobs of `ap`; either
+ * of p / ap may be NULL, not both) and leaves in *device_flag (device int32) the smallest block-table index whose id is
+ * outside [0, num_blocks), or -1 if all are fine.  Entries the plan does not use are not looked at (they may hold stale
+ * ids).  Asynchronous on `cuda_stream`: read the flag after the stream has caught up.  Never allocates or synchronises.
+ * MSA_ERR_OUT_OF_RANGE if a plan needs more than block_table_len entries. */
+int msa_check_block_ids(msa_handle h, msa_plan p, msa_append_plan ap,
+                        const int32_t *block_table, int64_t block_table_len, int64_t num_blocks,
+                        int32_t *device_flag, void *cuda_stream);
 
 /* Number of kernels the last msa_forward / msa_forward_host on this handle launched. */
 int msa_last_launch_count(msa_handle h);

@@ -6,7 +6,7 @@ in-tree build helper and a ctypes binding with the same names.  No CPU fallback 
 from .binding import (  # noqa: F401
     MSA_OK, MSA_ERR_INVALID_ARG, MSA_ERR_UNSUPPORTED, MSA_ERR_OVERLAP, MSA_ERR_UNSORTED,
     MSA_ERR_OUT_OF_RANGE, MSA_ERR_MISALIGNED, MSA_ERR_WORKSPACE, MSA_ERR_CUDA, MSA_ERR_NO_DEVICE,
-    MSA_ERR_STATIC_WS, MSA_STATIC_WS_BYTES, msa_forward_static_ws,
+    MSA_ERR_STATIC_WS, MSA_STATIC_WS_BYTES, msa_forward_static_ws, msa_check_block_ids,
     MSA_SEG_PAGED, MSA_SEG_CONTIG, MSA_SEG_SELF, MSA_POOL_BF16, MSA_POOL_FP8_E4M3,
     MsaError, MsaSession, MsaEvictor, make_descriptors,
     msa_create, msa_destroy, msa_plan_create, msa_plan_destroy, msa_plan_get_info, msa_plan_export,

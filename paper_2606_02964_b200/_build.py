@@ -8,7 +8,7 @@ import sys
 _PKG = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_PKG, "csrc")
 LIB_PATH = os.path.join(_PKG, "libmsa.so")
-SOURCES = ["msa_api.cu", "msa_fwd.cu", "msa_merge.cu", "msa_append.cu", "msa_dequant.cu", "msa_planner.cpp", "msa_evictor.cpp"]
+SOURCES = ["msa_api.cu", "msa_fwd.cu", "msa_merge.cu", "msa_append.cu", "msa_dequant.cu", "msa_check.cu", "msa_planner.cpp", "msa_evictor.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--shared", "-cudart", "static"]
 

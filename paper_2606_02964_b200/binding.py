@@ -64,7 +64,7 @@ EXPORTS = ["msa_create", "msa_destroy", "msa_plan_create", "msa_plan_destroy", "
            "msa_last_launch_count", "msa_set_timing", "msa_get_timing", "msa_strerror", "msa_last_cuda_error", "msa_version",
            "msa_append_plan_create", "msa_append_plan_destroy", "msa_kv_append",
            "msa_plan_create_writeback", "msa_forward_writeback", "msa_forward_host_async", "msa_forward_host_wait",
-           "msa_forward_static_ws"]
+           "msa_forward_static_ws", "msa_check_block_ids"]
 EVICTOR_EXPORTS = ["msa_evictor_create", "msa_evictor_destroy", "msa_evictor_add", "msa_evictor_remove", "msa_evictor_evict",
                    "msa_evictor_evict_linear", "msa_evictor_set_lambda", "msa_evictor_size", "msa_evictor_weight"]
 
@@ -101,6 +101,7 @@ def _lib() -> ctypes.CDLL:
         lib.msa_forward_static_ws.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, i64, f32, vp, vp, vp]
         lib.msa_forward_host_async.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, i64, f32, vp, vp, vp, i32]
         lib.msa_forward_host_wait.argtypes = [vp, i32]
+        lib.msa_check_block_ids.argtypes = [vp, vp, vp, vp, i64, i64, vp, vp]
         lib.msa_last_launch_count.argtypes = [vp]
         lib.msa_set_timing.argtypes = [vp, ctypes.c_int]
         lib.msa_get_timing.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(ctypes.c_double),
@@ -290,6 +291,13 @@ def msa_forward_host_async(h, p, q_host, pool_k, pool_v, block_table_host, conti
 
 def msa_forward_host_wait(h, slot: int = 0) -> None:
     _check(_lib().msa_forward_host_wait(h, slot), "msa_forward_host_wait")
+
+
+def msa_check_block_ids(h, plan, append_plan, block_table, num_blocks: int, flag, stream: Optional[int] = None) -> None:
+    """Debug check: flag (int32 CUDA tensor, 1 element) <- smallest block-table index the plan(s) refer to whose id is outside
+    [0, num_blocks), or -1.  Asynchronous on `stream`."""
+    _check(_lib().msa_check_block_ids(h, plan, append_plan, _dptr(block_table), int(block_table.numel()), int(num_blocks),
+                                      _dptr(flag), stream), "msa_check_block_ids")
 
 
 def msa_last_launch_count(h) -> int:

@@ -967,6 +967,40 @@ int msa_kv_append(msa_handle h, msa_append_plan ap, const void *contig_k, const 
     return MSA_OK;
 }
 
+int msa_check_block_ids(msa_handle h, msa_plan p, msa_append_plan ap, const int32_t *block_table, int64_t block_table_len,
+                        int64_t num_blocks, int32_t *device_flag, void *cuda_stream)
+{
+    if (!h || (!p && !ap) || (p && p->h != h) || (ap && ap->h != h)) return MSA_ERR_INVALID_ARG;
+    if (h->planning_only) return MSA_ERR_NO_DEVICE;
+    if (!block_table || !device_flag || block_table_len < 0 || num_blocks < 0) return MSA_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(block_table) & 3u) || (reinterpret_cast<uintptr_t>(device_flag) & 3u)) return MSA_ERR_MISALIGNED;
+    CheckParams cp;
+    memset(&cp, 0, sizeof cp);
+    if (p) {
+        const HostPlan &hp = p->hp;
+        if (hp.uses_paged && hp.info.max_block_table_index >= block_table_len) return MSA_ERR_OUT_OF_RANGE;
+        if (hp.has_writeback && hp.wb_max_bt >= block_table_len) return MSA_ERR_OUT_OF_RANGE;
+        cp.vblocks = p->d_vblocks;
+        cp.n_vblocks = static_cast<int32_t>(hp.vblocks.size());
+        if (hp.has_writeback) {
+            cp.vb_dst = p->d_vb_dst;
+            cp.n_vb_dst = static_cast<int32_t>(hp.vb_dst.size());
+        }
+    }
+    if (ap) {
+        if (ap->max_bt >= block_table_len) return MSA_ERR_OUT_OF_RANGE;
+        cp.units = ap->d_units;
+        cp.n_units = static_cast<int32_t>(ap->units.size());
+    }
+    cp.block_table = block_table;
+    cp.num_blocks = num_blocks;
+    cp.flag = device_flag;
+    DeviceGuard guard(h->cfg.device);
+    if (guard.err != cudaSuccess) return cuda_fail(guard.err, "msa_check_block_ids: cudaSetDevice");
+    MSA_CUDA(launch_check_ids(cp, static_cast<cudaStream_t>(cuda_stream)));
+    return MSA_OK;
+}
+
 int msa_last_launch_count(msa_handle h) { return h ? h->last_launches : 0; }
 
 int msa_set_timing(msa_handle h, int max_steps)

@@ -37,40 +37,9 @@
 #include "msa_ptx.cuh"
 #include "msa_softmax.cuh"
 #include "msa_kv8.cuh"
+#include "msa_prof.cuh"      // PROF_* hooks: empty unless built with -DMSA_PROF (never the shipped library)
 
 namespace msa {
-
-// Optional role-level cycle counters (build with -DMSA_PROF; never in the shipped library):
-// lane 0 of one warp per role accumulates clock64() deltas into g_prof[cta][slot].
-#ifdef MSA_PROF
-__device__ unsigned long long g_prof[160][32];
-__device__ long long g_trace[4][64][12];
-#define PROF_TRACE(role, step, ev) \
-    do { if (blockIdx.x == 0 && u == u_begin && (step) < 64) g_trace[role][step][ev] = clock64(); } while (0)
-#if MSA_PROF == 2   /* event trace only: no accumulators in the hot loops */
-#define PROF_DECL()
-#define PROF_T0()
-#define PROF_ADD(slot)
-#define PROF_INC(slot, v)
-#define PROF_FLUSH(lo, hi)
-#else
-#define PROF_DECL() unsigned long long prof_acc[32] = {}
-#define PROF_T0() const long long prof_t0_ = clock64()
-#define PROF_ADD(slot) prof_acc[slot] += static_cast<unsigned long long>(clock64() - prof_t0_)
-#define PROF_INC(slot, v) prof_acc[slot] += static_cast<unsigned long long>(v)
-#define PROF_FLUSH(lo, hi)                                                             \
-    do {                                                                               \
-        _Pragma("unroll") for (int i_ = (lo); i_ < (hi); ++i_) g_prof[blockIdx.x][i_] += prof_acc[i_]; \
-    } while (0)
-#endif
-#else
-#define PROF_TRACE(role, step, ev)
-#define PROF_DECL()
-#define PROF_T0()
-#define PROF_ADD(slot)
-#define PROF_INC(slot, v)
-#define PROF_FLUSH(lo, hi)
-#endif
 
 template <int D, bool KV8 = false, int QT = 2>
 struct PipeCfg {
@@ -115,11 +84,7 @@ enum PipeBar : int {
 };
 constexpr int kConvWarps = 4;          // KV8: warps 8-11 convert (and, per unit, do the epilogue)
 
-#ifdef MSA_NO_WRITEBACK           /* A/B builds only: the ring without its second "empty" arrival */
-constexpr bool kWritebackRing = false;
-#else
-constexpr bool kWritebackRing = true;
-#endif
+constexpr bool kWritebackRing = true;  // the ring's "empty" barriers take a second arrival (the loader, or the write-back warp)
 constexpr uint32_t kNamedStFull = 1;   // named barriers 1, 2: (l, ref) of chain 0 / 1 are in shared memory (128 + 128 threads)
 
 struct RingPos {
@@ -208,9 +173,6 @@ __device__ __forceinline__ void kv8_convert_tile(uint32_t stg, uint32_t dst, uin
                      : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3)
                      : "r"(src0 + static_cast<uint32_t>(row0 * D)));
     };
-#ifdef MSA_KV8_SKIP_CONVERT           /* timing experiments only: wrong results */
-    return;
-#endif
     const bool all_full = m_paged == 0xffu && __all_sync(0xffffffffu, lane >= kVbPerTile || (nvp & 0xff) == kBlock);
     if (all_full && even_w >= 0) {
         // The common tile (eight full cached blocks), iterations dealt out evenly: warp w takes w, w + 4, ...  Four

@@ -77,6 +77,18 @@ struct DequantParams {
 };
 cudaError_t launch_dequant(const DequantParams &p, int num_sms, cudaStream_t stream);
 
+// Block-id check (msa_check.cu): entries of the block table a plan refers to
+struct CheckParams {
+    const VBlock *vblocks;        // forward plan: its virtual blocks (paged entries name a block-table index), or NULL
+    const int32_t *vb_dst;        // write-back plan: destination block-table index per virtual block or -1, or NULL
+    const AppendUnit *units;      // append plan: its copy units, or NULL
+    int32_t n_vblocks, n_vb_dst, n_units;
+    const int32_t *block_table;
+    int64_t num_blocks;
+    int32_t *flag;                // device int32: smallest offending block-table index, or -1
+};
+cudaError_t launch_check_ids(const CheckParams &p, cudaStream_t stream);
+
 cudaError_t configure_append();   // per device, like configure_fwd
 cudaError_t launch_append(const AppendParams &p, int num_sms, cudaStream_t stream);
 

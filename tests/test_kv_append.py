@@ -212,3 +212,55 @@ def test_forward_writeback_is_forward_plus_kv_append_bit_for_bit(seed, kw):
     msa_plan_destroy(plain)
     msa_plan_destroy(plan)
     msa_destroy(h)
+
+
+# ------------------------------------------------------------------ debug check of the block ids
+@pytest.mark.gpu
+def test_check_block_ids_flags_the_smallest_bad_entry_a_plan_refers_to():
+    """msa_check_block_ids (SURVEY.md 8(b) debug mode): -1 on a good table; the smallest offending block-table index when ids the
+    plan refers to are negative or >= num_blocks; entries the plan does not use are ignored; forward and append plans alike."""
+    from paper_2606_02964_b200 import msa_check_block_ids
+    dev = "cuda:0"
+    p = W.random_problem(321, n_req=3, Hq=8, Hkv=2, D=128, max_ctx=700, max_q=60, device=dev)
+    h = msa_create(p.Hq, p.Hkv, p.D, p.q_to_kv)
+    R, n, S, m = make_descriptors(p.req, p.seg_kind, p.seg_abs_start, p.seg_len, p.seg_block_off, p.seg_row_off)
+    plan = msa_plan_create(h, R, n, S, m)
+    vb = msa_plan_export(plan, 0)
+    used = np.unique(vb["src"][(vb["paged"] != 0) & (vb["nvalid"] > 0)])
+    assert len(used) >= 4
+    nb = int(p.pool_k.shape[0])
+    pad = 5                                                         # entries beyond the plan's: never looked at
+    bt = torch.cat([p.block_table, torch.full((pad,), 10 ** 9, dtype=torch.int32, device=dev)])
+    flag = torch.zeros(1, dtype=torch.int32, device=dev)
+    st = torch.cuda.current_stream().cuda_stream
+
+    def check(table, plan_=plan, ap_=None):
+        msa_check_block_ids(h, plan_, ap_, table, nb, flag, st)
+        torch.cuda.synchronize()
+        return int(flag.item())
+
+    assert check(bt) == -1
+    lo, hi = int(used[1]), int(used[-2])
+    bad = bt.clone()
+    bad[hi] = nb                                                    # one past the pool
+    assert check(bad) == hi
+    bad[lo] = -3
+    assert check(bad) == lo                                         # the smallest offending index
+    unused = sorted(set(range(int(p.block_table.numel()))) - set(int(x) for x in used))
+    if unused:
+        only_unused = bt.clone()
+        only_unused[unused[0]] = -1
+        assert check(only_unused) == -1
+    with pytest.raises(MsaError) as e:
+        msa_check_block_ids(h, plan, None, bt[: int(used[-1])], nb, flag, st)
+    assert e.value.status == MSA_ERR_OUT_OF_RANGE
+    # an append plan: jobs into entries [2, 5) of a table of their own
+    ap = msa_append_plan_create(h, [(0, 40, 2)])
+    tbl = torch.tensor([10 ** 9, -7, 3, 1, 0, 10 ** 9], dtype=torch.int32, device=dev)
+    assert check(tbl, None, ap) == -1
+    tbl[4] = nb
+    assert check(tbl, None, ap) == 4
+    assert check(bt, plan, None) == -1
+    msa_append_plan_destroy(ap)
+    msa_plan_destroy(plan)
+    msa_destroy(h)
