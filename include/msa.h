@@ -44,8 +44,7 @@ enum {
     MSA_ERR_INVALID_ARG = -1,      /* NULL pointer, negative size, non-positive / non-finite scale */
     MSA_ERR_UNSUPPORTED = -2,      /* head_dim not in {64,128}, block_size != 16, Hq % Hkv != 0, G > 16,
                                       head map that does not give every KV head exactly G q heads, an fp8 pool
-                                      scale that is not a power of two in [2^-14, 2^7], KV write-back into an
-                                      fp8 pool through the forward launch */
+                                      scale that is not a power of two in [2^-14, 2^7] */
     MSA_ERR_OVERLAP = -3,          /* segments of one request overlap in absolute position, or two
                                       requests write the same q rows */
     MSA_ERR_UNSORTED = -4,         /* segments of one request not in ascending abs_start */
@@ -321,7 +320,12 @@ int msa_kv_append(msa_handle h, msa_append_plan ap,
  * completed on the stream, pool[block_table[job.block_off + i/16]][i%16] = arena[job.row_off + i] for every job, bit for
  * bit, and O / LSE are bit-identical to msa_forward on the same plan.  The destination blocks must not be read by this
  * or any concurrently running call.  MSA_ERR_INVALID_ARG if the plan has no write-back jobs; MSA_ERR_OUT_OF_RANGE if a
- * job's block-table slice exceeds block_table_len.  msa_forward on a write-back plan computes O / LSE only. */
+ * job's block-table slice exceeds block_table_len.  msa_forward on a write-back plan computes O / LSE only.
+ *
+ * fp8 pool: the same two calls work, but the store is not fused -- the forward kernel moves bf16 tiles as they are and cannot
+ * quantise them -- so msa_forward_writeback issues the forward kernel and then msa_kv_append's quantising kernel on the
+ * same stream (one more launch; the bytes written are those of msa_kv_append, O / LSE those of msa_forward).  The
+ * restrictions on the jobs above do not apply there; the validation is msa_append_plan_create's. */
 int msa_plan_create_writeback(msa_handle h, const msa_request *requests, int32_t n_req,
                               const msa_segment *segments, int32_t n_seg,
                               const msa_append *jobs, int32_t n_jobs, msa_plan *out);

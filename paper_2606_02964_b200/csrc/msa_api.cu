@@ -144,6 +144,9 @@ struct msa_plan_s {
     const int32_t *d_deq_src = nullptr;
     const VBlock *d_vblocks_deq = nullptr;
     size_t ws_partials = 0, ws_pool = 0, ws_ident = 0;     // workspace layout in bytes: [partials | copy of K | copy of V | identity table]
+    // fp8 pool, write-back plans: the jobs as an append plan of the plan's own -- msa_forward_writeback runs the quantising
+    // msa_kv_append kernel behind the forward kernel (the fused store moves bf16 tiles as they are and cannot quantise)
+    struct msa_append_plan_s *wb_append = nullptr;
 };
 
 struct msa_append_plan_s {
@@ -328,7 +331,20 @@ int msa_plan_create_writeback(msa_handle h, const msa_request *requests, int32_t
                               int32_t n_seg, const msa_append *jobs, int32_t n_jobs, msa_plan *out)
 {
     if (n_jobs < 0 || (n_jobs > 0 && !jobs)) return MSA_ERR_INVALID_ARG;
-    if (h && h->kv8 && n_jobs > 0) return MSA_ERR_UNSUPPORTED;   // the fused write-back stores bf16 tiles as they are: use msa_kv_append
+    if (h && h->kv8 && n_jobs > 0) {
+        // fp8 pool: the same call, two launches (forward kernel, then the quantising append kernel on the same stream)
+        if (!out) return MSA_ERR_INVALID_ARG;
+        msa_append_plan ap = nullptr;
+        int rc = msa_append_plan_create(h, jobs, n_jobs, &ap);
+        if (rc != MSA_OK) return rc;
+        rc = plan_create(h, requests, n_req, segments, n_seg, nullptr, 0, out);
+        if (rc != MSA_OK) {
+            msa_append_plan_destroy(ap);
+            return rc;
+        }
+        (*out)->wb_append = ap;
+        return MSA_OK;
+    }
     return plan_create(h, requests, n_req, segments, n_seg, jobs, n_jobs, out);
 }
 
@@ -471,6 +487,7 @@ extern "C" {
 void msa_plan_destroy(msa_plan p)
 {
     if (!p) return;
+    if (p->wb_append) msa_append_plan_destroy(p->wb_append);
     if (p->d_buf) {
         DeviceGuard guard(p->device);
         cudaFree(p->d_buf);
@@ -652,8 +669,22 @@ int forward_impl(msa_handle h, msa_plan p, const void *q, int64_t total_q, const
     if (h->planning_only) return MSA_ERR_NO_DEVICE;
     h->last_launches = 0;
     const HostPlan &hp = p->hp;
+    if (writeback && h->kv8) {
+        // fp8 pool: forward (no fused store), then the plan's own append plan through the quantising kernel, same stream
+        if (!p->wb_append) return MSA_ERR_INVALID_ARG;
+        if (!pool_k || !pool_v || !block_table || num_blocks < 1) return MSA_ERR_INVALID_ARG;
+        if (p->wb_append->max_bt >= block_table_len || p->wb_append->max_row >= contig_rows) return MSA_ERR_OUT_OF_RANGE;
+        int rc = forward_impl(h, p, q, total_q, pool_k, pool_v, num_blocks, block_table, block_table_len, contig_k, contig_v,
+                              contig_rows, softmax_scale, o, lse, workspace, workspace_bytes, cuda_stream, false);
+        if (rc != MSA_OK) return rc;
+        const int fwd_launches = h->last_launches;
+        rc = msa_kv_append(h, p->wb_append, contig_k, contig_v, contig_rows, const_cast<void *>(pool_k), const_cast<void *>(pool_v),
+                           num_blocks, block_table, block_table_len, cuda_stream);
+        if (rc != MSA_OK) return rc;
+        h->last_launches += fwd_launches;
+        return MSA_OK;
+    }
     if (writeback) {
-        if (h->kv8) return MSA_ERR_UNSUPPORTED;
         if (!hp.has_writeback) return MSA_ERR_INVALID_ARG;          // the plan must come from msa_plan_create_writeback
         if (!pool_k || !pool_v || !block_table || num_blocks < 1 || num_blocks * MSA_BLOCK_SIZE > 0x7fffffffLL) return MSA_ERR_INVALID_ARG;
         if (hp.wb_max_bt >= block_table_len) return MSA_ERR_OUT_OF_RANGE;

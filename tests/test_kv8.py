@@ -39,13 +39,17 @@ def test_scales_must_be_powers_of_two_within_range():
     assert e.value.status == MSA_ERR_INVALID_ARG
 
 
-def test_fused_writeback_is_refused_on_an_fp8_pool():
+def test_writeback_plan_on_an_fp8_pool_validates_like_an_append_plan():
+    """An fp8 handle accepts write-back plans (forward kernel + quantising append kernel in one call); bad jobs are refused."""
+    from paper_2606_02964_b200 import MSA_ERR_OVERLAP, msa_plan_destroy
     h = msa_create(4, 2, 64, device=-1, pool_format=MSA_POOL_FP8_E4M3)
     R, n_req, S, n_seg = make_descriptors(np.array([[0, 16, 16, 0, 2]], np.int32), [SEG_PAGED, SEG_SELF], [0, 16], [16, 16],
                                           [0, 0], [0, 0])
-    with pytest.raises(MsaError) as e:
-        msa_plan_create_writeback(h, R, n_req, S, n_seg, [(0, 16, 1)])
-    assert e.value.status == MSA_ERR_UNSUPPORTED
+    msa_plan_destroy(msa_plan_create_writeback(h, R, n_req, S, n_seg, [(0, 16, 1)]))
+    for jobs, code in (([(0, 16, 1), (0, 16, 1)], MSA_ERR_OVERLAP), ([(0, 0, 1)], MSA_ERR_INVALID_ARG)):
+        with pytest.raises(MsaError) as e:
+            msa_plan_create_writeback(h, R, n_req, S, n_seg, jobs)
+        assert e.value.status == code
     msa_destroy(h)
 
 
@@ -372,6 +376,48 @@ def test_kv8_append_quantises_like_the_oracle_and_feeds_the_forward(Hq, Hkv, D):
     p2.seg_kind, p2.seg_block_off, p2.num_blocks = kind2, boff2, n_pool + extra
     o, lse, _ = gpu_forward(p2)
     compare(p2, o, lse, strict=False)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("want", ["prepass", "kernel_pair", "kernel_split"])
+def test_kv8_forward_writeback_is_forward_plus_quantising_append(want):
+    """msa_forward_writeback on an fp8 handle: O / LSE bit-identical to msa_forward, and the pool afterwards holds, byte for
+    byte, the oracle quantiser's codes of the arena rows where the oracle's write-back puts them (canary everywhere else)."""
+    from paper_2606_02964_b200 import msa_forward_writeback, msa_last_launch_count, msa_plan_destroy, msa_workspace_bytes
+    p8 = W.to_fp8_pool(_three_paths(DEV)[want], k_exp=[-6, -4], v_exp=[-5, -7])
+    bt = p8.block_table_np
+    n_pool, extra_rows = int(p8.pool_k.shape[0]), []
+    jobs, cursor = [], len(bt)
+    for s_ in range(len(p8.seg_kind)):
+        if int(p8.seg_kind[s_]) != SEG_PAGED:
+            n = int(p8.seg_len[s_])
+            jobs.append((int(p8.seg_row_off[s_]), n, cursor))
+            cursor += (n + 15) // 16
+    extra = cursor - len(bt)
+    bt2 = np.concatenate([bt, (n_pool + np.random.default_rng(6).permutation(extra)).astype(np.int32)])
+    canary = 0x5a
+    grow = lambda t: torch.cat([t, torch.full((extra,) + tuple(t.shape[1:]), canary, dtype=torch.uint8, device=DEV)])
+    pool_k, pool_v = grow(p8.pool_k), grow(p8.pool_v)
+    start_k, start_v = pool_k.cpu().numpy(), pool_v.cpu().numpy()
+    bt2_d = torch.from_numpy(bt2).to(DEV)
+    with MsaSession(p8) as s:
+        o_ref, l_ref = s.forward()
+        o_ref, l_ref, n_fwd = o_ref.clone(), l_ref.clone(), msa_last_launch_count(s.h)
+        R, n_req, S, n_seg = make_descriptors(p8.req, p8.seg_kind, p8.seg_abs_start, p8.seg_len, p8.seg_block_off, p8.seg_row_off)
+        plan = msa_plan_create_writeback(s.h, R, n_req, S, n_seg, jobs)
+        nb = msa_workspace_bytes(plan)
+        ws = torch.empty(max(nb, 16), dtype=torch.uint8, device=DEV)
+        o, lse = torch.zeros_like(o_ref), torch.zeros_like(l_ref)
+        msa_forward_writeback(s.h, plan, p8.q, pool_k, pool_v, bt2_d, p8.contig_k, p8.contig_v, p8.scale, o, lse, ws,
+                              torch.cuda.current_stream().cuda_stream)
+        assert msa_last_launch_count(s.h) == n_fwd + 1
+        torch.cuda.synchronize()
+        msa_plan_destroy(plan)
+    assert torch.equal(o, o_ref) and torch.equal(lse, l_ref)
+    for pool, start, arena, scales in ((pool_k, start_k, p8.contig_k, p8.k_scale), (pool_v, start_v, p8.contig_v, p8.v_scale)):
+        a = arena.float().cpu().double().numpy()
+        codes = np.stack([quantize_e4m3(a[:, hh, :], float(scales[hh]), oracle.e4m3_to_double) for hh in range(p8.Hkv)], axis=1)
+        assert np.array_equal(pool.cpu().numpy(), kv_append(start, codes, bt2, jobs))
 
 
 @pytest.mark.gpu
