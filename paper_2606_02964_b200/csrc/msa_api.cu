@@ -1007,6 +1007,8 @@ int msa_check_block_ids(msa_handle h, msa_plan p, msa_append_plan ap, const int3
     if ((reinterpret_cast<uintptr_t>(block_table) & 3u) || (reinterpret_cast<uintptr_t>(device_flag) & 3u)) return MSA_ERR_MISALIGNED;
     CheckParams cp;
     memset(&cp, 0, sizeof cp);
+    msa_append_plan own = p ? p->wb_append : nullptr;        // fp8 write-back plan: its destinations are an append plan of its own
+    if (own && own->max_bt >= block_table_len) return MSA_ERR_OUT_OF_RANGE;
     if (p) {
         const HostPlan &hp = p->hp;
         if (hp.uses_paged && hp.info.max_block_table_index >= block_table_len) return MSA_ERR_OUT_OF_RANGE;
@@ -1028,7 +1030,17 @@ int msa_check_block_ids(msa_handle h, msa_plan p, msa_append_plan ap, const int3
     cp.flag = device_flag;
     DeviceGuard guard(h->cfg.device);
     if (guard.err != cudaSuccess) return cuda_fail(guard.err, "msa_check_block_ids: cudaSetDevice");
-    MSA_CUDA(launch_check_ids(cp, static_cast<cudaStream_t>(cuda_stream)));
+    MSA_CUDA(launch_check_ids(cp, true, static_cast<cudaStream_t>(cuda_stream)));
+    if (own) {
+        CheckParams c2;
+        memset(&c2, 0, sizeof c2);
+        c2.units = own->d_units;
+        c2.n_units = static_cast<int32_t>(own->units.size());
+        c2.block_table = block_table;
+        c2.num_blocks = num_blocks;
+        c2.flag = device_flag;
+        MSA_CUDA(launch_check_ids(c2, false, static_cast<cudaStream_t>(cuda_stream)));
+    }
     return MSA_OK;
 }
 

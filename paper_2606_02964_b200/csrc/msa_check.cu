@@ -26,9 +26,10 @@ __global__ void __launch_bounds__(256) msa_check_ids_kernel(const CheckParams P)
     }
 }
 
-cudaError_t launch_check_ids(const CheckParams &p, cudaStream_t stream)
+// reset: start the flag at -1 (a second launch that adds another set of entries to the same verdict passes false)
+cudaError_t launch_check_ids(const CheckParams &p, bool reset, cudaStream_t stream)
 {
-    cudaError_t e = cudaMemsetAsync(p.flag, 0xff, sizeof(int32_t), stream);
+    cudaError_t e = reset ? cudaMemsetAsync(p.flag, 0xff, sizeof(int32_t), stream) : cudaSuccess;
     if (e != cudaSuccess) return e;
     const int n_total = p.n_vblocks + p.n_vb_dst + p.n_units;
     if (n_total <= 0) return cudaSuccess;

@@ -87,7 +87,7 @@ struct CheckParams {
     int64_t num_blocks;
     int32_t *flag;                // device int32: smallest offending block-table index, or -1
 };
-cudaError_t launch_check_ids(const CheckParams &p, cudaStream_t stream);
+cudaError_t launch_check_ids(const CheckParams &p, bool reset, cudaStream_t stream);
 
 cudaError_t configure_append();   // per device, like configure_fwd
 cudaError_t launch_append(const AppendParams &p, int num_sms, cudaStream_t stream);

@@ -264,3 +264,23 @@ def test_check_block_ids_flags_the_smallest_bad_entry_a_plan_refers_to():
     msa_append_plan_destroy(ap)
     msa_plan_destroy(plan)
     msa_destroy(h)
+    # write-back plans: the destinations count as well -- fused store (bf16 pool) and the fp8 pool's append plan
+    from paper_2606_02964_b200 import MSA_POOL_FP8_E4M3
+    p = W.random_problem(331, device=dev, Hq=8, Hkv=2, D=128, max_ctx=900, max_q=150)
+    jobs, bt2, extra, _, _ = _jobs_and_redescription(p)
+    nb2 = int(p.pool_k.shape[0]) + extra
+    R, n, S, m = make_descriptors(p.req, p.seg_kind, p.seg_abs_start, p.seg_len, p.seg_block_off, p.seg_row_off)
+    first_dst = int(jobs[0][2])
+    for fmt in (0, MSA_POOL_FP8_E4M3):
+        h = msa_create(p.Hq, p.Hkv, p.D, p.q_to_kv, pool_format=fmt)
+        plan = msa_plan_create_writeback(h, R, n, S, m, jobs)
+        tbl = torch.from_numpy(bt2).to(dev)
+        msa_check_block_ids(h, plan, None, tbl, nb2, flag, st)
+        torch.cuda.synchronize()
+        assert int(flag.item()) == -1
+        tbl[first_dst + 1] = nb2 + 4                                # a destination block beyond the pool
+        msa_check_block_ids(h, plan, None, tbl, nb2, flag, st)
+        torch.cuda.synchronize()
+        assert int(flag.item()) == first_dst + 1, fmt
+        msa_plan_destroy(plan)
+        msa_destroy(h)
