@@ -88,6 +88,30 @@ def test_static_workspace_calls_in_a_row_match_msa_forward():
 
 
 @pytest.mark.gpu
+def test_static_workspace_on_an_fp8_handle_and_a_side_stream():
+    """An fp8 prefill plan keeps, besides the partials, the bf16 copy of its cached blocks and the copy's block table in the
+    workspace (written by the dequantising pre-pass of the same call): through the built-in array, on a stream that is not
+    the default one, twice in a row -- bit-identical to msa_forward with a caller workspace."""
+    ctx = ContextSpec([(SEG_PAGED, 0, 500), (SEG_CONTIG, 500, 100), (SEG_SELF, 600, 300)])
+    p = build_problem("static_ws_fp8", 8, 2, 128, [ctx], [RunSpec(0, 600, 300)], seed=34, device=DEV)
+    p8 = W.to_fp8_pool(p, k_exp=[-6, -4], v_exp=[-5, -7])
+    side = torch.cuda.Stream()
+    with MsaSession(p8) as s:
+        need = msa_workspace_bytes(s.plan)
+        assert 2 * 32 * 16 * p8.Hkv * p8.D * 2 <= need <= MSA_STATIC_WS_BYTES          # the copy of 32 cached blocks is in there
+        ro, rl = _existing_path(s)
+        for _ in range(2):
+            o = torch.full_like(s.o, float("nan"))
+            lse = torch.full_like(s.lse, float("nan"))
+            side.wait_stream(torch.cuda.current_stream())
+            msa_forward_static_ws(s.h, s.plan, p8.q, p8.pool_k, p8.pool_v, p8.block_table, p8.contig_k, p8.contig_v, p8.scale,
+                                  o, lse, side.cuda_stream)
+            assert msa_last_launch_count(s.h) >= 2                                  # pre-pass + forward kernel (+ merge)
+            side.synchronize()
+            assert torch.equal(o, ro) and torch.equal(lse, rl)
+
+
+@pytest.mark.gpu
 def test_static_workspace_refuses_a_plan_beyond_its_size():
     """An fp8 prefill plan dequantises the cached blocks it refers to into the workspace: 640 blocks x 64 KiB > 32 MiB."""
     Hq, Hkv, D, L, T = 32, 8, 128, 640 * 16, 512
