@@ -34,6 +34,22 @@ def test_library_exports_every_declared_symbol():
     assert set(binding.EVICTOR_EXPORTS) == declared2
 
 
+def test_binding_constants_equal_the_headers():
+    """Status codes, segment kinds, pool formats and MSA_STATIC_WS_BYTES of binding.py against include/msa.h, and every status
+    code has a text of its own."""
+    hdr = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "msa.h")).read(), flags=re.S)
+    enums = {k: int(v) for k, v in re.findall(r"\b(MSA_[A-Z0-9_]+)\s*=\s*(-?\d+)", hdr)}
+    assert len([k for k in enums if k.startswith("MSA_ERR_")]) == 10 and enums["MSA_OK"] == 0
+    for name, value in enums.items():
+        assert getattr(binding, name) == value, name
+    m = re.search(r"#define\s+MSA_STATIC_WS_BYTES\s+\((\d+)u\s*<<\s*(\d+)\)", hdr)
+    assert m and binding.MSA_STATIC_WS_BYTES == int(m.group(1)) << int(m.group(2))
+    lib = binding._lib()
+    texts = [lib.msa_strerror(v).decode() for k, v in enums.items() if k.startswith("MSA_ERR_") or k == "MSA_OK"]
+    assert len(set(texts)) == len(texts) and "unknown status" not in texts
+    assert lib.msa_strerror(-99).decode() == "unknown status"
+
+
 def test_create_rejects_unsupported_shapes_and_reports_no_device():
     for args in [(32, 8, 96), (30, 8, 128), (64, 2, 128)]:          # head_dim, divisibility, G > 16
         with pytest.raises(MsaError) as e:
