@@ -223,7 +223,8 @@ int msa_forward(msa_handle h, msa_plan p,
  * The call itself allocates no device memory and frees none (no cudaMalloc / cudaFree / cudaMallocAsync, no library
  * routine that allocates; msa_create and msa_plan_create, which own small device buffers, are set-up calls and are not
  * covered by this promise).  The FIRST call on a device does a one-time set-up: it looks up the array's device address
- * (which makes the CUDA runtime load that part of the library, and that is where the 32 MiB are actually reserved).
+ * (with the CUDA runtime's default lazy module loading this is also the moment that part of the library is loaded on the
+ * device and the 32 MiB are actually reserved; with CUDA_MODULE_LOADING=EAGER that happens when the context is created).
  * Make that first call at start-up, on any small split-KV or ordinary plan, before the engine takes the rest of the
  * memory and before any stream capture is begun.
  *
